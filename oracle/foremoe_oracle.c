@@ -1,0 +1,394 @@
+/*
+ * foremoe_oracle.c -- plain, slow, single-threaded CPU restatement of the ForeMoE micro-step
+ * plan + dispatch + combine path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build, load or call this file.  It shares no code, header, table or helper with the CUDA path
+ * (paper_2606_11867_b200/csrc); the product never routes through it.
+ *
+ * Every function is the definition written out (histogram, stable counting sort, row copy,
+ * weighted sum) or, for the Stage-4 token assignment the paper only sketches, the algorithm step
+ * by step in the paper's order: "assign each token unit to the replica whose rank has the
+ * smallest accumulated load" (Alg. 3 lines 18-21; App. D),
+ * iterated "until the replicas' ranks converge toward equal utilization", with the
+ * readings of DESIGN.md section 3 where the paper is silent.  No blocking, fusion or closed forms.
+ *
+ * Notation (Table 1): E experts, P ranks, Ns = Nb + Nr slots per rank,
+ * S = P*Ns global slots, slot j belongs to rank j / Ns, K = top-k, T tokens in the step,
+ * micro-step i = tokens [mb_off[i], mb_off[i+1]), instance = one (micro-step, layer),
+ * pair = one (token, k) entry, c[e] = w_{s,e} with the single source rank.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"):
+ *   O1 hist      numpy.bincount; sums = T_i*K; closed form on constructed ids.
+ *   O2 quota     brute force over ALL integer splits on tiny inputs (max rank load is the
+ *                exhaustive optimum); subset closed form; ceil(LP*) of Eq.(10) by HiGHS
+ *                (PAPER.md:397-407); Eq.(8)/(9) invariants; hand-worked vectors in tests/golden/.
+ *                The CHOICE among optimal splits (who gets remainders) is fixed only by this
+ *                file's tie-breaks: parity unpinned against the paper for that choice.
+ *   O3/O4 assign numpy.argsort(kind="stable"); bijection; per-slot counts equal quotas.
+ *   O5 gather    numpy fancy indexing.
+ *   O6 combine   float64 sum within the fp32 error bound; exact cases (w=1, w=1/K).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_OK 0
+#define ORACLE_BAD_ARG (-1)
+#define ORACLE_NO_MEM (-4)
+
+/* data-dependent fault bits (same meaning as the library's dev_status, include/foremoe.h) */
+#define FAULT_ID_RANGE 1      /* expert id outside [0, E)                          */
+#define FAULT_NO_HOST 2       /* expert with tokens but no slot: Eq.(7) violated   */
+#define FAULT_SLOT_EXPERT 4   /* slot_expert value outside [-1, E)                 */
+#define FAULT_MB_OFF 8        /* mb_off not non-decreasing / not 0..T              */
+#define FAULT_QUOTA_IN 16     /* caller quota violates Eq.(8)/(9) or is negative   */
+
+/* ------------------------------------------------------------------------------------------
+ * O1: load histogram.  hist[i][l][e] = #{(t,k): mb_off[i] <= t < mb_off[i+1], ids[l][t][k]==e}
+ * (w_{s,e} of PAPER.md:204/:247 with one source); step_hist[l][e] = sum_i hist[i][l][e]
+ * (the aggregate of PAPER.md:284).  Returns fault bits.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_load_hist(int L, int T, int K, int E, int n_mb, const int32_t *ids,
+                     const int32_t *mb_off, int32_t *hist, int64_t *step_hist) {
+  int fault = 0;
+  memset(hist, 0, sizeof(int32_t) * (size_t)n_mb * L * E);
+  if (step_hist) memset(step_hist, 0, sizeof(int64_t) * (size_t)L * E);
+  if (mb_off[0] != 0 || mb_off[n_mb] != T) fault |= FAULT_MB_OFF;
+  for (int i = 0; i < n_mb; i++)
+    if (mb_off[i + 1] < mb_off[i]) fault |= FAULT_MB_OFF;
+  if (fault) return fault;
+  for (int i = 0; i < n_mb; i++)
+    for (int l = 0; l < L; l++)
+      for (int t = mb_off[i]; t < mb_off[i + 1]; t++)
+        for (int k = 0; k < K; k++) {
+          int32_t e = ids[((size_t)l * T + t) * K + k];
+          if (e < 0 || e >= E) { fault |= FAULT_ID_RANGE; continue; }
+          hist[((size_t)i * L + l) * E + e] += 1;
+          if (step_hist) step_hist[(size_t)l * E + e] += 1;
+        }
+  return fault;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O2: Stage-4 token assignment as integer quotas for ONE instance.
+ *
+ * c[E] counts, slot_expert[S] placement (-1 = empty slot).  Outputs quota[S], rank_load[P],
+ * slot_off[S+1].  stop_after: 1 = Phase A + ONE water-filling pass (the literal single pass of
+ * Alg. 3 lines 18-21), 2 = Phase B fixpoint, 3 = Phase C too (the rule).  stats[0] = passes run,
+ * stats[1] = units moved by Phase C.  Returns fault bits.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+  int E, P, Ns, S;
+  const int32_t *c;
+  const int32_t *slot_expert;
+  int32_t *active;    /* [S] 1 if slot is the lowest-indexed slot of its expert on its rank */
+  int32_t *n_active;  /* [E] number of active hosts */
+  int32_t *host_ptr;  /* [E+1] active hosts of e = host_slot[host_ptr[e] .. host_ptr[e+1]) */
+  int32_t *host_slot; /* [S]   ... in ascending slot index */
+  int64_t *load;      /* [P] */
+  int32_t *q;         /* [S] */
+} inst_t;
+
+/* a before b in the processing order: descending count, ties ascending expert id (reading 3) */
+static int goes_before(const int32_t *c, int32_t ea, int32_t eb) {
+  if (c[ea] != c[eb]) return c[ea] > c[eb];
+  return ea < eb;
+}
+
+/* water-fill one replicated expert, unit by unit: each unit goes to the active
+ * host whose rank currently has the smallest load, ties to the lowest slot index. */
+static void fill_units(inst_t *I, int e) {
+  for (int32_t u = 0; u < I->c[e]; u++) {
+    int best = -1;
+    for (int a = I->host_ptr[e]; a < I->host_ptr[e + 1]; a++) {   /* ascending slot index */
+      int j = I->host_slot[a];
+      if (best < 0 || I->load[j / I->Ns] < I->load[best / I->Ns]) best = j;
+    }
+    I->q[best] += 1;
+    I->load[best / I->Ns] += 1;
+  }
+}
+
+int oracle_quota(int E, int P, int Ns, const int32_t *c, const int32_t *slot_expert,
+                 int32_t *quota, int32_t *rank_load, int32_t *slot_off, int stop_after,
+                 int32_t *stats) {
+  const int S = P * Ns;
+  int fault = 0;
+  inst_t I;
+  I.E = E; I.P = P; I.Ns = Ns; I.S = S; I.c = c; I.slot_expert = slot_expert;
+  I.active = (int32_t *)calloc((size_t)S, sizeof(int32_t));
+  I.n_active = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  I.load = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  I.q = (int32_t *)calloc((size_t)S, sizeof(int32_t));
+  I.host_ptr = (int32_t *)calloc((size_t)E + 1, sizeof(int32_t));
+  I.host_slot = (int32_t *)calloc((size_t)S + 1, sizeof(int32_t));
+  int32_t *R = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *old = (int32_t *)calloc((size_t)S, sizeof(int32_t));
+  int32_t *visited = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int32_t *par_rank = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int32_t *par_exp = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int32_t *queue = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  if (stats) { stats[0] = 0; stats[1] = 0; }
+  if (!I.host_ptr || !I.host_slot || !I.active || !I.n_active || !I.load || !I.q || !R || !old || !visited || !par_rank ||
+      !par_exp || !queue) { fault = ORACLE_NO_MEM; goto done; }
+
+  /* hosts: active = lowest-indexed slot of expert e on its rank (reading 10) */
+  for (int j = 0; j < S; j++) {
+    int32_t e = slot_expert[j];
+    if (e < -1 || e >= E) { fault |= FAULT_SLOT_EXPERT; continue; }
+    if (e < 0) continue;
+    int first = 1;
+    for (int j2 = (j / Ns) * Ns; j2 < j; j2++)
+      if (slot_expert[j2] == e) first = 0;
+    I.active[j] = first;
+    I.n_active[e] += first;
+  }
+  for (int e = 0; e < E; e++) {          /* active host lists, ascending slot index */
+    I.host_ptr[e + 1] = I.host_ptr[e];
+    for (int j = 0; j < S; j++)
+      if (slot_expert[j] == e && I.active[j]) I.host_slot[I.host_ptr[e + 1]++] = j;
+  }
+  for (int e = 0; e < E; e++) {
+    if (c[e] < 0) fault |= FAULT_ID_RANGE;
+    if (c[e] > 0 && I.n_active[e] == 0) fault |= FAULT_NO_HOST;
+  }
+  if (fault) goto write_out;
+
+  /* Phase A: forced load of singly hosted experts */
+  int nR = 0;
+  for (int e = 0; e < E; e++) {
+    if (I.n_active[e] == 1) {
+      for (int j = 0; j < S; j++)
+        if (slot_expert[j] == e && I.active[j]) { I.q[j] = c[e]; I.load[j / Ns] += c[e]; }
+    } else if (I.n_active[e] >= 2) {
+      R[nR++] = e;
+    }
+  }
+  /* replicated experts in descending count, ties ascending id (reading 3) */
+  for (int a = 1; a < nR; a++) {          /* insertion sort */
+    int32_t e = R[a];
+    int b = a;
+    while (b > 0 && goes_before(c, e, R[b - 1])) { R[b] = R[b - 1]; b--; }
+    R[b] = e;
+  }
+
+  /* Phase B: Gauss-Seidel water-filling passes until a full pass changes no quota (cap 256) */
+  int passes = 0;
+  for (int pass = 0; pass < 256; pass++) {
+    int changed = 0;
+    passes++;
+    for (int a = 0; a < nR; a++) {
+      int e = R[a];
+      for (int j = 0; j < S; j++)
+        if (slot_expert[j] == e && I.active[j]) {
+          old[j] = I.q[j];
+          I.load[j / Ns] -= I.q[j];
+          I.q[j] = 0;
+        }
+      fill_units(&I, e);
+      for (int j = 0; j < S; j++)
+        if (slot_expert[j] == e && I.active[j] && I.q[j] != old[j]) changed = 1;
+    }
+    if (!changed || stop_after == 1) break;
+  }
+  if (stats) stats[0] = passes;
+
+  /* Phase C: unit augmentations until the lowest max-load rank has no improving path */
+  if (stop_after >= 3) {
+    for (;;) {
+      int64_t mx = -1; int h = 0;
+      for (int r = 0; r < P; r++) if (I.load[r] > mx) { mx = I.load[r]; h = r; }
+      memset(visited, 0, sizeof(int32_t) * (size_t)P);
+      int head = 0, tail = 0, target = -1;
+      visited[h] = 1; queue[tail++] = h; par_rank[h] = -1; par_exp[h] = -1;
+      while (head < tail && target < 0) {
+        int r = queue[head++];
+        /* replicated experts with quota on r, ascending expert id */
+        for (int e = 0; e < E && target < 0; e++) {
+          if (I.n_active[e] < 2) continue;
+          int on_r = -1;
+          for (int j = r * Ns; j < (r + 1) * Ns; j++)
+            if (slot_expert[j] == e && I.active[j]) on_r = j;
+          if (on_r < 0 || I.q[on_r] <= 0) continue;
+          for (int j = 0; j < S && target < 0; j++) {   /* active hosts, ascending slot index */
+            if (slot_expert[j] != e || !I.active[j]) continue;
+            int r2 = j / Ns;
+            if (visited[r2]) continue;
+            visited[r2] = 1; par_rank[r2] = r; par_exp[r2] = e; queue[tail++] = r2;
+            if (I.load[r2] <= mx - 2) target = r2;
+          }
+        }
+      }
+      if (target < 0) break;
+      /* move one unit of each expert on the path target <- ... <- h */
+      for (int r2 = target; par_rank[r2] >= 0; r2 = par_rank[r2]) {
+        int r = par_rank[r2], e = par_exp[r2];
+        for (int j = r * Ns; j < (r + 1) * Ns; j++)
+          if (slot_expert[j] == e && I.active[j]) I.q[j] -= 1;
+        for (int j = r2 * Ns; j < (r2 + 1) * Ns; j++)
+          if (slot_expert[j] == e && I.active[j]) I.q[j] += 1;
+      }
+      I.load[h] -= 1;
+      I.load[target] += 1;
+      if (stats) stats[1] += 1;
+    }
+  }
+
+write_out:
+  slot_off[0] = 0;
+  for (int j = 0; j < S; j++) {
+    quota[j] = I.q[j];
+    slot_off[j + 1] = slot_off[j] + I.q[j];
+  }
+  for (int r = 0; r < P; r++) {
+    int64_t s = 0;
+    for (int j = r * Ns; j < (r + 1) * Ns; j++) s += I.q[j];
+    rank_load[r] = (int32_t)s;
+  }
+done:
+  free(I.host_ptr); free(I.host_slot); free(I.active); free(I.n_active); free(I.load); free(I.q); free(R); free(old);
+  free(visited); free(par_rank); free(par_exp); free(queue);
+  return fault;
+}
+
+/* validate a caller-supplied quota against Eq.(8) conservation and Eq.(9) feasibility
+ * (PAPER.md:266-270): sum over hosts of e equals c[e]; quota > 0 only on slots holding e. */
+int oracle_check_quota(int E, int S, const int32_t *c, const int32_t *slot_expert,
+                       const int32_t *quota) {
+  int fault = 0;
+  int64_t *sum = (int64_t *)calloc((size_t)E, sizeof(int64_t));
+  if (!sum) return ORACLE_NO_MEM;
+  for (int j = 0; j < S; j++) {
+    if (quota[j] < 0) fault |= FAULT_QUOTA_IN;
+    if (slot_expert[j] < 0) { if (quota[j] != 0) fault |= FAULT_QUOTA_IN; continue; }
+    sum[slot_expert[j]] += quota[j];
+  }
+  for (int e = 0; e < E; e++) if (sum[e] != c[e]) fault |= FAULT_QUOTA_IN;
+  free(sum);
+  return fault;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3 + O4 for ONE instance: n_pairs = T_i*K ids in (t,k) order.
+ * O3: the pair with 0-based rank n among the instance's pairs of expert e goes to the host slot
+ *     j of e (ascending slot index) whose cumulative-quota interval contains n (reading 1:
+ *     contiguous blocks of the expert's stable token order; PAPER.md:250 gives only fractions).
+ * O4: stable counting sort by slot: dst = slot_off[j] + #{earlier pairs with slot j};
+ *     inv[p] = base + dst, perm[base + dst] = base + p, where base = mb_off[i]*K places the
+ *     instance's rows inside its layer (layer-global row indices).
+ * ------------------------------------------------------------------------------------------ */
+int oracle_assign_instance(int E, int S, int n_pairs, int32_t base, const int32_t *ids,
+                           const int32_t *slot_expert, const int32_t *quota,
+                           const int32_t *slot_off, int32_t *pair_slot, int32_t *inv,
+                           int32_t *perm) {
+  int fault = 0;
+  int32_t *seen = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *filled = (int32_t *)calloc((size_t)S, sizeof(int32_t));
+  if (!seen || !filled) { free(seen); free(filled); return ORACLE_NO_MEM; }
+  for (int p = 0; p < n_pairs; p++) {
+    int32_t e = ids[p];
+    if (e < 0 || e >= E) { fault |= FAULT_ID_RANGE; pair_slot[p] = -1; continue; }
+    int32_t n = seen[e]++;
+    int32_t cum = 0, slot = -1;
+    for (int j = 0; j < S; j++) {
+      if (slot_expert[j] != e) continue;
+      if (n < cum + quota[j]) { slot = j; break; }
+      cum += quota[j];
+    }
+    pair_slot[p] = slot;
+    if (slot < 0) fault |= FAULT_NO_HOST;
+  }
+  for (int p = 0; p < n_pairs; p++) {
+    int32_t j = pair_slot[p];
+    if (j < 0) { inv[p] = -1; continue; }
+    int32_t dst = slot_off[j] + filled[j]++;
+    inv[p] = base + dst;
+    perm[dst] = base + p;
+  }
+  free(seen); free(filled);
+  return fault;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5: gather (dispatch).  buf[d][:] = x[(perm[d] - pair_base) / K][:], bit copy of row_bytes.
+ * perm holds n_rows layer-global pair indices; pair_base = first token of the range * K; x row 0
+ * is that first token; buf row 0 is layer-global row pair_base.  (dispatch "routes
+ * each token ... to the rank hosting its assigned expert".)
+ * ------------------------------------------------------------------------------------------ */
+int oracle_gather(int64_t n_rows, int K, int64_t row_bytes, int32_t pair_base,
+                  const int32_t *perm, const uint8_t *x, uint8_t *buf) {
+  for (int64_t d = 0; d < n_rows; d++) {
+    int64_t t = ((int64_t)perm[d] - pair_base) / K;
+    memcpy(buf + d * row_bytes, x + t * row_bytes, (size_t)row_bytes);
+  }
+  return 0;
+}
+
+static float bf16_to_float(uint16_t b) {
+  uint32_t u = (uint32_t)b << 16;
+  float f;
+  memcpy(&f, &u, sizeof f);
+  return f;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O6: combine.  y[t][h] = sum_{k=0}^{K-1} w[t][k] * float(eo[inv[t*K+k] - row_base][h]),
+ * accumulated as acc = fmaf(w, v, acc) from acc = 0.0f with k ascending, fp32 output
+ * ("the weighted sum of the selected experts' outputs, where the weights are the
+ * corresponding router probabilities"; order / fma / output type = reading 16).
+ * act_dtype 0 = bf16 rows, 1 = fp32 rows.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_combine(int64_t n_tok, int K, int H, int act_dtype, int32_t row_base,
+                   const int32_t *inv, const float *w, const void *eo, float *y) {
+  for (int64_t t = 0; t < n_tok; t++)
+    for (int h = 0; h < H; h++) {
+      float acc = 0.0f;
+      for (int k = 0; k < K; k++) {
+        int64_t row = (int64_t)inv[t * K + k] - row_base;
+        float v = act_dtype == 0 ? bf16_to_float(((const uint16_t *)eo)[row * H + h])
+                                 : ((const float *)eo)[row * H + h];
+        acc = fmaf(w[t * K + k], v, acc);
+      }
+      y[t * H + h] = acc;
+    }
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Whole-step plan: O1 must have been run (hist).  For every instance (i,l): O2 then O3+O4.
+ * quota_in (may be NULL): caller-supplied quotas, validated by Eq.(8)/(9) instead of computed.
+ * ------------------------------------------------------------------------------------------ */
+int oracle_plan(int L, int T, int K, int E, int P, int Ns, int n_mb, const int32_t *ids,
+                const int32_t *mb_off, const int32_t *hist, const int32_t *slot_expert,
+                const int32_t *quota_in, int32_t *quota, int32_t *rank_load, int32_t *slot_off,
+                int32_t *pair_slot, int32_t *inv, int32_t *perm) {
+  const int S = P * Ns;
+  int fault = 0;
+  for (int i = 0; i < n_mb; i++)
+    for (int l = 0; l < L; l++) {
+      size_t inst = (size_t)i * L + l;
+      const int32_t *c = hist + inst * E;
+      const int32_t *se = slot_expert + (size_t)l * S;
+      int32_t *q = quota + inst * S, *so = slot_off + inst * (S + 1);
+      if (quota_in) {
+        fault |= oracle_check_quota(E, S, c, se, quota_in + inst * S);
+        so[0] = 0;
+        for (int j = 0; j < S; j++) { q[j] = quota_in[inst * S + j]; so[j + 1] = so[j] + q[j]; }
+        for (int r = 0; r < P; r++) {
+          int32_t s = 0;
+          for (int j = r * Ns; j < (r + 1) * Ns; j++) s += q[j];
+          rank_load[inst * P + r] = s;
+        }
+      } else {
+        fault |= oracle_quota(E, P, Ns, c, se, q, rank_load + inst * P, so, 3, NULL);
+      }
+      if (fault & (FAULT_NO_HOST | FAULT_SLOT_EXPERT | FAULT_QUOTA_IN)) continue;
+      size_t p0 = ((size_t)l * T + mb_off[i]) * K;
+      int n_pairs = (mb_off[i + 1] - mb_off[i]) * K;
+      fault |= oracle_assign_instance(E, S, n_pairs, mb_off[i] * K, ids + p0, se, q, so,
+                                      pair_slot + p0, inv + p0, perm + p0);
+    }
+  return fault;
+}

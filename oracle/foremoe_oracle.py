@@ -1,0 +1,135 @@
+"""ctypes + numpy front end of oracle/foremoe_oracle.c -- TEST INFRASTRUCTURE ONLY.
+
+Argument marshalling only; every step is computed by the plain C in foremoe_oracle.c (see its
+header for the citations and the pins).  All arrays are host numpy arrays.  bf16 rows are
+carried as uint16 bit patterns.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+FAULT_ID_RANGE = 1
+FAULT_NO_HOST = 2
+FAULT_SLOT_EXPERT = 4
+FAULT_MB_OFF = 8
+FAULT_QUOTA_IN = 16
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def load_hist(ids: np.ndarray, mb_off: np.ndarray, E: int, want_step: bool = True):
+    """O1.  ids int32 [L,T,K] -> hist int32 [n_mb,L,E], step_hist int64 [L,E], fault bits."""
+    ids = _i32(ids)
+    mb_off = _i32(mb_off)
+    L, T, K = ids.shape
+    n_mb = mb_off.shape[0] - 1
+    hist = np.zeros((n_mb, L, E), dtype=np.int32)
+    step = np.zeros((L, E), dtype=np.int64) if want_step else None
+    fault = lib().oracle_load_hist(L, T, K, E, n_mb, _p(ids), _p(mb_off), _p(hist), _p(step))
+    return hist, step, fault
+
+
+def quota(c: np.ndarray, slot_expert: np.ndarray, P: int, Ns: int, stop_after: int = 3):
+    """O2 for one instance -> quota[S], rank_load[P], slot_off[S+1], (passes, moved), fault."""
+    c = _i32(c)
+    se = _i32(slot_expert)
+    E, S = c.shape[0], P * Ns
+    assert se.shape == (S,)
+    q = np.zeros(S, dtype=np.int32)
+    rl = np.zeros(P, dtype=np.int32)
+    so = np.zeros(S + 1, dtype=np.int32)
+    stats = np.zeros(2, dtype=np.int32)
+    fault = lib().oracle_quota(E, P, Ns, _p(c), _p(se), _p(q), _p(rl), _p(so), stop_after,
+                               _p(stats))
+    return q, rl, so, (int(stats[0]), int(stats[1])), fault
+
+
+def check_quota(c, slot_expert, q) -> int:
+    c, se, q = _i32(c), _i32(slot_expert), _i32(q)
+    return lib().oracle_check_quota(c.shape[0], se.shape[0], _p(c), _p(se), _p(q))
+
+
+def assign_instance(ids_flat, slot_expert, q, slot_off, E: int, base: int = 0):
+    """O3+O4 for one instance -> pair_slot, inv, perm (each [n_pairs]), fault."""
+    ids_flat = _i32(ids_flat).ravel()
+    se, q, so = _i32(slot_expert), _i32(q), _i32(slot_off)
+    n = ids_flat.shape[0]
+    ps = np.full(n, -1, dtype=np.int32)
+    inv = np.full(n, -1, dtype=np.int32)
+    perm = np.full(n, -1, dtype=np.int32)
+    fault = lib().oracle_assign_instance(E, se.shape[0], n, base, _p(ids_flat), _p(se), _p(q),
+                                         _p(so), _p(ps), _p(inv), _p(perm))
+    return ps, inv, perm, fault
+
+
+def plan(ids, mb_off, hist, slot_expert, P: int, Ns: int, quota_in=None):
+    """Whole-step O2+O3+O4 -> dict(quota, rank_load, slot_off, pair_slot, inv, perm, fault)."""
+    ids, mb_off, hist, se = _i32(ids), _i32(mb_off), _i32(hist), _i32(slot_expert)
+    L, T, K = ids.shape
+    n_mb = mb_off.shape[0] - 1
+    E = hist.shape[2]
+    S = P * Ns
+    assert se.shape == (L, S) and hist.shape == (n_mb, L, E)
+    qi = None if quota_in is None else _i32(quota_in)
+    out = dict(
+        quota=np.zeros((n_mb, L, S), dtype=np.int32),
+        rank_load=np.zeros((n_mb, L, P), dtype=np.int32),
+        slot_off=np.zeros((n_mb, L, S + 1), dtype=np.int32),
+        pair_slot=np.full((L, T, K), -1, dtype=np.int32),
+        inv=np.full((L, T, K), -1, dtype=np.int32),
+        perm=np.full((L, T * K), -1, dtype=np.int32),
+    )
+    out["fault"] = lib().oracle_plan(L, T, K, E, P, Ns, n_mb, _p(ids), _p(mb_off), _p(hist),
+                                     _p(se), _p(qi), _p(out["quota"]), _p(out["rank_load"]),
+                                     _p(out["slot_off"]), _p(out["pair_slot"]), _p(out["inv"]),
+                                     _p(out["perm"]))
+    return out
+
+
+def gather(perm: np.ndarray, x: np.ndarray, K: int, pair_base: int = 0) -> np.ndarray:
+    """O5.  perm: layer-global pair indices of the rows wanted; x: [n_tok, H] rows (any dtype)."""
+    perm = _i32(perm).ravel()
+    x = np.ascontiguousarray(x)
+    row_bytes = x.shape[1] * x.dtype.itemsize
+    buf = np.empty((perm.shape[0], x.shape[1]), dtype=x.dtype)
+    lib().oracle_gather.argtypes = [C.c_int64, C.c_int, C.c_int64, C.c_int32, C.c_void_p,
+                                    C.c_void_p, C.c_void_p]
+    lib().oracle_gather(perm.shape[0], K, row_bytes, pair_base, _p(perm), _p(x), _p(buf))
+    return buf
+
+
+def combine(inv: np.ndarray, w: np.ndarray, eo: np.ndarray, act_dtype: int,
+            row_base: int = 0) -> np.ndarray:
+    """O6.  inv int32 [n_tok,K] layer-global rows, w fp32 [n_tok,K], eo [n_rows,H] (uint16 bf16
+    bits when act_dtype == 0, float32 when 1) -> y fp32 [n_tok,H]."""
+    inv = _i32(inv)
+    w = np.ascontiguousarray(w, dtype=np.float32)
+    eo = np.ascontiguousarray(eo)
+    assert eo.dtype == (np.uint16 if act_dtype == 0 else np.float32)
+    n_tok, K = inv.shape
+    H = eo.shape[1]
+    y = np.empty((n_tok, H), dtype=np.float32)
+    lib().oracle_combine.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int32,
+                                     C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib().oracle_combine(n_tok, K, H, act_dtype, row_base, _p(inv), _p(w), _p(eo), _p(y))
+    return y

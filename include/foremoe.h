@@ -1,0 +1,173 @@
+/*
+ * foremoe.h -- C ABI of the B200 (sm_100a) library for the data-parallel hot path behind
+ * ForeMoE's micro-step MoE load balancing (arxiv/paper_2606_11867).
+ *
+ * Given the routing foresight recorded at rollout (top-K expert ids + gate weights per token per
+ * MoE layer, PAPER.md:112 sec. 4, :130 sec. 5), micro-step boundaries (sec. 2.3) and a
+ * step-level expert placement with replica slots over P logical EP ranks (x_{e,j}, PAPER.md:249
+ * sec. 7.2), the library computes on ONE GPU
+ *   (1) the per-(micro-step, layer) expert load histogram  w_{s,e}  (PAPER.md:204 Table 1, :247),
+ *   (2) Stage 4 "token assignment" with the placement fixed (sec. 8.2 Eq.(10);
+ *       water-filling variant PAPER.md:821-828 Alg. 3 lines 18-21, :844-846 App. D) as integer
+ *       per-slot quotas, and the slot of every (token, k) pair,
+ *   (3) the dispatch realising the plan (PAPER.md:58 sec. 2.1, :427 sec. 9): stable counting-sort
+ *       permutation + offsets, row gather into contiguous per-rank / per-slot buffers, and the
+ *       inverse weighted top-K combine (sec. 2.1).
+ *
+ * Notation (Table 1): L MoE layers, E experts, K top-k, P logical ranks,
+ * Ns = Nb + Nr slots per rank (Nb = E / P base, Nr redundant), S = P * Ns global slots, slot j
+ * belongs to rank j / Ns, T tokens in the step, micro-step i = tokens [mb_off[i], mb_off[i+1]),
+ * T_i its token count, H hidden size.  instance = one (micro-step, layer).  pair = one
+ * (token, k) entry; pair p = t * K + k is the LAYER-GLOBAL pair index.  The dispatched rows of
+ * layer l form one array of T * K rows; instance (i, l) owns rows [mb_off[i]*K, mb_off[i+1]*K),
+ * ordered by rank, then by slot, stable in (t, k) order inside a slot (reading 13).
+ *
+ * General rules
+ *  - Every data pointer is a DEVICE pointer owned by the caller unless the argument is marked
+ *    "host".  The foremoe_shape_t pointer is a host pointer, read during the call only.
+ *  - The library allocates no device memory, keeps no global state and is re-entrant per stream.
+ *    All entry points except foremoe_workspace_bytes / foremoe_version / foremoe_step_host
+ *    enqueue work on `stream` (a cudaStream_t passed as void*) and return without synchronising.
+ *  - Return value: FOREMOE_OK, or a negative host-detectable error (nothing was enqueued).
+ *  - Data-dependent faults cannot be seen without a sync; they are OR-ed into *dev_status
+ *    (device int32, may be NULL, never cleared by the library): FOREMOE_FAULT_* bits.  On a
+ *    device fault the affected instance's outputs are unspecified, all writes stay in bounds.
+ *  - Requirements: T * K < 2^31; 1 <= K <= 32, K <= E; E % P == 0 and Nb == E / P; Nr >= 0;
+ *    row bytes H * es (es = 2 for bf16, 4 for fp32) a multiple of 16; x / buf / expert_out / y
+ *    16-byte aligned; int32 / fp32 arrays 4-byte aligned (K = 10 id rows are only 8-byte
+ *    aligned -- nothing wider is assumed).
+ */
+#ifndef FOREMOE_H_
+#define FOREMOE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FOREMOE_OK 0
+#define FOREMOE_ERR_INVALID_ARG (-1)      /* NULL, bad dims, misaligned pointer, bad mb range */
+#define FOREMOE_ERR_WORKSPACE (-2)        /* workspace_bytes too small                        */
+#define FOREMOE_ERR_CUDA (-3)             /* CUDA error at launch / copy                      */
+
+#define FOREMOE_FAULT_ID_RANGE 1          /* expert id outside [0, E) (pair ignored)          */
+#define FOREMOE_FAULT_NO_HOST 2           /* expert with tokens but no slot: Eq.(7) violated,
+                                             or hist inconsistent with ids                    */
+#define FOREMOE_FAULT_SLOT_EXPERT 4       /* slot_expert value outside [-1, E)                */
+#define FOREMOE_FAULT_MB_OFF 8            /* mb_off not non-decreasing or not 0 .. T          */
+#define FOREMOE_FAULT_QUOTA_IN 16         /* caller quota violates Eq.(8)/(9) or is negative  */
+
+#define FOREMOE_ACT_BF16 0
+#define FOREMOE_ACT_FP32 1
+
+typedef struct {
+  int32_t L, E, K;             /* MoE layers, experts, top-k                                   */
+  int32_t P, Nb, Nr;           /* logical ranks, base / redundant slots per rank               */
+  int32_t T, n_mb;             /* tokens in the step, micro-steps                              */
+  int32_t H, act_dtype;        /* hidden size; FOREMOE_ACT_BF16 / FOREMOE_ACT_FP32             */
+  int32_t placement_mb_stride; /* 0: slot_expert is [L][S] (step-level placement);
+                                  L*S: slot_expert is [n_mb][L][S] (one placement per micro-step,
+                                  PAPER.md:343 A^{(i)})                                         */
+} foremoe_shape_t;
+
+/* Library version (major * 100 + minor).  Host only. */
+int foremoe_version(void);
+
+/* Bytes of device scratch foremoe_assign needs for this shape.  Host only, no CUDA call. */
+int foremoe_workspace_bytes(const foremoe_shape_t *shape, size_t *bytes /* host, out */);
+
+/*
+ * (a1) Load histogram -- w_{s,e} with the single source rank and its step
+ * aggregate (sec. 8.1).
+ *   ids       [L][T][K] int32, expert ids of the routing trace (layer-major).
+ *   mb_off    [n_mb+1]  int32, micro-step token boundaries, mb_off[0] = 0, mb_off[n_mb] = T.
+ *   hist      [n_mb][L][E] int32 out: hist[i][l][e] = #{(t,k): t in micro-step i, ids[l][t][k] == e}.
+ *   step_hist [L][E] int64 out, or NULL: sum over micro-steps.
+ * Faults: ID_RANGE (the pair is not counted), MB_OFF (hist and step_hist are all zero).
+ */
+int foremoe_load_hist(const foremoe_shape_t *shape, const int32_t *ids, const int32_t *mb_off,
+                      int32_t *hist, int64_t *step_hist, int32_t *dev_status, void *stream);
+
+/*
+ * (a2-a4) Stage-4 token assignment for every instance of the step, placement fixed.
+ *   hist        [n_mb][L][E] from foremoe_load_hist on the same ids / mb_off.
+ *   slot_expert [L][S] (or [n_mb][L][S], see placement_mb_stride) int32: expert held by global
+ *               slot j = rank * Ns + local; -1 = empty slot (reading 9).
+ *   quota_in    NULL: quotas are computed by the exact water-filling rule (O2):
+ *               forced loads, Gauss-Seidel water-filling passes to a fixpoint (PAPER.md:826-827,
+ *               :844-846), unit augmentations until max rank load is optimal.
+ *               else [n_mb][L][S] caller-supplied quotas (e.g. from an LP of Eq.(10)), validated
+ *               against Eq.(8) conservation and Eq.(9) feasibility.
+ *   quota       [n_mb][L][S]   out: tokens each slot receives.
+ *   rank_load   [n_mb][L][P]   out: L_r of Eq.(4) = sum of the quotas of rank r's slots.
+ *   slot_off    [n_mb][L][S+1] out: exclusive prefix of quota (rows of slot j inside the instance).
+ *   pair_slot   [L][T][K]      out: global slot of every pair: the pair with stable rank n among
+ *               the instance's pairs of expert e goes to the host slot of e (ascending slot index)
+ *               whose cumulative-quota interval contains n (reading 1).  -1 on fault.
+ *   inv         [L][T][K]      out: layer-global destination row of every pair
+ *               = mb_off[i]*K + slot_off[j] + (stable rank of the pair inside slot j).  -1 on fault.
+ *   workspace   device scratch of at least foremoe_workspace_bytes() bytes, 16-byte aligned.
+ * Faults: ID_RANGE, NO_HOST, SLOT_EXPERT, MB_OFF, QUOTA_IN.
+ */
+int foremoe_assign(const foremoe_shape_t *shape, const int32_t *ids, const int32_t *mb_off,
+                   const int32_t *hist, const int32_t *slot_expert, const int32_t *quota_in,
+                   int32_t *quota, int32_t *rank_load, int32_t *slot_off, int32_t *pair_slot,
+                   int32_t *inv, void *workspace, size_t workspace_bytes, int32_t *dev_status,
+                   void *stream);
+
+/*
+ * (a4-a5) Dispatch of micro-steps [mb_begin, mb_end) of one layer: the permutation and the row
+ * gather into contiguous per-rank / per-slot buffers.
+ *   inv   [L][T][K] from foremoe_assign (the whole array; the call indexes layer / range itself).
+ *   x     [T_range][H] activations, row 0 = token mb_off[mb_begin]; bf16 or fp32 per act_dtype.
+ *   perm  [T_range*K] int32 out, or NULL: perm[d - row0] = p for the pair p with inv[l][p] = d,
+ *         row0 = mb_off[mb_begin]*K (layer-global pair index; stable counting sort by slot).
+ *   buf   [T_range*K][H] out: buf[d - row0][:] = x[p / K - mb_off[mb_begin]][:], bitwise copy.
+ * Pairs with inv < 0 (faulted in assign) are skipped; their rows of buf are left untouched.
+ */
+int foremoe_dispatch(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin, int32_t mb_end,
+                     const int32_t *mb_off, const int32_t *inv, const void *x, int32_t *perm,
+                     void *buf, int32_t *dev_status, void *stream);
+
+/*
+ * (a6) Combine of micro-steps [mb_begin, mb_end) of one layer: the weighted top-K sum
+ * in fp32 with fused multiply-add, k ascending, from acc = 0 (reading 16):
+ *   y[t - t0][h] = fma(w[l][t][K-1], eo[inv[l][t][K-1] - row0][h], ... fma(w[l][t][0], eo[...][h], 0))
+ *   w          [L][T][K] fp32 gate weights of the trace (the whole array).
+ *   expert_out [T_range*K][H] rows in the order of buf (bf16 or fp32 per act_dtype).
+ *   y          [T_range][H] fp32 out.
+ * Pairs with inv < 0 contribute nothing.
+ */
+int foremoe_combine(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin, int32_t mb_end,
+                    const int32_t *mb_off, const int32_t *inv, const float *w,
+                    const void *expert_out, float *y, int32_t *dev_status, void *stream);
+
+/* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
+ * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */
+int foremoe_step_host_arena_bytes(const foremoe_shape_t *shape, const int32_t *mb_off_h,
+                                  size_t *bytes /* host, out */);
+
+/*
+ * The whole path from HOST buffers (end-to-end leg): copies the trace, boundaries and placement
+ * to the device, runs load_hist + assign for the step, then for every micro-step i and layer l
+ * copies x of the micro-step in (once per micro-step), runs dispatch + combine with the identity
+ * expert (expert_out = buf) and copies y back.  Synchronises `stream` before returning.
+ *   ids_h [L][T][K], w_h [L][T][K], mb_off_h [n_mb+1], slot_expert_h [L][S]: host (pinned for speed).
+ *   x_h   [T][H] host activations (one row per token of the step; reused by every layer).
+ *   quota_h [n_mb][L][S], rank_load_h [n_mb][L][P], slot_off_h [n_mb][L][S+1]: host out (may be NULL).
+ *   y_h   [T][H] fp32 host out: rows of micro-step i are overwritten by every layer in turn, so
+ *         on return it holds the last layer's output; every layer's y crosses the bus.
+ *   arena device scratch of foremoe_step_host_arena_bytes() bytes, 256-byte aligned.
+ *   status_h host int32 out: the OR of all device fault bits of the step.
+ */
+int foremoe_step_host(const foremoe_shape_t *shape, const int32_t *ids_h, const float *w_h,
+                      const int32_t *mb_off_h, const int32_t *slot_expert_h, const void *x_h,
+                      int32_t *quota_h, int32_t *rank_load_h, int32_t *slot_off_h, float *y_h,
+                      void *arena, size_t arena_bytes, int32_t *status_h, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FOREMOE_H_ */

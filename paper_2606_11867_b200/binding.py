@@ -1,0 +1,217 @@
+"""Thin Python binding of the C-ABI library (include/foremoe.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``libforemoe.so``; PyTorch supplies device
+memory and streams.  There is no CPU fallback: importing the library fails loudly when the
+extension has not been built (``python -m paper_2606_11867_b200.build``).
+
+Function names and arguments mirror the header: ``load_hist``, ``assign``, ``dispatch``,
+``combine``, ``workspace_bytes``, ``step_host``.  Tensors must be contiguous; device entry points
+take CUDA tensors and enqueue on the current stream without synchronising.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import dataclasses
+import os
+from typing import Optional
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libforemoe.so")
+
+OK = 0
+ERR_INVALID_ARG = -1
+ERR_WORKSPACE = -2
+ERR_CUDA = -3
+
+FAULT_ID_RANGE = 1
+FAULT_NO_HOST = 2
+FAULT_SLOT_EXPERT = 4
+FAULT_MB_OFF = 8
+FAULT_QUOTA_IN = 16
+
+ACT_BF16 = 0
+ACT_FP32 = 1
+
+EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
+           "foremoe_dispatch", "foremoe_combine", "foremoe_step_host_arena_bytes",
+           "foremoe_step_host")
+
+
+class ForeMoEError(RuntimeError):
+    def __init__(self, fn: str, code: int):
+        names = {ERR_INVALID_ARG: "INVALID_ARG", ERR_WORKSPACE: "WORKSPACE_TOO_SMALL",
+                 ERR_CUDA: "CUDA_ERROR"}
+        super().__init__(f"{fn} failed: {names.get(code, code)}")
+        self.code = code
+
+
+class _CShape(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("L", "E", "K", "P", "Nb", "Nr", "T", "n_mb", "H",
+                                         "act_dtype", "placement_mb_stride")]
+
+
+@dataclasses.dataclass
+class Shape:
+    """foremoe_shape_t (Table 1 notation)."""
+    L: int
+    E: int
+    K: int
+    P: int
+    Nb: int
+    Nr: int
+    T: int
+    n_mb: int
+    H: int
+    act_dtype: int = ACT_BF16
+    placement_mb_stride: int = 0
+
+    @property
+    def Ns(self) -> int:
+        return self.Nb + self.Nr
+
+    @property
+    def S(self) -> int:
+        return self.P * self.Ns
+
+    @property
+    def act_torch_dtype(self):
+        return torch.bfloat16 if self.act_dtype == ACT_BF16 else torch.float32
+
+    def c(self) -> _CShape:
+        return _CShape(self.L, self.E, self.K, self.P, self.Nb, self.Nr, self.T, self.n_mb,
+                       self.H, self.act_dtype, self.placement_mb_stride)
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """The loaded C-ABI library.  Raises if it was not built: there is no fallback path."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2606_11867_b200.build` "
+                "(the ForeMoE path has no CPU or PyTorch fallback)")
+        l = C.CDLL(LIB_PATH)
+        vp, i32, sz = C.c_void_p, C.c_int32, C.c_size_t
+        sp = C.POINTER(_CShape)
+        l.foremoe_version.restype = C.c_int
+        l.foremoe_version.argtypes = []
+        l.foremoe_workspace_bytes.argtypes = [sp, C.POINTER(sz)]
+        l.foremoe_load_hist.argtypes = [sp, vp, vp, vp, vp, vp, vp]
+        l.foremoe_assign.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
+        l.foremoe_dispatch.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+        l.foremoe_combine.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+        l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
+        l.foremoe_step_host.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
+        for name in EXPORTS:
+            getattr(l, name).restype = C.c_int
+        _lib = l
+    return _lib
+
+
+def _dev(t: Optional[torch.Tensor], dtype=None) -> Optional[int]:
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError("expected a CUDA tensor")
+    if not t.is_contiguous():
+        raise ValueError("expected a contiguous tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _host(t: Optional[torch.Tensor], dtype=None) -> Optional[int]:
+    if t is None:
+        return None
+    if t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous host tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _check(fn: str, rc: int) -> None:
+    if rc != OK:
+        raise ForeMoEError(fn, rc)
+
+
+def version() -> int:
+    return lib().foremoe_version()
+
+
+def workspace_bytes(shape: Shape) -> int:
+    out = C.c_size_t(0)
+    _check("foremoe_workspace_bytes", lib().foremoe_workspace_bytes(C.byref(shape.c()), C.byref(out)))
+    return out.value
+
+
+def load_hist(shape: Shape, ids, mb_off, hist, step_hist=None, dev_status=None) -> None:
+    """(a1) hist[n_mb,L,E] int32 (and step_hist[L,E] int64) from ids[L,T,K], mb_off[n_mb+1]."""
+    _check("foremoe_load_hist", lib().foremoe_load_hist(
+        C.byref(shape.c()), _dev(ids, torch.int32), _dev(mb_off, torch.int32),
+        _dev(hist, torch.int32), _dev(step_hist, torch.int64), _dev(dev_status, torch.int32),
+        _stream()))
+
+
+def assign(shape: Shape, ids, mb_off, hist, slot_expert, quota_in, quota, rank_load, slot_off,
+           pair_slot, inv, workspace, dev_status=None) -> None:
+    """(a2-a4) quotas, rank loads, slot offsets, pair_slot and inv for every instance."""
+    _check("foremoe_assign", lib().foremoe_assign(
+        C.byref(shape.c()), _dev(ids, torch.int32), _dev(mb_off, torch.int32),
+        _dev(hist, torch.int32), _dev(slot_expert, torch.int32), _dev(quota_in, torch.int32),
+        _dev(quota, torch.int32), _dev(rank_load, torch.int32), _dev(slot_off, torch.int32),
+        _dev(pair_slot, torch.int32), _dev(inv, torch.int32), _dev(workspace),
+        workspace.numel() * workspace.element_size(), _dev(dev_status, torch.int32), _stream()))
+
+
+def dispatch(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, x, perm, buf,
+             dev_status=None) -> None:
+    """(a4-a5) perm[T_range*K] and buf[T_range*K,H] for micro-steps [mb_begin, mb_end)."""
+    _check("foremoe_dispatch", lib().foremoe_dispatch(
+        C.byref(shape.c()), layer, mb_begin, mb_end, _dev(mb_off, torch.int32),
+        _dev(inv, torch.int32), _dev(x, shape.act_torch_dtype), _dev(perm, torch.int32),
+        _dev(buf, shape.act_torch_dtype), _dev(dev_status, torch.int32), _stream()))
+
+
+def combine(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, w, expert_out, y,
+            dev_status=None) -> None:
+    """(a6) y[T_range,H] fp32 = weighted top-K sum of expert_out rows."""
+    _check("foremoe_combine", lib().foremoe_combine(
+        C.byref(shape.c()), layer, mb_begin, mb_end, _dev(mb_off, torch.int32),
+        _dev(inv, torch.int32), _dev(w, torch.float32), _dev(expert_out, shape.act_torch_dtype),
+        _dev(y, torch.float32), _dev(dev_status, torch.int32), _stream()))
+
+
+def step_host_arena_bytes(shape: Shape, mb_off_h) -> int:
+    out = C.c_size_t(0)
+    _check("foremoe_step_host_arena_bytes", lib().foremoe_step_host_arena_bytes(
+        C.byref(shape.c()), _host(mb_off_h, torch.int32), C.byref(out)))
+    return out.value
+
+
+def step_host(shape: Shape, ids_h, w_h, mb_off_h, slot_expert_h, x_h, quota_h, rank_load_h,
+              slot_off_h, y_h, arena, status_h) -> None:
+    """The whole path from HOST tensors (pinned for speed); synchronises before returning."""
+    _check("foremoe_step_host", lib().foremoe_step_host(
+        C.byref(shape.c()), _host(ids_h, torch.int32), _host(w_h, torch.float32),
+        _host(mb_off_h, torch.int32), _host(slot_expert_h, torch.int32),
+        _host(x_h, shape.act_torch_dtype), _host(quota_h, torch.int32),
+        _host(rank_load_h, torch.int32), _host(slot_off_h, torch.int32),
+        _host(y_h, torch.float32), _dev(arena), arena.numel() * arena.element_size(),
+        _host(status_h, torch.int32), _stream()))
+
+
+def shape_of(cfg, T: Optional[int] = None, n_mb: Optional[int] = None) -> Shape:
+    """Shape of a synth.TraceConfig."""
+    return Shape(L=cfg.L, E=cfg.E, K=cfg.K, P=cfg.P, Nb=cfg.Nb, Nr=cfg.Nr,
+                 T=cfg.T if T is None else T, n_mb=cfg.n_mb if n_mb is None else n_mb, H=cfg.H,
+                 act_dtype=cfg.act_dtype)

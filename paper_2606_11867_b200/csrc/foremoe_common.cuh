@@ -1,0 +1,105 @@
+// Shared device/host helpers of the ForeMoE sm_100a library (internal; the public contract is
+// include/foremoe.h).  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/foremoe.h"
+
+namespace foremoe {
+
+constexpr int kChunkPairs = 4096;    // pairs ranked by one CTA of k_assign_pairs / k_chunk_hist
+constexpr int kChunkThreads = 256;
+constexpr int kChunkWarps = kChunkThreads / 32;
+constexpr int kQuotaThreads = 128;
+constexpr int kMaxWaterPasses = 256;  // Phase B cap (O2)
+
+// Derived sizes, computed once per call on the host.
+struct Dims {
+  int L, E, K, P, Nb, Nr, Ns, S, T, n_mb, H, act_dtype;
+  int es;            // bytes per activation element
+  int row_bytes;     // H * es
+  int row_vec;       // row_bytes / 16
+  int n_inst;        // n_mb * L
+  int n_pl;          // number of placements: L or n_mb * L
+  int pl_per_mb;     // 1 if one placement per micro-step
+  int tpc;           // tokens per chunk
+  int max_chunks;    // upper bound on chunks per layer
+};
+
+inline int make_dims(const foremoe_shape_t *s, Dims *d) {
+  if (!s) return FOREMOE_ERR_INVALID_ARG;
+  if (s->L <= 0 || s->E <= 0 || s->K <= 0 || s->P <= 0 || s->Nb <= 0 || s->Nr < 0 || s->T < 0 ||
+      s->n_mb <= 0 || s->H <= 0)
+    return FOREMOE_ERR_INVALID_ARG;
+  if (s->K > s->E || s->K > 32) return FOREMOE_ERR_INVALID_ARG;
+  if (s->E % s->P != 0 || s->Nb != s->E / s->P) return FOREMOE_ERR_INVALID_ARG;
+  if (s->act_dtype != FOREMOE_ACT_BF16 && s->act_dtype != FOREMOE_ACT_FP32)
+    return FOREMOE_ERR_INVALID_ARG;
+  if ((int64_t)s->T * s->K >= ((int64_t)1 << 31)) return FOREMOE_ERR_INVALID_ARG;
+  d->L = s->L; d->E = s->E; d->K = s->K; d->P = s->P; d->Nb = s->Nb; d->Nr = s->Nr;
+  d->Ns = s->Nb + s->Nr;
+  if ((int64_t)d->P * d->Ns >= ((int64_t)1 << 24)) return FOREMOE_ERR_INVALID_ARG;
+  d->S = d->P * d->Ns;
+  d->T = s->T; d->n_mb = s->n_mb; d->H = s->H; d->act_dtype = s->act_dtype;
+  d->es = s->act_dtype == FOREMOE_ACT_BF16 ? 2 : 4;
+  int64_t rb = (int64_t)s->H * d->es;
+  if (rb % 16 != 0 || rb >= ((int64_t)1 << 30)) return FOREMOE_ERR_INVALID_ARG;
+  d->row_bytes = (int)rb;
+  d->row_vec = (int)(rb / 16);
+  if ((int64_t)s->n_mb * s->L >= ((int64_t)1 << 28)) return FOREMOE_ERR_INVALID_ARG;
+  d->n_inst = s->n_mb * s->L;
+  if (s->placement_mb_stride == 0) { d->n_pl = s->L; d->pl_per_mb = 0; }
+  else if (s->placement_mb_stride == s->L * d->S) { d->n_pl = d->n_inst; d->pl_per_mb = 1; }
+  else return FOREMOE_ERR_INVALID_ARG;
+  d->tpc = kChunkPairs / s->K;
+  d->max_chunks = (s->T + d->tpc - 1) / d->tpc + s->n_mb;
+  return FOREMOE_OK;
+}
+
+inline bool aligned(const void *p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+// Workspace carve-up of foremoe_assign (all sections int32, 16-byte aligned).
+struct Workspace {
+  size_t chunk_off, mb_ok, pl_host_ptr, pl_host_slot, pl_active, pl_rslot, pl_fault, inst_cum_end,
+      inst_slot_adj, inst_ok, chunk_cnt, total;
+};
+
+inline Workspace make_workspace(const Dims &d) {
+  Workspace w;
+  size_t off = 0;
+  auto take = [&](size_t n_int) { size_t o = off; off += ((n_int * 4 + 15) / 16) * 16; return o; };
+  w.chunk_off = take((size_t)d.n_mb + 1);
+  w.mb_ok = take(4);
+  w.pl_host_ptr = take((size_t)d.n_pl * (d.E + 1));
+  w.pl_host_slot = take((size_t)d.n_pl * d.S);
+  w.pl_active = take((size_t)d.n_pl * d.S);
+  w.pl_rslot = take((size_t)d.n_pl * d.S);
+  w.pl_fault = take((size_t)d.n_pl);
+  w.inst_cum_end = take((size_t)d.n_inst * d.S);
+  w.inst_slot_adj = take((size_t)d.n_inst * d.S);
+  w.inst_ok = take((size_t)d.n_inst);
+  w.chunk_cnt = take((size_t)d.L * d.max_chunks * d.E);
+  w.total = off;
+  return w;
+}
+
+__device__ __forceinline__ void raise_fault(int32_t *dev_status, int bits) {
+  if (dev_status && bits) atomicOr(dev_status, bits);
+}
+
+// Largest i in [0, n) with off[i] <= v, for a non-decreasing off[0..n] with off[0] <= v < off[n]:
+// the last of any run of equal boundaries, so empty ranges are skipped.
+__device__ __forceinline__ int find_range(const int32_t *__restrict__ off, int n, int v) {
+  int lo = 0, hi = n;          // invariant: off[lo] <= v < off[hi]
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (__ldg(off + mid) <= v) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+int num_sms();
+
+}  // namespace foremoe

@@ -1,0 +1,292 @@
+// Data-path kernels of the ForeMoE hot path (sm_100a): dispatch = permutation + row gather (a4/a5)
+// and the weighted top-K combine (a6).  HBM-bound row movers: no tensor cores (nothing here is a
+// dense contraction), 16-byte vectors, whole rows contiguous, persistent grids sized from the SM
+// count.  Contract: include/foremoe.h.
+#include "foremoe_common.cuh"
+
+namespace foremoe {
+
+// ---- 16-byte global accesses with cache hints ---------------------------------------------------
+// rows of x / expert_out are read once per launch and rows of buf / y are written once: keep them
+// out of L1 and mark them streaming.
+__device__ __forceinline__ int4 ld16_stream(const void *p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st16_stream(void *p, const int4 &v) {
+  asm volatile("st.global.cs.v4.s32 [%0], {%1, %2, %3, %4};"
+               :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+struct RangeInfo { int t_begin, t_end, row0; };
+
+__device__ __forceinline__ RangeInfo load_range(const int32_t *__restrict__ mb_off, int mb_begin,
+                                                int mb_end, int K) {
+  RangeInfo r;
+  r.t_begin = __ldg(mb_off + mb_begin);
+  r.t_end = __ldg(mb_off + mb_end);
+  r.row0 = r.t_begin * K;
+  return r;
+}
+
+// =============================================================================================
+// a4 + a5: dispatch.  Token-major: the row of token t is read ONCE and stored to its K
+// destination rows inv[t*K + k] (reading x once matters when x does not fit L2, e.g. H = 7168).
+// One warp per (token, slice) item, slice = 32 * U 16-byte vectors; U loads in flight per lane,
+// then K * U stores.  perm[inv[p] - row0] = p is scattered by the lanes that hold inv.
+// =============================================================================================
+template <int U>
+__global__ void __launch_bounds__(256)
+k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb_off, int mb_begin,
+                int mb_end, int K, int row_vec, int n_slices, const int4 *__restrict__ x,
+                int32_t *__restrict__ perm, int4 *__restrict__ buf) {
+  const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
+  const int lane = threadIdx.x & 31;
+  const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
+  const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
+  for (long long item = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+       item < n_items; item += warps) {
+    const int tl = (int)(item / n_slices);
+    const int sl = (int)(item - (long long)tl * n_slices);
+    const int p0 = (rg.t_begin + tl) * K;
+    int d = -1;
+    if (lane < K) {
+      d = __ldg(inv_l + p0 + lane);
+      if (d >= 0) d -= rg.row0;
+      if (perm && sl == 0 && d >= 0) perm[d] = p0 + lane;
+    }
+    const int4 *src = x + (size_t)tl * row_vec;
+    const int v0 = sl * (32 * U) + lane;
+    int4 r[U];
+#pragma unroll
+    for (int u = 0; u < U; u++)
+      if (v0 + u * 32 < row_vec) r[u] = ld16_stream(src + v0 + u * 32);
+    for (int k = 0; k < K; k++) {
+      const int dk = __shfl_sync(0xffffffffu, d, k);
+      if (dk < 0) continue;
+      int4 *dst = buf + (size_t)dk * row_vec;
+#pragma unroll
+      for (int u = 0; u < U; u++)
+        if (v0 + u * 32 < row_vec) st16_stream(dst + v0 + u * 32, r[u]);
+    }
+  }
+}
+
+// =============================================================================================
+// a6: combine.  y[t][h] = sum_k w[t][k] * float(eo[inv[t*K+k]][h]), fp32 fma, k ascending from
+// acc = 0 (order / fma / fp32 output = DESIGN.md reading 16).
+// One warp per (token, slice) item; per lane KB * U independent 16-byte loads in flight
+// (k in groups of KB, masked tail), fma into registers, 16-byte stores of the fp32 row.
+// =============================================================================================
+__device__ __forceinline__ float bf16_lo(int v) { return __int_as_float(v << 16); }
+__device__ __forceinline__ float bf16_hi(int v) { return __int_as_float(v & 0xffff0000); }
+
+template <bool kBf16, int KB, int U>
+__global__ void __launch_bounds__(256)
+k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
+               const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K, int row_vec,
+               int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
+  constexpr int kF = kBf16 ? 8 : 4;          // floats produced per 16-byte input vector
+  const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
+  const int lane = threadIdx.x & 31;
+  const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
+  const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
+  for (long long item = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+       item < n_items; item += warps) {
+    const int tl = (int)(item / n_slices);
+    const int sl = (int)(item - (long long)tl * n_slices);
+    const int p0 = (rg.t_begin + tl) * K;
+    int d = -1;
+    float wv = 0.f;
+    if (lane < K) {
+      d = __ldg(inv_l + p0 + lane);
+      if (d >= 0) d -= rg.row0;
+      wv = __ldg(w_l + p0 + lane);
+    }
+    const int v0 = sl * (32 * U) + lane;
+    float acc[U][kF];
+#pragma unroll
+    for (int u = 0; u < U; u++)
+#pragma unroll
+      for (int f = 0; f < kF; f++) acc[u][f] = 0.f;
+
+    for (int k0 = 0; k0 < K; k0 += KB) {
+      int4 r[KB][U];
+      float wk[KB];
+      bool on[KB];
+#pragma unroll
+      for (int kk = 0; kk < KB; kk++) {
+        const int k = k0 + kk;
+        const int dk = __shfl_sync(0xffffffffu, d, k & 31);
+        wk[kk] = __shfl_sync(0xffffffffu, wv, k & 31);
+        on[kk] = (k < K) && (dk >= 0);
+        const int4 *src = eo + (size_t)(on[kk] ? dk : 0) * row_vec;
+#pragma unroll
+        for (int u = 0; u < U; u++)
+          if (on[kk] && v0 + u * 32 < row_vec) r[kk][u] = ld16_stream(src + v0 + u * 32);
+      }
+#pragma unroll
+      for (int kk = 0; kk < KB; kk++) {
+        if (!on[kk]) continue;
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+          if (kBf16) {
+            acc[u][0] = __fmaf_rn(wk[kk], bf16_lo(r[kk][u].x), acc[u][0]);
+            acc[u][1] = __fmaf_rn(wk[kk], bf16_hi(r[kk][u].x), acc[u][1]);
+            acc[u][2] = __fmaf_rn(wk[kk], bf16_lo(r[kk][u].y), acc[u][2]);
+            acc[u][3] = __fmaf_rn(wk[kk], bf16_hi(r[kk][u].y), acc[u][3]);
+            acc[u][4] = __fmaf_rn(wk[kk], bf16_lo(r[kk][u].z), acc[u][4]);
+            acc[u][5] = __fmaf_rn(wk[kk], bf16_hi(r[kk][u].z), acc[u][5]);
+            acc[u][6] = __fmaf_rn(wk[kk], bf16_lo(r[kk][u].w), acc[u][6]);
+            acc[u][7] = __fmaf_rn(wk[kk], bf16_hi(r[kk][u].w), acc[u][7]);
+          } else {
+            acc[u][0] = __fmaf_rn(wk[kk], __int_as_float(r[kk][u].x), acc[u][0]);
+            acc[u][1] = __fmaf_rn(wk[kk], __int_as_float(r[kk][u].y), acc[u][1]);
+            acc[u][2] = __fmaf_rn(wk[kk], __int_as_float(r[kk][u].z), acc[u][2]);
+            acc[u][3] = __fmaf_rn(wk[kk], __int_as_float(r[kk][u].w), acc[u][3]);
+          }
+        }
+      }
+    }
+    // fp32 row of token tl: row_vec * kF floats = row_vec * kF / 4 float4
+    float4 *dst = y + (size_t)tl * row_vec * (kF / 4);
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+      const int v = v0 + u * 32;
+      if (v < row_vec) {
+        int4 o;
+        o.x = __float_as_int(acc[u][0]); o.y = __float_as_int(acc[u][1]);
+        o.z = __float_as_int(acc[u][2]); o.w = __float_as_int(acc[u][3]);
+        st16_stream(dst + (size_t)v * (kF / 4), o);
+        if (kBf16) {
+          o.x = __float_as_int(acc[u][4]); o.y = __float_as_int(acc[u][5]);
+          o.z = __float_as_int(acc[u][6]); o.w = __float_as_int(acc[u][7]);
+          st16_stream(dst + (size_t)v * 2 + 1, o);
+        }
+      }
+    }
+  }
+}
+
+// ---- launch configuration -------------------------------------------------------------------------
+static int g_dispatch_u = 0;        // 0 = auto
+static int g_combine_u = 0;         // 0 = auto
+static int g_dispatch_cta_per_sm = 0, g_combine_cta_per_sm = 0;
+
+template <typename Kern>
+static int occupancy_ctas(Kern kern, int threads) {
+  int n = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, threads, 0) != cudaSuccess || n <= 0) n = 1;
+  return n;
+}
+
+template <int U>
+static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
+                           int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
+  static int occ = 0;
+  if (!occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
+  const int per_sm = g_dispatch_cta_per_sm > 0 ? g_dispatch_cta_per_sm : occ;
+  const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
+  k_dispatch_rows<U><<<num_sms() * per_sm, 256, 0, st>>>(inv_l, mb_off, mb_begin, mb_end, d.K,
+                                                         d.row_vec, n_slices, (const int4 *)x, perm,
+                                                         (int4 *)buf);
+  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}
+
+template <bool kBf16, int KB, int U>
+static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
+                          const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
+                          cudaStream_t st) {
+  static int occ = 0;
+  if (!occ) occ = occupancy_ctas(k_combine_rows<kBf16, KB, U>, 256);
+  const int per_sm = g_combine_cta_per_sm > 0 ? g_combine_cta_per_sm : occ;
+  const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
+  k_combine_rows<kBf16, KB, U><<<num_sms() * per_sm, 256, 0, st>>>(
+      inv_l, w_l, mb_off, mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)eo, (float4 *)y);
+  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}
+
+template <bool kBf16, int KB>
+static int launch_combine_u(int U, const Dims &d, const int32_t *inv_l, const float *w_l,
+                            const int32_t *mb_off, int mb_begin, int mb_end, const void *eo,
+                            float *y, cudaStream_t st) {
+  if (U >= 2) return launch_combine<kBf16, KB, 2>(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+  return launch_combine<kBf16, KB, 1>(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+}
+
+template <bool kBf16>
+static int launch_combine_kb(int KB, int U, const Dims &d, const int32_t *inv_l, const float *w_l,
+                             const int32_t *mb_off, int mb_begin, int mb_end, const void *eo,
+                             float *y, cudaStream_t st) {
+#define FOREMOE_KB_CASE(n) \
+  case n: return launch_combine_u<kBf16, n>(U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+  switch (KB) {
+    FOREMOE_KB_CASE(1) FOREMOE_KB_CASE(2) FOREMOE_KB_CASE(3) FOREMOE_KB_CASE(4)
+    FOREMOE_KB_CASE(5) FOREMOE_KB_CASE(6) FOREMOE_KB_CASE(7) FOREMOE_KB_CASE(8)
+  }
+#undef FOREMOE_KB_CASE
+  return FOREMOE_ERR_INVALID_ARG;
+}
+
+static int check_range(const Dims &d, int layer, int mb_begin, int mb_end) {
+  if (layer < 0 || layer >= d.L || mb_begin < 0 || mb_end > d.n_mb || mb_begin > mb_end)
+    return FOREMOE_ERR_INVALID_ARG;
+  return FOREMOE_OK;
+}
+
+}  // namespace foremoe
+
+using namespace foremoe;
+
+extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_data_variant(int dispatch_u, int dispatch_cta_per_sm,
+                                               int combine_u, int combine_cta_per_sm) {
+  g_dispatch_u = dispatch_u; g_dispatch_cta_per_sm = dispatch_cta_per_sm;
+  g_combine_u = combine_u; g_combine_cta_per_sm = combine_cta_per_sm;
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
+                                int32_t mb_end, const int32_t *mb_off, const int32_t *inv,
+                                const void *x, int32_t *perm, void *buf, int32_t *dev_status,
+                                void *stream) {
+  (void)dev_status;
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if ((rc = check_range(d, layer, mb_begin, mb_end))) return rc;
+  if (!mb_off || !inv || !x || !buf || !aligned(x, 16) || !aligned(buf, 16))
+    return FOREMOE_ERR_INVALID_ARG;
+  if (mb_begin == mb_end) return FOREMOE_OK;
+  const int32_t *inv_l = inv + (size_t)layer * d.T * d.K;
+  cudaStream_t st = (cudaStream_t)stream;
+  int U = g_dispatch_u;
+  if (U <= 0) U = d.row_vec >= 256 ? 8 : d.row_vec >= 128 ? 4 : d.row_vec >= 64 ? 2 : 1;
+  if (U >= 8) return launch_dispatch<8>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
+  if (U >= 4) return launch_dispatch<4>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
+  if (U >= 2) return launch_dispatch<2>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
+  return launch_dispatch<1>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_combine(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
+                               int32_t mb_end, const int32_t *mb_off, const int32_t *inv,
+                               const float *w, const void *expert_out, float *y,
+                               int32_t *dev_status, void *stream) {
+  (void)dev_status;
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if ((rc = check_range(d, layer, mb_begin, mb_end))) return rc;
+  if (!mb_off || !inv || !w || !expert_out || !y || !aligned(expert_out, 16) || !aligned(y, 16))
+    return FOREMOE_ERR_INVALID_ARG;
+  if (mb_begin == mb_end) return FOREMOE_OK;
+  const size_t lo = (size_t)layer * d.T * d.K;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int groups = (d.K + 7) / 8;
+  const int KB = (d.K + groups - 1) / groups;
+  int U = g_combine_u;
+  if (U <= 0) U = (d.row_vec >= 64 && KB <= 4) ? 2 : 1;
+  if (d.act_dtype == FOREMOE_ACT_BF16)
+    return launch_combine_kb<true>(KB, U, d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
+  return launch_combine_kb<false>(KB, U, d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
+}

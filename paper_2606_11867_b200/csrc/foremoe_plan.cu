@@ -1,0 +1,735 @@
+// Plan kernels of the ForeMoE hot path (sm_100a): load histogram (a1), Stage-4 integer quotas
+// (a2), replica assignment + stable counting-sort destinations (a3/a4).
+// Contract: include/foremoe.h.  Rule and readings: DESIGN.md sec. 3.
+#include <limits.h>
+
+#include "foremoe_common.cuh"
+
+namespace foremoe {
+
+// =============================================================================================
+// a1: load histogram  (w_{s,e}, PAPER.md:204 / :247, single source rank)
+//
+// Tiles are fixed token ranges of one layer; a tile may straddle micro-step boundaries, so it is
+// walked segment by segment, each segment counted into a shared-memory histogram and flushed to
+// hist[i][l][:] with one global atomic per non-zero bin.  Warp aggregation: lanes holding the same
+// expert id elect a leader that adds the group's population once (match.any), so a hot expert
+// costs one shared atomic per warp instead of a serialised same-bank burst.
+// =============================================================================================
+template <bool kWarpAgg>
+__global__ void __launch_bounds__(256)
+k_load_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off, int L, int T, int K,
+            int E, int n_mb, int tile_tokens, int tiles_per_layer, int32_t *__restrict__ hist,
+            int32_t *dev_status) {
+  extern __shared__ int32_t sh[];   // [E]
+  const int tid = threadIdx.x;
+  const int lane = tid & 31;
+
+  // every CTA validates the boundaries itself (n_mb + 1 ints): no workspace in this entry point
+  int bad = 0;
+  for (int i = tid; i <= n_mb; i += blockDim.x) {
+    int v = mb_off[i];
+    if (i == 0 && v != 0) bad = 1;
+    if (i == n_mb && v != T) bad = 1;
+    if (i < n_mb && mb_off[i + 1] < v) bad = 1;
+  }
+  bad = __syncthreads_or(bad);
+  if (bad) {
+    if (blockIdx.x == 0 && tid == 0) raise_fault(dev_status, FOREMOE_FAULT_MB_OFF);
+    return;
+  }
+
+  int fault = 0;
+  const int n_tiles = L * tiles_per_layer;
+  for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int l = tile / tiles_per_layer;
+    int t0 = (tile - l * tiles_per_layer) * tile_tokens;
+    const int t1 = min(T, t0 + tile_tokens);
+    if (t0 >= t1) continue;
+    int i = find_range(mb_off, n_mb, t0);
+    const int32_t *lids = ids + (size_t)l * T * K;
+    while (t0 < t1) {
+      const int seg_end = min(t1, __ldg(mb_off + i + 1));
+      for (int e = tid; e < E; e += blockDim.x) sh[e] = 0;
+      __syncthreads();
+      const int p1 = seg_end * K;
+      // uniform trip count so that every lane takes part in match.any
+      for (int p = t0 * K + tid - lane; p < p1; p += blockDim.x) {
+        const int pp = p + lane;
+        int e = pp < p1 ? __ldg(lids + pp) : -1;
+        const bool ok = (unsigned)e < (unsigned)E;
+        if (pp < p1 && !ok) fault = FOREMOE_FAULT_ID_RANGE;
+        if (kWarpAgg) {
+          const unsigned key = ok ? (unsigned)e : (0x80000000u | lane);
+          const unsigned grp = __match_any_sync(0xffffffffu, key);
+          if (ok && lane == __ffs(grp) - 1) atomicAdd(&sh[e], __popc(grp));
+        } else {
+          if (ok) atomicAdd(&sh[e], 1);
+        }
+      }
+      __syncthreads();
+      int32_t *dst = hist + ((size_t)i * L + l) * E;
+      for (int e = tid; e < E; e += blockDim.x) {
+        const int v = sh[e];
+        if (v) atomicAdd(dst + e, v);
+      }
+      __syncthreads();
+      t0 = seg_end;
+      ++i;
+      while (i < n_mb && __ldg(mb_off + i + 1) <= t0) ++i;   // skip empty micro-steps
+    }
+  }
+  if (fault) raise_fault(dev_status, fault);
+}
+
+// step aggregate  w-bar_{s,e} = sum_i w^{(i)}_{s,e}
+__global__ void k_step_hist(const int32_t *__restrict__ hist, int n_mb, int LE,
+                            int64_t *__restrict__ step_hist) {
+  const int x = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x >= LE) return;
+  int64_t s = 0;
+  for (int i = 0; i < n_mb; i++) s += hist[(size_t)i * LE + x];
+  step_hist[x] = s;
+}
+
+// =============================================================================================
+// assign, step 0: micro-step tables.  chunk_off[i] = number of ranking chunks before micro-step i
+// (a chunk = up to tpc consecutive tokens of ONE instance).  One CTA.
+// =============================================================================================
+__global__ void k_mb_tables(const int32_t *__restrict__ mb_off, int n_mb, int T, int tpc,
+                            int32_t *__restrict__ chunk_off, int32_t *__restrict__ mb_ok,
+                            int32_t *dev_status) {
+  int bad = 0;
+  for (int i = threadIdx.x; i <= n_mb; i += blockDim.x) {
+    int v = mb_off[i];
+    if (i == 0 && v != 0) bad = 1;
+    if (i == n_mb && v != T) bad = 1;
+    if (i < n_mb && mb_off[i + 1] < v) bad = 1;
+  }
+  bad = __syncthreads_or(bad);
+  if (threadIdx.x == 0) {
+    *mb_ok = !bad;
+    int run = 0;
+    for (int i = 0; i < n_mb; i++) {
+      chunk_off[i] = run;
+      if (!bad) run += (mb_off[i + 1] - mb_off[i] + tpc - 1) / tpc;
+    }
+    chunk_off[n_mb] = run;
+    if (bad) raise_fault(dev_status, FOREMOE_FAULT_MB_OFF);
+  }
+}
+
+// =============================================================================================
+// assign, step 1: per-placement tables.  One CTA per placement (layer, or (micro-step, layer)).
+//   host_ptr/host_slot : CSR list of ALL slots holding expert e, ascending slot index
+//   active[j]          : slot j is the lowest-indexed slot of its expert on its rank (reading 10)
+//   rslot[r*Ns + s]    : active slots of rank r ordered by ascending expert id, then -1 padding
+// =============================================================================================
+__global__ void __launch_bounds__(256)
+k_placement_tables(const int32_t *__restrict__ slot_expert, int E, int S, int Ns, int P,
+                   int32_t *__restrict__ host_ptr, int32_t *__restrict__ host_slot,
+                   int32_t *__restrict__ active, int32_t *__restrict__ rslot,
+                   int32_t *__restrict__ pl_fault, int32_t *dev_status) {
+  extern __shared__ int32_t sm[];
+  int32_t *se = sm;            // [S]
+  int32_t *cnt = sm + S;       // [E+1]
+  int32_t *act = cnt + E + 1;  // [S]
+  const int pl = blockIdx.x;
+  const int32_t *src = slot_expert + (size_t)pl * S;
+  host_ptr += (size_t)pl * (E + 1);
+  host_slot += (size_t)pl * S;
+  active += (size_t)pl * S;
+  rslot += (size_t)pl * S;
+
+  int bad = 0;
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {
+    int e = src[j];
+    if (e < -1 || e >= E) { bad = 1; e = -1; }
+    se[j] = e;
+  }
+  bad = __syncthreads_or(bad);
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    int n = 0;
+    for (int j = 0; j < S; j++) n += (se[j] == e);
+    cnt[e] = n;
+  }
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {
+    const int e = se[j];
+    int a = e >= 0;
+    for (int j2 = (j / Ns) * Ns; j2 < j; j2++) a &= (se[j2] != e);
+    act[j] = a;
+    active[j] = a;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int run = 0;
+    for (int e = 0; e < E; e++) { int n = cnt[e]; cnt[e] = run; run += n; }
+    cnt[E] = run;
+    pl_fault[pl] = bad;
+    if (bad) raise_fault(dev_status, FOREMOE_FAULT_SLOT_EXPERT);
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e <= E; e += blockDim.x) host_ptr[e] = cnt[e];
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    int pos = cnt[e];
+    for (int j = 0; j < S; j++)
+      if (se[j] == e) host_slot[pos++] = j;
+  }
+  // active slots of each rank by ascending expert id (they hold distinct experts)
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {
+    const int r0 = (j / Ns) * Ns;
+    if (act[j]) {
+      int pos = 0;
+      for (int j2 = r0; j2 < r0 + Ns; j2++) pos += (act[j2] && se[j2] < se[j]);
+      rslot[r0 + pos] = j;
+    }
+    int n_act = 0;
+    for (int j2 = r0; j2 < r0 + Ns; j2++) n_act += act[j2];
+    if (j - r0 >= n_act) rslot[j] = -1;
+  }
+}
+
+// =============================================================================================
+// assign, step 2: per-chunk expert counts (input of the stable ranking).
+// grid (max_chunks, L).
+// =============================================================================================
+struct ChunkInfo { int i, t0, t1; };
+
+__device__ __forceinline__ bool locate_chunk(const int32_t *__restrict__ chunk_off,
+                                             const int32_t *__restrict__ mb_off, int n_mb, int tpc,
+                                             int c, ChunkInfo *ci) {
+  if (c >= __ldg(chunk_off + n_mb)) return false;
+  const int i = find_range(chunk_off, n_mb, c);
+  ci->i = i;
+  ci->t0 = __ldg(mb_off + i) + (c - __ldg(chunk_off + i)) * tpc;
+  ci->t1 = min(__ldg(mb_off + i + 1), ci->t0 + tpc);
+  return true;
+}
+
+__global__ void __launch_bounds__(kChunkThreads)
+k_chunk_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off,
+             const int32_t *__restrict__ chunk_off, int L, int T, int K, int E, int n_mb, int tpc,
+             int max_chunks, int32_t *__restrict__ chunk_cnt) {
+  extern __shared__ int32_t sh[];   // [E]
+  ChunkInfo ci;
+  const int c = blockIdx.x, l = blockIdx.y;
+  if (!locate_chunk(chunk_off, mb_off, n_mb, tpc, c, &ci)) return;
+  for (int e = threadIdx.x; e < E; e += blockDim.x) sh[e] = 0;
+  __syncthreads();
+  const int32_t *src = ids + ((size_t)l * T + ci.t0) * K;
+  const int np = (ci.t1 - ci.t0) * K;
+  for (int p = threadIdx.x; p < np; p += blockDim.x) {
+    const int e = __ldg(src + p);
+    if ((unsigned)e < (unsigned)E) atomicAdd(&sh[e], 1);
+  }
+  __syncthreads();
+  int32_t *dst = chunk_cnt + ((size_t)l * max_chunks + c) * E;
+  for (int e = threadIdx.x; e < E; e += blockDim.x) dst[e] = sh[e];
+}
+
+// =============================================================================================
+// assign, step 3: one CTA per instance.
+//   warp 0   : Stage-4 integer quotas by the exact water-filling rule (O2):
+//              Phase A forced loads, Phase B Gauss-Seidel water-filling passes to a fixpoint
+//              ("assign each token unit to the replica whose rank has the
+//              smallest accumulated load", :844-846), Phase C unit augmentations.
+//   warps 1+ : exclusive scan of the instance's chunk counts over chunks (per expert).
+// then quota / rank_load / slot_off and the pair-lookup tables are written by all threads.
+// =============================================================================================
+struct QuotaSmem {
+  int32_t *c, *q, *load, *se, *act, *hptr, *hslot, *rslot, *R, *nact, *visited, *par_rank,
+      *par_from, *par_to, *queue, *soff;
+};
+
+// One replicated expert: closed form of the unit-by-unit fill.  With host loads l_j (the expert's
+// own quota removed), lam = largest integer with sum_j max(0, lam - l_j) <= c; every host gets
+// max(0, lam - l_j); the remaining units go one each to the first hosts (ascending slot index)
+// among {l_j <= lam}.  Run by one lane.
+__device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e, int Ns) {
+  const int a0 = s.hptr[e], a1 = s.hptr[e + 1];
+  int cur = INT_MAX;
+  for (int a = a0; a < a1; a++) {
+    const int j = s.hslot[a];
+    if (!s.act[j]) continue;
+    const int r = j / Ns;
+    const int lj = s.load[r] - s.q[j];
+    s.load[r] = lj;
+    cur = min(cur, lj);
+  }
+  int64_t rem = s.c[e];
+  int lam;
+  for (;;) {
+    int m = 0, nxt = INT_MAX;
+    for (int a = a0; a < a1; a++) {
+      const int j = s.hslot[a];
+      if (!s.act[j]) continue;
+      const int lj = s.load[j / Ns];
+      if (lj <= cur) m++; else nxt = min(nxt, lj);
+    }
+    if (nxt == INT_MAX || rem < (int64_t)(nxt - cur) * m) {
+      lam = cur + (int)(rem / m);
+      rem = rem % m;
+      break;
+    }
+    rem -= (int64_t)(nxt - cur) * m;
+    cur = nxt;
+  }
+  int changed = 0;
+  for (int a = a0; a < a1; a++) {
+    const int j = s.hslot[a];
+    if (!s.act[j]) continue;
+    const int r = j / Ns;
+    const int lj = s.load[r];
+    int g = 0;
+    if (lj <= lam) {
+      g = lam - lj;
+      if (rem > 0) { g++; rem--; }
+    }
+    changed |= (g != s.q[j]);
+    s.q[j] = g;
+    s.load[r] = lj + g;
+  }
+  return changed;
+}
+
+// Phase C: while the lowest max-load rank h reaches (breadth first, ranks expanded through
+// replicated experts in ascending expert id, hosts in ascending slot index) a rank with
+// load <= max - 2, move one unit along the path.  Run by one lane.
+__device__ __forceinline__ void augment_units(const QuotaSmem &s, int P, int Ns) {
+  for (;;) {
+    int mx = INT_MIN, h = 0;
+    for (int r = 0; r < P; r++)
+      if (s.load[r] > mx) { mx = s.load[r]; h = r; }
+    for (int r = 0; r < P; r++) s.visited[r] = 0;
+    int head = 0, tail = 0, target = -1;
+    s.visited[h] = 1; s.queue[tail++] = h; s.par_rank[h] = -1;
+    while (head < tail && target < 0) {
+      const int r = s.queue[head++];
+      for (int k = 0; k < Ns && target < 0; k++) {
+        const int j = s.rslot[r * Ns + k];
+        if (j < 0) break;
+        const int e = s.se[j];
+        if (s.nact[e] < 2 || s.q[j] <= 0) continue;
+        for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
+          const int j2 = s.hslot[a];
+          if (!s.act[j2]) continue;
+          const int r2 = j2 / Ns;
+          if (s.visited[r2]) continue;
+          s.visited[r2] = 1; s.par_rank[r2] = r; s.par_from[r2] = j; s.par_to[r2] = j2;
+          s.queue[tail++] = r2;
+          if (s.load[r2] <= mx - 2) { target = r2; break; }
+        }
+      }
+    }
+    if (target < 0) return;
+    for (int r2 = target; s.par_rank[r2] >= 0; r2 = s.par_rank[r2]) {
+      s.q[s.par_from[r2]] -= 1;
+      s.q[s.par_to[r2]] += 1;
+    }
+    s.load[h] -= 1;
+    s.load[target] += 1;
+  }
+}
+
+__global__ void __launch_bounds__(kQuotaThreads)
+k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
+        const int32_t *__restrict__ mb_ok, const int32_t *__restrict__ chunk_off,
+        const int32_t *__restrict__ pl_host_ptr, const int32_t *__restrict__ pl_host_slot,
+        const int32_t *__restrict__ pl_active, const int32_t *__restrict__ pl_rslot,
+        const int32_t *__restrict__ pl_fault, const int32_t *__restrict__ slot_expert, int L, int E,
+        int P, int Ns, int pl_per_mb, int max_chunks, int32_t *__restrict__ quota,
+        int32_t *__restrict__ rank_load, int32_t *__restrict__ slot_off,
+        int32_t *__restrict__ inst_cum_end, int32_t *__restrict__ inst_slot_adj,
+        int32_t *__restrict__ inst_ok, int32_t *__restrict__ chunk_cnt, int32_t *dev_status) {
+  extern __shared__ int32_t sm[];
+  const int S = P * Ns;
+  const int inst = blockIdx.x;
+  const int i = inst / L, l = inst - i * L;
+  const int pl = pl_per_mb ? inst : l;
+  const int tid = threadIdx.x, nt = blockDim.x;
+  if (!*mb_ok) return;
+
+  QuotaSmem s;
+  int32_t *p = sm;
+  s.c = p; p += E;
+  s.nact = p; p += E;
+  s.R = p; p += E;
+  s.hptr = p; p += E + 1;
+  s.q = p; p += S;
+  s.se = p; p += S;
+  s.act = p; p += S;
+  s.hslot = p; p += S;
+  s.rslot = p; p += S;
+  s.soff = p; p += S + 1;
+  s.load = p; p += P;
+  s.visited = p; p += P;
+  s.par_rank = p; p += P;
+  s.par_from = p; p += P;
+  s.par_to = p; p += P;
+  s.queue = p; p += P;
+  __shared__ int nR_raw;
+
+  for (int e = tid; e < E; e += nt) s.c[e] = hist[(size_t)inst * E + e];
+  for (int e = tid; e <= E; e += nt) s.hptr[e] = pl_host_ptr[(size_t)pl * (E + 1) + e];
+  for (int j = tid; j < S; j += nt) {
+    int e = slot_expert[(size_t)pl * S + j];
+    s.se[j] = (e < -1 || e >= E) ? -1 : e;
+    s.act[j] = pl_active[(size_t)pl * S + j];
+    s.hslot[j] = pl_host_slot[(size_t)pl * S + j];
+    s.rslot[j] = pl_rslot[(size_t)pl * S + j];
+    s.q[j] = 0;
+  }
+  for (int r = tid; r < P; r += nt) s.load[r] = 0;
+  if (tid == 0) nR_raw = 0;
+  __syncthreads();
+
+  int fault = pl_fault[pl] ? FOREMOE_FAULT_SLOT_EXPERT : 0;
+  for (int e = tid; e < E; e += nt) {
+    int n = 0;
+    for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) n += s.act[s.hslot[a]];
+    s.nact[e] = n;
+    if (s.c[e] < 0) fault |= FOREMOE_FAULT_ID_RANGE;
+    if (s.c[e] > 0 && n == 0) fault |= FOREMOE_FAULT_NO_HOST;
+  }
+  if (quota_in) {
+    const int32_t *qi = quota_in + (size_t)inst * S;
+    for (int j = tid; j < S; j += nt) {
+      const int v = qi[j];
+      if (v < 0 || (s.se[j] < 0 && v != 0)) fault |= FOREMOE_FAULT_QUOTA_IN;
+      s.q[j] = v;
+    }
+    for (int e = tid; e < E; e += nt) {
+      int64_t sum = 0;
+      for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) sum += qi[s.hslot[a]];
+      if (sum != s.c[e]) fault |= FOREMOE_FAULT_QUOTA_IN;
+    }
+  }
+  // every lane of a warp that saw a fault raises it once per warp
+  {
+    unsigned any = __reduce_or_sync(0xffffffffu, (unsigned)fault);
+    if ((tid & 31) == 0 && any) raise_fault(dev_status, (int)any);
+  }
+  const int any_fault = __syncthreads_or(fault);
+
+  if (any_fault) {
+    // outputs of a faulted instance: all-zero plan, pairs get -1
+    for (int j = tid; j < S; j += nt) quota[(size_t)inst * S + j] = 0;
+    for (int j = tid; j <= S; j += nt) slot_off[(size_t)inst * (S + 1) + j] = 0;
+    for (int r = tid; r < P; r += nt) rank_load[(size_t)inst * P + r] = 0;
+    if (tid == 0) inst_ok[inst] = 0;
+    return;
+  }
+
+  if (!quota_in) {
+    // Phase A: forced load of singly hosted experts; collect the replicated set
+    for (int e = tid; e < E; e += nt) {
+      if (s.nact[e] == 1) {
+        for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
+          const int j = s.hslot[a];
+          if (s.act[j]) { s.q[j] = s.c[e]; atomicAdd(&s.load[j / Ns], s.c[e]); }
+        }
+      } else if (s.nact[e] >= 2) {
+        s.soff[atomicAdd(&nR_raw, 1)] = e;    // soff doubles as the unsorted list (|R| <= S/2)
+      }
+    }
+    __syncthreads();
+    const int nR = nR_raw;
+    // processing order: descending count, ties ascending expert id (reading 3) -- rank sort
+    for (int a = tid; a < nR; a += nt) {
+      const int e = s.soff[a], ce = s.c[e];
+      int pos = 0;
+      for (int b = 0; b < nR; b++) {
+        const int e2 = s.soff[b], c2 = s.c[e2];
+        pos += (c2 > ce) || (c2 == ce && e2 < e);
+      }
+      s.R[pos] = e;
+    }
+    __syncthreads();
+    if (tid == 0) {
+      // Phase B: Gauss-Seidel water-filling to a fixpoint
+      for (int pass = 0; pass < kMaxWaterPasses; pass++) {
+        int changed = 0;
+        for (int a = 0; a < nR; a++) changed |= water_fill_expert(s, s.R[a], Ns);
+        if (!changed) break;
+      }
+      // Phase C: exactness cleanup
+      augment_units(s, P, Ns);
+    }
+  }
+  if (tid >= 32) {
+    // exclusive scan over the instance's chunks, per expert (in place)
+    const int c0 = chunk_off[i], c1 = chunk_off[i + 1];
+    int32_t *cc = chunk_cnt + (size_t)l * max_chunks * E;
+    for (int e = tid - 32; e < E; e += nt - 32) {
+      int run = 0;
+      int c = c0;
+      for (; c + 4 <= c1; c += 4) {
+        const int v0 = cc[(size_t)c * E + e], v1 = cc[(size_t)(c + 1) * E + e];
+        const int v2 = cc[(size_t)(c + 2) * E + e], v3 = cc[(size_t)(c + 3) * E + e];
+        cc[(size_t)c * E + e] = run; run += v0;
+        cc[(size_t)(c + 1) * E + e] = run; run += v1;
+        cc[(size_t)(c + 2) * E + e] = run; run += v2;
+        cc[(size_t)(c + 3) * E + e] = run; run += v3;
+      }
+      for (; c < c1; c++) {
+        const int v = cc[(size_t)c * E + e];
+        cc[(size_t)c * E + e] = run; run += v;
+      }
+    }
+  }
+  __syncthreads();
+
+  // outputs
+  if (tid == 0) {
+    int run = 0;
+    for (int j = 0; j < S; j++) { s.soff[j] = run; run += s.q[j]; }
+    s.soff[S] = run;
+    inst_ok[inst] = 1;
+  }
+  __syncthreads();
+  for (int j = tid; j < S; j += nt) quota[(size_t)inst * S + j] = s.q[j];
+  for (int j = tid; j <= S; j += nt) slot_off[(size_t)inst * (S + 1) + j] = s.soff[j];
+  for (int r = tid; r < P; r += nt)
+    rank_load[(size_t)inst * P + r] = s.soff[(r + 1) * Ns] - s.soff[r * Ns];
+  // pair lookup: a pair of expert e with stable rank n goes to the first host slot j (ascending)
+  // with n < cum_end[j]; its row inside the instance is slot_adj[j] + n
+  for (int e = tid; e < E; e += nt) {
+    int cum = 0;
+    for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
+      const int j = s.hslot[a];
+      inst_slot_adj[(size_t)inst * S + j] = s.soff[j] - cum;
+      cum += s.q[j];
+      inst_cum_end[(size_t)inst * S + j] = cum;
+    }
+  }
+}
+
+// =============================================================================================
+// assign, step 4: stable rank of every pair among its expert's pairs of the instance, then the
+// slot (a3) and the destination row (a4).  One CTA per chunk; each warp owns a contiguous segment
+// of the chunk, so the order (chunk, warp, iteration, lane) is the (t, k) order.
+// grid (max_chunks, L).
+// =============================================================================================
+__global__ void __launch_bounds__(kChunkThreads)
+k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off,
+               const int32_t *__restrict__ chunk_off, const int32_t *__restrict__ pl_host_ptr,
+               const int32_t *__restrict__ pl_host_slot, const int32_t *__restrict__ inst_cum_end,
+               const int32_t *__restrict__ inst_slot_adj, const int32_t *__restrict__ inst_ok,
+               const int32_t *__restrict__ chunk_cnt, int L, int T, int K, int E, int S, int n_mb,
+               int tpc, int max_chunks, int pl_per_mb, int32_t *__restrict__ pair_slot,
+               int32_t *__restrict__ inv, int32_t *dev_status) {
+  extern __shared__ int32_t sm[];
+  int32_t *hptr = sm;                 // [E+1]
+  int32_t *hslot = hptr + E + 1;      // [S]
+  int32_t *cum_end = hslot + S;       // [S]
+  int32_t *slot_adj = cum_end + S;    // [S]
+  int32_t *wcnt = slot_adj + S;       // [kChunkWarps][E]
+  ChunkInfo ci;
+  const int c = blockIdx.x, l = blockIdx.y;
+  if (!locate_chunk(chunk_off, mb_off, n_mb, tpc, c, &ci)) return;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int inst = ci.i * L + l;
+  const int pl = pl_per_mb ? inst : l;
+  const size_t pbase = ((size_t)l * T + ci.t0) * K;
+  const int np = (ci.t1 - ci.t0) * K;
+  int32_t *o_slot = pair_slot + pbase, *o_inv = inv + pbase;
+  if (!inst_ok[inst]) {
+    for (int p = tid; p < np; p += blockDim.x) { o_slot[p] = -1; o_inv[p] = -1; }
+    return;
+  }
+  for (int e = tid; e <= E; e += blockDim.x) hptr[e] = pl_host_ptr[(size_t)pl * (E + 1) + e];
+  for (int j = tid; j < S; j += blockDim.x) {
+    hslot[j] = pl_host_slot[(size_t)pl * S + j];
+    cum_end[j] = inst_cum_end[(size_t)inst * S + j];
+    slot_adj[j] = inst_slot_adj[(size_t)inst * S + j];
+  }
+  for (int x = tid; x < kChunkWarps * E; x += blockDim.x) wcnt[x] = 0;
+  __syncthreads();
+
+  constexpr int kIter = kChunkPairs / kChunkThreads;   // 32-pair groups per warp
+  const int32_t *src = ids + pbase;
+  const int seg0 = warp * (kIter * 32);
+  int my[kIter];
+#pragma unroll
+  for (int it = 0; it < kIter; it++) {
+    const int p = seg0 + it * 32 + lane;
+    my[it] = p < np ? __ldg(src + p) : -1;
+  }
+  int32_t *wc = wcnt + warp * E;
+#pragma unroll
+  for (int it = 0; it < kIter; it++)
+    if ((unsigned)my[it] < (unsigned)E) atomicAdd(&wc[my[it]], 1);
+  __syncthreads();
+  // exclusive scan over warps, seeded with the chunk's base (pairs of e in earlier chunks)
+  const int32_t *cbase = chunk_cnt + ((size_t)l * max_chunks + c) * E;
+  for (int e = tid; e < E; e += blockDim.x) {
+    int run = cbase[e];
+#pragma unroll
+    for (int w = 0; w < kChunkWarps; w++) {
+      const int v = wcnt[w * E + e];
+      wcnt[w * E + e] = run;
+      run += v;
+    }
+  }
+  __syncthreads();
+
+  const int row_base = __ldg(mb_off + ci.i) * K;
+  const unsigned lt = (1u << lane) - 1u;
+  int fault = 0;
+#pragma unroll
+  for (int it = 0; it < kIter; it++) {
+    const int p = seg0 + it * 32 + lane;
+    const int e = my[it];
+    const bool ok = (unsigned)e < (unsigned)E;
+    const unsigned key = ok ? (unsigned)e : (0x80000000u | lane);
+    const unsigned grp = __match_any_sync(0xffffffffu, key);
+    int n = 0;
+    if (ok) n = wc[e] + __popc(grp & lt);
+    __syncwarp();
+    if (ok && lane == 31 - __clz(grp)) wc[e] = n + 1;   // last lane of the group advances the counter
+    __syncwarp();
+    if (p < np) {
+      int slot = -1, dst = -1;
+      if (ok) {
+        for (int a = hptr[e]; a < hptr[e + 1]; a++) {
+          const int j = hslot[a];
+          if (n < cum_end[j]) { slot = j; dst = row_base + slot_adj[j] + n; break; }
+        }
+        if (slot < 0) fault |= FOREMOE_FAULT_NO_HOST;
+      } else {
+        fault |= FOREMOE_FAULT_ID_RANGE;
+      }
+      o_slot[p] = slot;
+      o_inv[p] = dst;
+    }
+  }
+  if (fault) raise_fault(dev_status, fault);
+}
+
+}  // namespace foremoe
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+using namespace foremoe;
+
+namespace foremoe {
+int num_sms() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+      n = 0;
+      return 148;
+    }
+  }
+  return n;
+}
+}  // namespace foremoe
+
+extern "C" __attribute__((visibility("default"))) int foremoe_version(void) { return 100; }
+
+extern "C" __attribute__((visibility("default"))) int foremoe_workspace_bytes(const foremoe_shape_t *shape, size_t *bytes) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!bytes) return FOREMOE_ERR_INVALID_ARG;
+  *bytes = make_workspace(d).total;
+  return FOREMOE_OK;
+}
+
+static int g_hist_variant = 1;   // 1 = warp-aggregated (default), 0 = plain shared atomics
+extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_hist_variant(int v) { g_hist_variant = v; }
+
+extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const foremoe_shape_t *shape, const int32_t *ids,
+                                 const int32_t *mb_off, int32_t *hist, int64_t *step_hist,
+                                 int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!ids || !mb_off || !hist) return FOREMOE_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemsetAsync(hist, 0, sizeof(int32_t) * (size_t)d.n_inst * d.E, st) != cudaSuccess)
+    return FOREMOE_ERR_CUDA;
+  if (d.T > 0) {
+    // tile = 8192 pairs: 32 per thread; the flush is E atomics per tile segment
+    const int tile_tokens = (8192 + d.K - 1) / d.K;
+    const int tiles_per_layer = (d.T + tile_tokens - 1) / tile_tokens;
+    const long long n_tiles = (long long)tiles_per_layer * d.L;
+    const int grid = (int)(n_tiles < (long long)num_sms() * 8 ? n_tiles : (long long)num_sms() * 8);
+    const size_t smem = sizeof(int32_t) * d.E;
+    if (g_hist_variant)
+      k_load_hist<true><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb,
+                                                 tile_tokens, tiles_per_layer, hist, dev_status);
+    else
+      k_load_hist<false><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb,
+                                                  tile_tokens, tiles_per_layer, hist, dev_status);
+  }
+  if (step_hist) {
+    const int LE = d.L * d.E;
+    k_step_hist<<<(LE + 255) / 256, 256, 0, st>>>(hist, d.n_mb, LE, step_hist);
+  }
+  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_assign(const foremoe_shape_t *shape, const int32_t *ids,
+                              const int32_t *mb_off, const int32_t *hist,
+                              const int32_t *slot_expert, const int32_t *quota_in, int32_t *quota,
+                              int32_t *rank_load, int32_t *slot_off, int32_t *pair_slot,
+                              int32_t *inv, void *workspace, size_t workspace_bytes,
+                              int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !pair_slot ||
+      !inv || !workspace)
+    return FOREMOE_ERR_INVALID_ARG;
+  if (!aligned(workspace, 16)) return FOREMOE_ERR_INVALID_ARG;
+  const Workspace w = make_workspace(d);
+  if (workspace_bytes < w.total) return FOREMOE_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  char *ws = (char *)workspace;
+  int32_t *chunk_off = (int32_t *)(ws + w.chunk_off), *mb_ok = (int32_t *)(ws + w.mb_ok);
+  int32_t *pl_host_ptr = (int32_t *)(ws + w.pl_host_ptr);
+  int32_t *pl_host_slot = (int32_t *)(ws + w.pl_host_slot);
+  int32_t *pl_active = (int32_t *)(ws + w.pl_active), *pl_rslot = (int32_t *)(ws + w.pl_rslot);
+  int32_t *pl_fault = (int32_t *)(ws + w.pl_fault);
+  int32_t *inst_cum_end = (int32_t *)(ws + w.inst_cum_end);
+  int32_t *inst_slot_adj = (int32_t *)(ws + w.inst_slot_adj);
+  int32_t *inst_ok = (int32_t *)(ws + w.inst_ok), *chunk_cnt = (int32_t *)(ws + w.chunk_cnt);
+
+  const size_t smem_quota = sizeof(int32_t) * ((size_t)4 * d.E + 1 + (size_t)6 * d.S + 1 + (size_t)6 * d.P);
+  const size_t smem_pairs = sizeof(int32_t) * ((size_t)d.E + 1 + (size_t)3 * d.S + (size_t)kChunkWarps * d.E);
+  const size_t smem_pl = sizeof(int32_t) * ((size_t)2 * d.S + d.E + 1);
+  if (smem_quota > 200 * 1024 || smem_pairs > 200 * 1024 || smem_pl > 200 * 1024)
+    return FOREMOE_ERR_INVALID_ARG;
+  if (smem_quota > 48 * 1024 &&
+      cudaFuncSetAttribute(k_quota, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_quota) != cudaSuccess)
+    return FOREMOE_ERR_CUDA;
+  if (smem_pairs > 48 * 1024 &&
+      cudaFuncSetAttribute(k_assign_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_pairs) != cudaSuccess)
+    return FOREMOE_ERR_CUDA;
+  if (smem_pl > 48 * 1024 &&
+      cudaFuncSetAttribute(k_placement_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_pl) != cudaSuccess)
+    return FOREMOE_ERR_CUDA;
+
+  k_mb_tables<<<1, 256, 0, st>>>(mb_off, d.n_mb, d.T, d.tpc, chunk_off, mb_ok, dev_status);
+  k_placement_tables<<<d.n_pl, 256, smem_pl, st>>>(slot_expert, d.E, d.S, d.Ns, d.P, pl_host_ptr,
+                                                   pl_host_slot, pl_active, pl_rslot, pl_fault,
+                                                   dev_status);
+  const dim3 cgrid(d.max_chunks, d.L);
+  if (d.T > 0)
+    k_chunk_hist<<<cgrid, kChunkThreads, sizeof(int32_t) * d.E, st>>>(
+        ids, mb_off, chunk_off, d.L, d.T, d.K, d.E, d.n_mb, d.tpc, d.max_chunks, chunk_cnt);
+  k_quota<<<d.n_inst, kQuotaThreads, smem_quota, st>>>(
+      hist, quota_in, mb_ok, chunk_off, pl_host_ptr, pl_host_slot, pl_active, pl_rslot, pl_fault,
+      slot_expert, d.L, d.E, d.P, d.Ns, d.pl_per_mb, d.max_chunks, quota, rank_load, slot_off,
+      inst_cum_end, inst_slot_adj, inst_ok, chunk_cnt, dev_status);
+  if (d.T > 0)
+    k_assign_pairs<<<cgrid, kChunkThreads, smem_pairs, st>>>(
+        ids, mb_off, chunk_off, pl_host_ptr, pl_host_slot, inst_cum_end, inst_slot_adj, inst_ok,
+        chunk_cnt, d.L, d.T, d.K, d.E, d.S, d.n_mb, d.tpc, d.max_chunks, d.pl_per_mb, pair_slot,
+        inv, dev_status);
+  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}

@@ -1,0 +1,340 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element, on the same seeded inputs.  Bit-exact for every integer output and gathered row; the
+fp32 combine within max relative error 1e-6 (BASELINE.json north_star) -- and, since both sides
+use the same fma order (reading 16), bit-identical.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import foremoe_oracle as orc
+from paper_2606_11867_b200 import binding as fm
+from paper_2606_11867_b200 import synth
+from tests import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+
+def _full_check(cfg, layers=None, mbs=None, what=""):
+    ids, w, mb_off, se = G.make_case(cfg)
+    ref = G.oracle_plan(ids, mb_off, se, cfg.E, cfg.P, cfg.Ns)
+    assert ref["fault"] == 0
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    assert sp.faults() == 0
+    G.assert_plan_equal(sp, ref, what)
+    layers = range(cfg.L) if layers is None else layers
+    mbs = range(cfg.n_mb) if mbs is None else mbs
+    x = G.activations(cfg, mb_off, mbs)
+    G.check_data_path(sp, ref, x, layers, mbs, what)
+    return sp, ref
+
+
+def test_tiny_config1_everything(cuda_device):
+    """BASELINE.json config 1 in full: E=8, top-2, 8 x 512 tokens, 4 ranks x (2+1), H=256 fp32."""
+    _full_check(synth.config(1), what="cfg1")
+
+
+@pytest.mark.parametrize("cfg_id,kw", [
+    (2, dict(L=3, n_samples=12, sample_len=700, H=2048, mb_samples=4)),   # 2800 tok: ragged chunks
+    (3, dict(L=2, n_samples=6, sample_len=1100, H=7168, mb_samples=2)),
+    (5, dict(L=2, n_samples=3, sample_len=3000, H=4096, mb_samples=1)),   # K=10: 8-byte id rows
+    (4, dict(L=2, n_samples=24, H=2048, mb_samples=5)),                   # lognormal lengths
+    (4, dict(L=1, n_samples=9, H=512, mb_samples=1)),
+])
+def test_scaled_configs(cuda_device, cfg_id, kw):
+    """Reduced copies of configs 2-5: several ranking chunks, ragged tails, every instance."""
+    _full_check(synth.config(cfg_id).scaled(**kw), what=f"cfg{cfg_id}-scaled")
+
+
+def test_ranged_calls_equal_per_instance(cuda_device):
+    cfg = synth.config(2).scaled(L=2, n_samples=10, sample_len=333, H=256, mb_samples=3)
+    ids, w, mb_off, se = G.make_case(cfg)
+    ref = G.oracle_plan(ids, mb_off, se, cfg.E, cfg.P, cfg.Ns)
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    s = sp.shape
+    for (b, e) in [(0, cfg.n_mb), (1, 3), (2, 2)]:
+        a_tok, b_tok = int(mb_off[b]), int(mb_off[e])
+        n = b_tok - a_tok
+        x = synth.gen_activations(cfg, max(n, 1), 99, G.DEV)
+        perm = torch.full((max(n * s.K, 1),), -5, dtype=torch.int32, device=G.DEV)
+        buf = torch.zeros((max(n * s.K, 1), s.H), dtype=s.act_torch_dtype, device=G.DEV)
+        y = torch.zeros((max(n, 1), s.H), dtype=torch.float32, device=G.DEV)
+        for l in range(cfg.L):
+            sp.dispatch(l, b, e, x, perm, buf)
+            sp.combine(l, b, e, buf, y)
+            torch.cuda.synchronize()
+            if n == 0:
+                assert (perm == -5).all()
+                continue
+            perm_ref = ref["perm"][l, a_tok * s.K:b_tok * s.K]
+            assert (perm[:n * s.K].cpu().numpy() == perm_ref).all()
+            buf_ref = orc.gather(perm_ref, G.to_bits(x), s.K, pair_base=a_tok * s.K)
+            assert (G.to_bits(buf)[:n * s.K] == buf_ref).all()
+            y_ref = orc.combine(ref["inv"][l, a_tok:b_tok], w[l, a_tok:b_tok], buf_ref, s.act_dtype,
+                                row_base=a_tok * s.K)
+            assert (y[:n].cpu().numpy().view(np.uint32) == y_ref.view(np.uint32)).all()
+
+
+def test_combine_identity_pins_on_gpu(cuda_device):
+    """combine(dispatch(x)) with unit weights is exactly K*x; with w = 1/K exactly x (K = 8)."""
+    cfg = synth.config(2).scaled(L=1, n_samples=2, sample_len=600, H=1024, mb_samples=2)
+    ids, w, mb_off, se = G.make_case(cfg)
+    for wval, scale in ((1.0, float(cfg.K)), (1.0 / cfg.K, 1.0)):
+        sp = G.gpu_plan(fm.shape_of(cfg), ids, np.full_like(w, wval), mb_off, se)
+        n = cfg.T
+        x = synth.gen_activations(cfg, n, 5, G.DEV)
+        buf = torch.empty((n * cfg.K, cfg.H), dtype=torch.bfloat16, device=G.DEV)
+        y = torch.empty((n, cfg.H), dtype=torch.float32, device=G.DEV)
+        sp.dispatch(0, 0, 1, x, None, buf)
+        sp.combine(0, 0, 1, buf, y)
+        assert torch.equal(y, x.float() * scale)
+
+
+# ------------------------------------------------------------------ edge cases
+def _random_case(rng, L, E, K, P, Nr, mb_sizes, dup_tokens=False, empty_slots=True,
+                 same_rank_dup=True, skew=1.0):
+    Nb = E // P
+    Ns = Nb + Nr
+    S = P * Ns
+    T = int(sum(mb_sizes))
+    mb_off = np.concatenate([[0], np.cumsum(mb_sizes)]).astype(np.int32)
+    p = (np.arange(E) + 1.0) ** (-skew)
+    p /= p.sum()
+    ids = np.empty((L, T, K), dtype=np.int32)
+    for l in range(L):
+        perm = rng.permutation(E)
+        if dup_tokens:
+            ids[l] = perm[rng.choice(E, size=(T, K), p=p)]
+        else:
+            g = rng.gumbel(size=(T, E)) + np.log(p)[None, :]
+            ids[l] = perm[np.argsort(-g, axis=1)[:, :K]]
+    w = rng.random((L, T, K), dtype=np.float32)
+    se = np.full((L, S), -1, dtype=np.int32)
+    for l in range(L):
+        base = rng.permutation(E)
+        for r in range(P):
+            se[l, r * Ns:r * Ns + Nb] = base[r * Nb:(r + 1) * Nb]
+            for a in range(Nr):
+                u = rng.random()
+                if empty_slots and u < 0.2:
+                    continue
+                if same_rank_dup and u < 0.35:
+                    se[l, r * Ns + Nb + a] = se[l, r * Ns + rng.integers(Nb)]   # inactive duplicate
+                else:
+                    se[l, r * Ns + Nb + a] = rng.integers(E)
+    return ids, w, mb_off, se, Nb, Ns
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_small_plans(cuda_device, seed):
+    """Random placements with empty slots, same-rank duplicates, empty micro-steps, duplicate ids
+    inside a token, K in {1,2,3,8,10,32}: every integer output equals the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    K = [1, 2, 3, 8, 10, 32][seed]
+    E, P, Nr = [8, 16, 12, 64, 40, 64][seed], [2, 4, 3, 8, 5, 4][seed], [1, 2, 3, 2, 4, 0][seed]
+    mb_sizes = [int(v) for v in rng.integers(0, 900, size=7)]
+    mb_sizes[2] = 0
+    mb_sizes[5] = 1
+    ids, w, mb_off, se, Nb, Ns = _random_case(rng, 5, E, K, P, Nr, mb_sizes,
+                                              dup_tokens=(seed % 2 == 1), skew=1.0 + 0.3 * seed)
+    ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+    assert ref["fault"] == 0
+    shape = fm.Shape(L=5, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=7, H=64,
+                     act_dtype=fm.ACT_FP32)
+    sp = G.gpu_plan(shape, ids, w, mb_off, se)
+    assert sp.faults() == 0
+    G.assert_plan_equal(sp, ref, f"random{seed}")
+    x = {i: torch.randn((max(mb_sizes[i], 1), 64), device=G.DEV) for i in range(7)}
+    G.check_data_path(sp, ref, x, range(5), range(7), f"random{seed}")
+
+
+def test_quota_kernel_many_instances(cuda_device):
+    """The quota kernel against the oracle's unit-by-unit rule on 2 x 128 x 6 random instances
+    with many replicas: Phase B needs several passes and Phase C augmentations occur."""
+    for (E, P, Nr, K, skew) in [(16, 8, 2, 2, 0.5), (32, 8, 4, 3, 0.8)]:
+        rng = np.random.default_rng(7)
+        L, mb_sizes = 128, [1, 2, 3, 4, 6, 100]
+        n_mb = len(mb_sizes)
+        ids, w, mb_off, se, Nb, Ns = _random_case(rng, L, E, K, P, Nr, mb_sizes, skew=skew)
+        ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+        assert ref["fault"] == 0
+        moved = passes = 0
+        for i in range(n_mb):
+            for l in range(L):
+                _, _, _, (np_, mv), _ = orc.quota(ref["hist"][i, l], se[l], P, Ns)
+                passes = max(passes, np_)
+                moved += mv
+        assert passes >= 3 and moved >= 5      # the cases exercise Phase B iteration and Phase C
+        shape = fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=n_mb, H=8,
+                         act_dtype=fm.ACT_FP32)
+        sp = G.gpu_plan(shape, ids, w, mb_off, se)
+        assert sp.faults() == 0
+        G.assert_plan_equal(sp, ref, "quota-many")
+
+
+def test_max_skew_single_expert(cuda_device):
+    """Degenerate: every pair selects one of two experts (K=2), one of them replicated 3 times."""
+    E, P, Nb, Nr, K, T = 8, 4, 2, 1, 2, 5000
+    ids = np.zeros((1, T, K), dtype=np.int32)
+    ids[0, :, 1] = 5
+    se = np.array([[0, 1, 5, 2, 3, 5, 4, 5, -1, 6, 7, 5]], dtype=np.int32)
+    mb_off = np.array([0, 4097, 5000], dtype=np.int32)
+    w = np.ones((1, T, K), dtype=np.float32)
+    ref = G.oracle_plan(ids, mb_off, se, E, P, Nb + Nr)
+    sp = G.gpu_plan(fm.Shape(L=1, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=T, n_mb=2, H=8,
+                             act_dtype=fm.ACT_FP32), ids, w, mb_off, se)
+    assert sp.faults() == 0 and ref["fault"] == 0
+    G.assert_plan_equal(sp, ref, "max-skew")
+    x = {i: torch.randn((int(mb_off[i + 1] - mb_off[i]), 8), device=G.DEV) for i in range(2)}
+    G.check_data_path(sp, ref, x, [0], [0, 1], "max-skew")
+
+
+def test_per_microstep_placement(cuda_device):
+    """placement_mb_stride = L*S: one placement per (micro-step, layer) (A^{(i)})."""
+    rng = np.random.default_rng(3)
+    L, n_mb, E, P, Nr, K = 2, 3, 16, 4, 2, 4
+    mb_sizes = [300, 0, 1200]
+    cases = [_random_case(rng, L, E, K, P, Nr, mb_sizes) for _ in range(n_mb)]
+    ids, w, mb_off, _, Nb, Ns = cases[0]
+    se = np.stack([c[3] for c in cases])                    # [n_mb, L, S]
+    S = P * Ns
+    shape = fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=n_mb, H=8,
+                     act_dtype=fm.ACT_FP32, placement_mb_stride=L * S)
+    sp = G.gpu_plan(shape, ids, w, mb_off, se)
+    assert sp.faults() == 0
+    hist, _, _ = orc.load_hist(ids, mb_off, E)
+    for i in range(n_mb):
+        a, b = int(mb_off[i]), int(mb_off[i + 1])
+        for l in range(L):
+            q, rl, so, _, f = orc.quota(hist[i, l], se[i, l], P, Ns)
+            assert f == 0
+            ps, inv, perm, f = orc.assign_instance(ids[l, a:b], se[i, l], q, so, E, base=a * K)
+            assert f == 0
+            assert (sp.quota[i, l].cpu().numpy() == q).all()
+            assert (sp.rank_load[i, l].cpu().numpy() == rl).all()
+            assert (sp.slot_off[i, l].cpu().numpy() == so).all()
+            assert (sp.pair_slot[l, a:b].cpu().numpy().ravel() == ps).all()
+            assert (sp.inv[l, a:b].cpu().numpy().ravel() == inv).all()
+
+
+def test_caller_supplied_quota(cuda_device):
+    """quota_in: a valid caller quota (here: everything on the LAST host of each expert) is
+    honoured and validated by Eq.(8)/(9); an invalid one raises FAULT_QUOTA_IN."""
+    cfg = synth.config(2).scaled(L=2, n_samples=4, sample_len=500, H=128, mb_samples=2)
+    ids, w, mb_off, se = G.make_case(cfg)
+    hist, _, _ = orc.load_hist(ids, mb_off, cfg.E)
+    qin = np.zeros((cfg.n_mb, cfg.L, cfg.S), dtype=np.int32)
+    for l in range(cfg.L):
+        last = {int(e): j for j, e in enumerate(se[l]) if e >= 0}
+        for e, j in last.items():
+            qin[:, l, j] = hist[:, l, e]
+    ref = G.oracle_plan(ids, mb_off, se, cfg.E, cfg.P, cfg.Ns, quota_in=qin)
+    assert ref["fault"] == 0
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se, quota_in=qin)
+    assert sp.faults() == 0
+    G.assert_plan_equal(sp, ref, "quota_in")
+    bad = qin.copy()
+    j0 = int(np.argmax(bad[0, 0]))
+    bad[0, 0, j0] -= 1
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se, quota_in=bad)
+    assert sp.faults() & fm.FAULT_QUOTA_IN
+    assert G.oracle_plan(ids, mb_off, se, cfg.E, cfg.P, cfg.Ns, quota_in=bad)["fault"] & orc.FAULT_QUOTA_IN
+
+
+def test_device_faults(cuda_device):
+    cfg = synth.config(1)
+    ids, w, mb_off, se = G.make_case(cfg)
+    shape = fm.shape_of(cfg)
+    # id out of range: not counted, pair gets -1, other pairs still match the oracle
+    bad_ids = ids.copy()
+    bad_ids[0, 100, 1] = cfg.E + 3
+    bad_ids[0, 700, 0] = -1
+    ref = G.oracle_plan(bad_ids, mb_off, se, cfg.E, cfg.P, cfg.Ns)
+    sp = G.gpu_plan(shape, bad_ids, w, mb_off, se)
+    assert sp.faults() == fm.FAULT_ID_RANGE and ref["fault"] == orc.FAULT_ID_RANGE
+    G.assert_plan_equal(sp, ref, "bad-id")
+    # expert with tokens but no slot
+    se2 = se.copy()
+    victim = int(ids[0, 0, 0])
+    se2[se2 == victim] = -1
+    sp = G.gpu_plan(shape, ids, w, mb_off, se2)
+    assert sp.faults() & fm.FAULT_NO_HOST
+    assert (sp.inv.cpu().numpy() == -1).all() and (sp.quota.cpu().numpy() == 0).all()
+    # slot_expert out of range
+    se3 = se.copy()
+    se3[0, 1] = cfg.E
+    sp = G.gpu_plan(shape, ids, w, mb_off, se3)
+    assert sp.faults() & fm.FAULT_SLOT_EXPERT
+    # broken boundaries: histogram is all zero (as the oracle's), fault raised
+    mb_bad = mb_off.copy()
+    mb_bad[3] = mb_bad[2] - 1
+    sp = G.gpu_plan(shape, ids, w, mb_bad, se)
+    assert sp.faults() & fm.FAULT_MB_OFF
+    assert (sp.hist.cpu().numpy() == 0).all()
+    mb_bad = mb_off.copy()
+    mb_bad[-1] -= 1
+    sp = G.gpu_plan(shape, ids, w, mb_bad, se)
+    assert sp.faults() & fm.FAULT_MB_OFF
+
+
+def test_host_errors(cuda_device):
+    cfg = synth.config(1)
+    ids, w, mb_off, se = G.make_case(cfg)
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    s = sp.shape
+    import dataclasses
+    with pytest.raises(fm.ForeMoEError) as ei:
+        fm.workspace_bytes(dataclasses.replace(s, K=s.E + 1))
+    assert ei.value.code == fm.ERR_INVALID_ARG
+    with pytest.raises(fm.ForeMoEError) as ei:
+        fm.workspace_bytes(dataclasses.replace(s, Nb=s.Nb + 1))
+    assert ei.value.code == fm.ERR_INVALID_ARG
+    with pytest.raises(fm.ForeMoEError) as ei:
+        fm.workspace_bytes(dataclasses.replace(s, H=3))          # row bytes not a multiple of 16
+    assert ei.value.code == fm.ERR_INVALID_ARG
+    small = torch.empty(64, dtype=torch.uint8, device=G.DEV)
+    with pytest.raises(fm.ForeMoEError) as ei:
+        fm.assign(s, sp.ids, sp.mb_off, sp.hist, sp.slot_expert, None, sp.quota, sp.rank_load,
+                  sp.slot_off, sp.pair_slot, sp.inv, small, sp.status)
+    assert ei.value.code == fm.ERR_WORKSPACE
+    x = torch.zeros((512, s.H), device=G.DEV)
+    buf = torch.zeros((1024, s.H), device=G.DEV)
+    with pytest.raises(fm.ForeMoEError) as ei:
+        sp.dispatch(0, 3, 2, x, None, buf)
+    assert ei.value.code == fm.ERR_INVALID_ARG
+    with pytest.raises(fm.ForeMoEError) as ei:
+        sp.dispatch(1, 0, 1, x, None, buf)                      # layer out of range
+    assert ei.value.code == fm.ERR_INVALID_ARG
+    with pytest.raises(fm.ForeMoEError) as ei:
+        fm.dispatch(s, 0, 0, 1, sp.mb_off, sp.inv, x.view(-1)[1:].view(-1)[:511 * s.H].view(511, s.H),
+                    None, buf)                                    # misaligned x
+    assert ei.value.code == fm.ERR_INVALID_ARG
+
+
+def test_step_host_matches_device_path(cuda_device):
+    """foremoe_step_host (host buffers in, plan + last layer's y out) equals the device calls."""
+    cfg = synth.config(2).scaled(L=3, n_samples=6, sample_len=400, H=256, mb_samples=2)
+    ids, w, mb_off, se = G.make_case(cfg)
+    s = fm.shape_of(cfg)
+    ref = G.oracle_plan(ids, mb_off, se, cfg.E, cfg.P, cfg.Ns)
+    pin = lambda a, dt: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).pin_memory()
+    ids_h, w_h, mb_h, se_h = pin(ids, torch.int32), pin(w, torch.float32), pin(mb_off, torch.int32), pin(se, torch.int32)
+    x_h = synth.gen_activations(cfg, cfg.T, 1, "cpu").pin_memory()
+    q_h = torch.empty((s.n_mb, s.L, s.S), dtype=torch.int32).pin_memory()
+    rl_h = torch.empty((s.n_mb, s.L, s.P), dtype=torch.int32).pin_memory()
+    so_h = torch.empty((s.n_mb, s.L, s.S + 1), dtype=torch.int32).pin_memory()
+    y_h = torch.empty((s.T, s.H), dtype=torch.float32).pin_memory()
+    st_h = torch.full((1,), -1, dtype=torch.int32).pin_memory()
+    arena = torch.empty(fm.step_host_arena_bytes(s, mb_h) + 256, dtype=torch.uint8, device=G.DEV)
+    off = (-arena.data_ptr()) % 256
+    fm.step_host(s, ids_h, w_h, mb_h, se_h, x_h, q_h, rl_h, so_h, y_h, arena[off:], st_h)
+    assert int(st_h[0]) == 0
+    assert (q_h.numpy() == ref["quota"]).all() and (rl_h.numpy() == ref["rank_load"]).all()
+    assert (so_h.numpy() == ref["slot_off"]).all()
+    l = s.L - 1
+    xb = G.to_bits(x_h)
+    for i in range(s.n_mb):
+        a, b = int(mb_off[i]), int(mb_off[i + 1])
+        buf_ref = orc.gather(ref["perm"][l, a * s.K:b * s.K], xb[a:b], s.K, pair_base=a * s.K)
+        y_ref = orc.combine(ref["inv"][l, a:b], w[l, a:b], buf_ref, s.act_dtype, row_base=a * s.K)
+        assert (y_h[a:b].numpy().view(np.uint32) == y_ref.view(np.uint32)).all()

@@ -1,0 +1,406 @@
+#!/usr/bin/env python
+"""bench.py -- routed tokens/s of the ForeMoE plan + dispatch + combine path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one RL step's routing trace: foremoe_load_hist +
+foremoe_assign for the whole step, then foremoe_dispatch + foremoe_combine (identity expert:
+expert_out = buf) for every (layer, micro-step) instance.  Workload: BASELINE.json configs[1]
+(Qwen3-30B-A3B-shaped trace) unless --config says otherwise.  Prints ONE JSON line (rank 0).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload on this box's host cores: a baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from paper_2606_11867_b200 import multi, synth
+
+METRIC = "routed tokens/s (plan+dispatch+combine)"
+UNIT = "tokens/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json's "~8 TB/s" denominator, context only
+FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def bytes_per_token(cfg) -> dict:
+    """Algorithmic bytes per routed token (DESIGN.md sec. 6 / SURVEY.md sec. 8(d))."""
+    es = 2 if cfg.act_dtype == synth.ACT_BF16 else 4
+    return dict(plan=28 * cfg.K, dispatch=es * cfg.H * (1 + cfg.K) + 8 * cfg.K,
+                combine=cfg.H * (es * cfg.K + 4) + 8 * cfg.K,
+                total=28 * cfg.K + es * cfg.H * (1 + cfg.K) + cfg.H * (es * cfg.K + 4))
+
+
+def workload_name(cfg) -> str:
+    dt = "bf16" if cfg.act_dtype == synth.ACT_BF16 else "fp32"
+    return (f"config {cfg.cfg_id} ({cfg.name}): L={cfg.L} E={cfg.E} top-{cfg.K} H={cfg.H} {dt}, "
+            f"{len(cfg.sample_len)} samples / {cfg.T} tokens in {cfg.n_mb} micro-steps, "
+            f"P={cfg.P} ranks x ({cfg.Nb}+{cfg.Nr}) slots")
+
+
+def measured_peak() -> tuple:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# --------------------------------------------------------------------------------------------
+# clocks: sampled DURING the timed region through NVML (what nvidia-smi reads)
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    def __init__(self, index: int, period_s: float = 0.1):
+        self.index, self.period, self.samples, self.reasons = index, period_s, [], set()
+        self.max_mhz, self._stop, self._thr, self.err = None, threading.Event(), None, None
+
+    def _run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                     nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                     nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                     nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap",
+                     nv.nvmlClocksEventReasonHwPowerBrakeSlowdown: "hw_power_brake_slowdown",
+                     nv.nvmlClocksEventReasonApplicationsClocksSetting: "applications_clocks_setting"}
+            while not self._stop.is_set():
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self._stop.wait(self.period)
+        except Exception as e:          # NVML missing: report it, do not fail the bench
+            self.err = repr(e)
+
+    def __enter__(self):
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._thr.join(5)
+
+    def summary(self) -> dict:
+        d = {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+             "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+             "samples": len(self.samples)}
+        if self.err:
+            d["error"] = self.err
+        return d
+
+
+def physical_gpu_index(local_index: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_index])
+        except Exception:
+            return local_index
+    return local_index
+
+
+# --------------------------------------------------------------------------------------------
+# CPU oracle on a bounded sample of the workload (cpu_baseline leg and --impl reference arm)
+# --------------------------------------------------------------------------------------------
+class OracleSample:
+    """`n_mb` micro-steps x `n_layers` layers of the config's recipe, generated on the CPU, run
+    through oracle/ (O1..O6) as it stands: single-threaded plain C."""
+
+    def __init__(self, cfg, n_layers: int, n_mb: int):
+        from oracle import foremoe_oracle as orc      # test infrastructure: allowed in this leg only
+        self.orc = orc
+        n_samples = min(len(cfg.sample_len), n_mb * cfg.mb_samples)
+        self.cfg = c = cfg.scaled(L=min(n_layers, cfg.L), n_samples=n_samples)
+        c.name = cfg.name
+        ids, w, mb_off = synth.gen_trace(c, "cpu")
+        self.ids, self.w, self.mb_off = ids.numpy(), w.numpy(), mb_off.numpy()
+        _, step, _ = orc.load_hist(self.ids, self.mb_off, c.E)
+        self.se = synth.gen_placement(c, step)
+        self.x = [synth.gen_activations(c, int(self.mb_off[i + 1] - self.mb_off[i]), i, "cpu")
+                  for i in range(c.n_mb)]
+        self.x = [t.view(torch.int16).numpy().view(np.uint16) if t.dtype == torch.bfloat16
+                  else t.numpy() for t in self.x]
+        self.routed_tokens = c.T * c.L
+        self.desc = (f"{c.L} layer(s) x {c.n_mb} micro-step(s) = {c.L * c.n_mb} instances, "
+                     f"{self.routed_tokens} routed tokens of the same recipe, generated on the CPU")
+
+    def step(self) -> float:
+        """One pass of the whole path over the sample; returns seconds."""
+        orc, c = self.orc, self.cfg
+        t0 = time.perf_counter()
+        hist, _, f = orc.load_hist(self.ids, self.mb_off, c.E)
+        plan = orc.plan(self.ids, self.mb_off, hist, self.se, c.P, c.Ns)
+        assert f == 0 and plan["fault"] == 0
+        for l in range(c.L):
+            for i in range(c.n_mb):
+                a, b = int(self.mb_off[i]), int(self.mb_off[i + 1])
+                buf = orc.gather(plan["perm"][l, a * c.K:b * c.K], self.x[i], c.K, pair_base=a * c.K)
+                orc.combine(plan["inv"][l, a:b], self.w[l, a:b], buf, c.act_dtype, row_base=a * c.K)
+        return time.perf_counter() - t0
+
+
+def run_reference(args, cfg) -> None:
+    """--impl reference: the oracle on host cores, same metric / unit / config."""
+    rank, _, world = multi.env_rank()
+    if rank != 0:
+        return
+    n_mb = max(1, min(4, int(60 / max(1, args.steps + args.warmup))))
+    samp = OracleSample(cfg, 1, n_mb)
+    for _ in range(args.warmup):
+        samp.step()
+    secs = [samp.step() for _ in range(args.steps)]
+    total = float(sum(secs))
+    val = samp.routed_tokens * args.steps / total
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if cfg.act_dtype == synth.ACT_BF16 else "f32",
+        "data": "synthetic", "config": {"workload": workload_name(cfg)},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": "each step = " + samp.desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------
+# our arm: everything resident in HBM, C-ABI calls through the binding
+# --------------------------------------------------------------------------------------------
+class Workload:
+    """Device-resident inputs and outputs of one rank's step (inputs are seeded and synthetic:
+    recipe in DESIGN.md sec. 4).  Nothing here is timed."""
+
+    def __init__(self, cfg, dev):
+        from paper_2606_11867_b200 import binding as fm
+        from paper_2606_11867_b200 import runner
+        self.fm, self.cfg, self.dev = fm, cfg, dev
+        self.shape = s = fm.shape_of(cfg)
+        ids, w, mb_off = synth.gen_trace(cfg, str(dev))
+        self.mb_off_h = cfg.mb_off()
+        # step-level placement from the step totals (harness-side stand-in for Stages 1-3)
+        se0 = torch.full((s.L, s.S), -1, dtype=torch.int32, device=dev)
+        self.plan = runner.StepPlan(s, ids, w, mb_off, se0)
+        self.plan.load_hist()
+        step_hist = self.plan.step_hist.cpu().numpy()
+        self.se_h = synth.gen_placement(cfg, step_hist)
+        self.plan.slot_expert.copy_(torch.from_numpy(self.se_h))
+        tok = [int(self.mb_off_h[i + 1] - self.mb_off_h[i]) for i in range(s.n_mb)]
+        self.tok = tok
+        self.x = [synth.gen_activations(cfg, max(n, 1), i, str(dev)) for i, n in enumerate(tok)]
+        mx = max(max(tok), 1)
+        self.buf = torch.empty((mx * s.K, s.H), dtype=s.act_torch_dtype, device=dev)
+        self.y = torch.empty((mx, s.H), dtype=torch.float32, device=dev)
+        self.perm = torch.empty((mx * s.K,), dtype=torch.int32, device=dev)
+        self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
+        self.routed_tokens = sum(tok) * s.L
+        self.launches_per_step = 2 + 5 + 2 * len(self.instances)
+
+    def step(self, probes=None, stride: int = 0):
+        """One pass of the whole path.  Layers outer, micro-steps inner: consecutive launches read
+        different x buffers, so no call finds its input left in L2 by the previous one."""
+        p = self.plan
+        if probes is not None:
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+        p.plan()
+        if probes is not None:
+            e1.record()
+            probes["plan"].append((e0, e1, self.cfg.T * self.cfg.L))
+        for n, (l, i) in enumerate(self.instances):
+            if probes is not None and stride and n % stride == 0:
+                a = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                a[0].record()
+                p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
+                a[1].record()
+                p.combine(l, i, i + 1, self.buf, self.y)
+                a[2].record()
+                probes["dispatch"].append((a[0], a[1], self.tok[i]))
+                probes["combine"].append((a[1], a[2], self.tok[i]))
+            else:
+                p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
+                p.combine(l, i, i + 1, self.buf, self.y)
+
+    def release(self):
+        self.plan = self.x = self.buf = self.y = self.perm = None
+        torch.cuda.empty_cache()
+
+
+def probe_stats(probes, bpt) -> dict:
+    out = {}
+    for name, lst in probes.items():
+        if not lst:
+            continue
+        ms = np.array([a.elapsed_time(b) for a, b, _ in lst])
+        toks = np.array([n for _, _, n in lst], dtype=np.float64)
+        gbs = float((toks * bpt[name]).sum() / (ms.sum() * 1e-3) / 1e9)
+        out[name] = {"launches_timed": len(lst), "avg_ms": float(ms.mean()), "gbs": gbs,
+                     "bytes_per_token": bpt[name]}
+    return out
+
+
+def run_e2e(args, cfg, wl: "Workload", dev) -> dict:
+    """The same step through foremoe_step_host: HOST (pinned) buffers in, plan + y out, every
+    host<->device copy inside the timed region."""
+    fm, s = wl.fm, wl.shape
+    pin = lambda t: t.contiguous().cpu().pin_memory()
+    ids_h, w_h = pin(wl.plan.ids), pin(wl.plan.w)
+    mb_h = torch.from_numpy(wl.mb_off_h.copy())
+    se_h = torch.from_numpy(wl.se_h.copy())
+    x_h = torch.empty((s.T, s.H), dtype=s.act_torch_dtype).pin_memory()
+    for i, n in enumerate(wl.tok):
+        if n:
+            x_h[int(wl.mb_off_h[i]):int(wl.mb_off_h[i + 1])].copy_(wl.x[i][:n])
+    routed = wl.routed_tokens
+    n_inst = len(wl.instances)
+    wl.release()
+    q_h = torch.empty((s.n_mb, s.L, s.S), dtype=torch.int32).pin_memory()
+    rl_h = torch.empty((s.n_mb, s.L, s.P), dtype=torch.int32).pin_memory()
+    so_h = torch.empty((s.n_mb, s.L, s.S + 1), dtype=torch.int32).pin_memory()
+    y_h = torch.empty((s.T, s.H), dtype=torch.float32).pin_memory()
+    st_h = torch.zeros(1, dtype=torch.int32).pin_memory()
+    arena = torch.empty(fm.step_host_arena_bytes(s, mb_h) + 256, dtype=torch.uint8, device=dev)
+    arena = arena[(-arena.data_ptr()) % 256:]
+    h2d = ids_h.numel() * 4 + w_h.numel() * 4 + mb_h.numel() * 4 + se_h.numel() * 4 \
+        + x_h.numel() * x_h.element_size()
+    d2h = (q_h.numel() + rl_h.numel() + so_h.numel() + 1) * 4 + s.L * y_h.numel() * 4
+    call = lambda: fm.step_host(s, ids_h, w_h, mb_h, se_h, x_h, q_h, rl_h, so_h, y_h, arena, st_h)
+    steps = max(1, min(args.steps, args.e2e_steps))
+    call()                                            # warm-up (also first-touch of the arena)
+    multi.barrier(dev); torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        call()                                        # synchronises before returning
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    assert int(st_h[0]) == 0, f"device fault bits {int(st_h[0])}"
+    ms_max, units = multi.aggregate(ms, routed * steps, dev)
+    return {"value": units / (ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+            "d2h_bytes_per_step": int(d2h), "steps": steps, "ms_per_step": ms_max / steps,
+            "api": "foremoe_step_host (pinned host buffers; x up once per micro-step, y of every "
+                   "instance down)", "gpu_launches": steps * (7 + 2 * n_inst)}
+
+
+def run_ours(args, cfg) -> None:
+    rank, local_rank, world = multi.env_rank()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
+    dev = torch.device("cuda", local_rank)
+    torch.cuda.set_device(dev)
+    multi.init("nccl", dev)
+    cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
+    wl = Workload(cfg, dev)
+    bpt = bytes_per_token(cfg)
+    peak, peak_src = measured_peak()
+
+    for _ in range(args.warmup):
+        wl.step()
+    torch.cuda.synchronize()
+    assert wl.plan.faults() == 0
+    probes = {"plan": [], "dispatch": [], "combine": []}
+    multi.barrier(dev); torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    with ClockSampler(physical_gpu_index(local_rank)) as clk:
+        e0.record()
+        for _ in range(args.steps):
+            wl.step(probes, args.probe_stride)
+        e1.record()
+        torch.cuda.synchronize()
+    multi.barrier(dev)
+    ms = e0.elapsed_time(e1)
+    assert wl.plan.faults() == 0
+    ms_max, units = multi.aggregate(ms, wl.routed_tokens * args.steps, dev)
+    value = units / (ms_max * 1e-3)
+    launches = wl.launches_per_step * args.steps
+    kern = probe_stats(probes, bpt)
+    dom = "combine" if bpt["combine"] >= bpt["dispatch"] else "dispatch"
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")      # written from the committed ncu capture
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get(f"config{cfg.cfg_id}", {}).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": f"foremoe_{dom} (k_{dom}_rows)",
+                "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "bytes_per_launch": bpt[dom] * max(wl.tok), "avg_launch_ms": kern[dom]["avg_ms"],
+                "whole_path_gbs": value / world * bpt["total"] / 1e9,
+                "whole_path_frac": value / world * bpt["total"] / 1e9 / peak,
+                "whole_path_frac_of_nominal_8TBs": value / world * bpt["total"] / 1e9 / NOMINAL_HBM_GBS,
+                "kernels": kern}
+    clocks = clk.summary()
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if cfg.act_dtype == synth.ACT_BF16 else "f32", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
+                   "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
+                         "launches read different x buffers; no flush needed",
+                   "bytes_per_routed_token": bpt["total"]},
+        "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
+    }
+    if not args.no_e2e:
+        line["e2e"] = run_e2e(args, cfg, wl, dev)
+    else:
+        wl.release()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        samp = OracleSample(cfg, 1, args.cpu_sample_mb)
+        secs = samp.step()
+        line["cpu_baseline"] = {"value": samp.routed_tokens / secs, "unit": UNIT, "cores": 1,
+                                "kind": "oracle", "sample": samp.desc, "seconds": secs}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5)")
+    ap.add_argument("--mb-samples", type=int, default=None, help="config 4: samples per micro-step")
+    ap.add_argument("--layers", type=int, default=None, help="debug: fewer layers (INVALID as a bench value)")
+    ap.add_argument("--probe-stride", type=int, default=8,
+                    help="CUDA-event brackets around every n-th instance's dispatch / combine launch")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample-mb", type=int, default=8)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = synth.config(args.config, mb_samples=args.mb_samples)
+    if args.layers:
+        cfg = cfg.scaled(L=args.layers)
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -2,34 +2,9 @@
 // and the weighted top-K combine (a6).  HBM-bound row movers: no tensor cores (nothing here is a
 // dense contraction), 16-byte vectors, whole rows contiguous, persistent grids sized from the SM
 // count.  Contract: include/foremoe.h.
-#include "foremoe_common.cuh"
+#include "foremoe_data.cuh"
 
 namespace foremoe {
-
-// ---- 16-byte global accesses with cache hints ---------------------------------------------------
-// rows of x / expert_out are read once per launch and rows of buf / y are written once: keep them
-// out of L1 and mark them streaming.
-__device__ __forceinline__ int4 ld16_stream(const void *p) {
-  int4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0, %1, %2, %3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-  return r;
-}
-__device__ __forceinline__ void st16_stream(void *p, const int4 &v) {
-  asm volatile("st.global.cs.v4.s32 [%0], {%1, %2, %3, %4};"
-               :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-}
-
-struct RangeInfo { int t_begin, t_end, row0; };
-
-__device__ __forceinline__ RangeInfo load_range(const int32_t *__restrict__ mb_off, int mb_begin,
-                                                int mb_end, int K) {
-  RangeInfo r;
-  r.t_begin = __ldg(mb_off + mb_begin);
-  r.t_end = __ldg(mb_off + mb_end);
-  r.row0 = r.t_begin * K;
-  return r;
-}
 
 // =============================================================================================
 // a4 + a5: dispatch.  Token-major: the row of token t is read ONCE and stored to its K
@@ -80,8 +55,6 @@ k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ m
 // One warp per (token, slice) item; per lane KB * U independent 16-byte loads in flight
 // (k in groups of KB, masked tail), fma into registers, 16-byte stores of the fp32 row.
 // =============================================================================================
-__device__ __forceinline__ float bf16_lo(int v) { return __int_as_float(v << 16); }
-__device__ __forceinline__ float bf16_hi(int v) { return __int_as_float(v & 0xffff0000); }
 
 template <bool kBf16, int KB, int U>
 __global__ void __launch_bounds__(256)
@@ -171,23 +144,14 @@ k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
 }
 
 // ---- launch configuration -------------------------------------------------------------------------
-static int g_dispatch_u = 0;        // 0 = auto
-static int g_combine_u = 0;         // 0 = auto
-static int g_dispatch_cta_per_sm = 0, g_combine_cta_per_sm = 0;
-
-template <typename Kern>
-static int occupancy_ctas(Kern kern, int threads) {
-  int n = 0;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, threads, 0) != cudaSuccess || n <= 0) n = 1;
-  return n;
-}
+DataTuning g_tune;
 
 template <int U>
 static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
                            int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
   static int occ = 0;
   if (!occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
-  const int per_sm = g_dispatch_cta_per_sm > 0 ? g_dispatch_cta_per_sm : occ;
+  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   k_dispatch_rows<U><<<num_sms() * per_sm, 256, 0, st>>>(inv_l, mb_off, mb_begin, mb_end, d.K,
                                                          d.row_vec, n_slices, (const int4 *)x, perm,
@@ -201,7 +165,7 @@ static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
                           cudaStream_t st) {
   static int occ = 0;
   if (!occ) occ = occupancy_ctas(k_combine_rows<kBf16, KB, U>, 256);
-  const int per_sm = g_combine_cta_per_sm > 0 ? g_combine_cta_per_sm : occ;
+  const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   k_combine_rows<kBf16, KB, U><<<num_sms() * per_sm, 256, 0, st>>>(
       inv_l, w_l, mb_off, mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)eo, (float4 *)y);
@@ -240,10 +204,13 @@ static int check_range(const Dims &d, int layer, int mb_begin, int mb_end) {
 
 using namespace foremoe;
 
-extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_data_variant(int dispatch_u, int dispatch_cta_per_sm,
-                                               int combine_u, int combine_cta_per_sm) {
-  g_dispatch_u = dispatch_u; g_dispatch_cta_per_sm = dispatch_cta_per_sm;
-  g_combine_u = combine_u; g_combine_cta_per_sm = combine_cta_per_sm;
+// sweeps only: key = field index of DataTuning in declaration order
+extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_tuning(int key, int value) {
+  int *f[] = {&g_tune.dispatch_impl, &g_tune.dispatch_u, &g_tune.dispatch_cta_per_sm,
+              &g_tune.dispatch_stages, &g_tune.dispatch_warps, &g_tune.combine_impl,
+              &g_tune.combine_u, &g_tune.combine_cta_per_sm, &g_tune.combine_depth,
+              &g_tune.combine_threads};
+  if (key >= 0 && key < (int)(sizeof(f) / sizeof(f[0]))) *f[key] = value;
 }
 
 extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
@@ -260,7 +227,11 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const for
   if (mb_begin == mb_end) return FOREMOE_OK;
   const int32_t *inv_l = inv + (size_t)layer * d.T * d.K;
   cudaStream_t st = (cudaStream_t)stream;
-  int U = g_dispatch_u;
+  if (g_tune.dispatch_impl == 1) {
+    rc = launch_dispatch_tma(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
+    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
+  }
+  int U = g_tune.dispatch_u;
   if (U <= 0) U = d.row_vec >= 256 ? 8 : d.row_vec >= 128 ? 4 : d.row_vec >= 64 ? 2 : 1;
   if (U >= 8) return launch_dispatch<8>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
   if (U >= 4) return launch_dispatch<4>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
@@ -282,9 +253,13 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine(const fore
   if (mb_begin == mb_end) return FOREMOE_OK;
   const size_t lo = (size_t)layer * d.T * d.K;
   cudaStream_t st = (cudaStream_t)stream;
+  if (g_tune.combine_impl == 1) {
+    rc = launch_combine_async(d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
+    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;
+  }
   const int groups = (d.K + 7) / 8;
   const int KB = (d.K + groups - 1) / groups;
-  int U = g_combine_u;
+  int U = g_tune.combine_u;
   if (U <= 0) U = (d.row_vec >= 64 && KB <= 4) ? 2 : 1;
   if (d.act_dtype == FOREMOE_ACT_BF16)
     return launch_combine_kb<true>(KB, U, d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);

@@ -24,6 +24,8 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
                 int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
   constexpr int kF = kBf16 ? 8 : 4;
   const int K = K_T > 0 ? K_T : K_rt;
+  pdl_wait();
+  pdl_launch_dependents();
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   int4 *data = (int4 *)smem;                                           // [(s*K + k)*nt + tid]
@@ -141,9 +143,10 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
   if (!occ || occ_key != smem * 1024 + threads) { occ = occupancy_ctas(kern, threads, smem); occ_key = smem * 1024 + threads; }
   const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 31) / 32;
-  kern<<<num_sms() * per_sm, threads, smem, st>>>(inv_l, w_l, mb_off, mb_begin, mb_end, d.K,
-                                                   d.row_vec, n_slices, (const int4 *)eo, (float4 *)y);
-  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+  const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, threads, smem, st, inv_l, w_l, mb_off,
+                                   mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)eo,
+                                   (float4 *)y);
+  return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
 template <bool kBf16, int K_T>
@@ -176,6 +179,7 @@ int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
                          const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
                          cudaStream_t st) {
   int threads = g_tune.combine_threads > 0 ? g_tune.combine_threads : 256;
+  if (g_tune.combine_threads <= 0 && (size_t)2 * d.K * threads * 16 > 96 * 1024) threads = 128;
   int D = g_tune.combine_depth;
   if (D <= 0) {
     // fill ~96 KB per CTA (two CTAs per SM): D * K * threads * 16 bytes

@@ -17,6 +17,8 @@ __global__ void __launch_bounds__(256)
 k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb_off, int mb_begin,
                 int mb_end, int K, int row_vec, int n_slices, const int4 *__restrict__ x,
                 int32_t *__restrict__ perm, int4 *__restrict__ buf) {
+  pdl_wait();
+  pdl_launch_dependents();
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const int lane = threadIdx.x & 31;
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
@@ -62,6 +64,8 @@ k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
                const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K, int row_vec,
                int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
   constexpr int kF = kBf16 ? 8 : 4;          // floats produced per 16-byte input vector
+  pdl_wait();
+  pdl_launch_dependents();
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const int lane = threadIdx.x & 31;
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
@@ -151,12 +155,14 @@ static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *m
                            int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
   static int occ = 0;
   if (!occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
-  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : occ;
+  // 16 CTAs per SM although only `occ` are resident: the store path runs ~10 % faster with fresh
+  // CTAs streaming in than with a strictly persistent grid (profiles/r01_sweeps.md)
+  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : (occ > 16 ? occ : 16);
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
-  k_dispatch_rows<U><<<num_sms() * per_sm, 256, 0, st>>>(inv_l, mb_off, mb_begin, mb_end, d.K,
-                                                         d.row_vec, n_slices, (const int4 *)x, perm,
-                                                         (int4 *)buf);
-  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+  const cudaError_t e = launch_pdl(k_dispatch_rows<U>, num_sms() * per_sm, 256, 0, st, inv_l, mb_off,
+                                   mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)x, perm,
+                                   (int4 *)buf);
+  return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
 template <bool kBf16, int KB, int U>
@@ -167,9 +173,10 @@ static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
   if (!occ) occ = occupancy_ctas(k_combine_rows<kBf16, KB, U>, 256);
   const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
-  k_combine_rows<kBf16, KB, U><<<num_sms() * per_sm, 256, 0, st>>>(
-      inv_l, w_l, mb_off, mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)eo, (float4 *)y);
-  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+  const cudaError_t e = launch_pdl(k_combine_rows<kBf16, KB, U>, num_sms() * per_sm, 256, 0, st, inv_l,
+                                   w_l, mb_off, mb_begin, mb_end, d.K, d.row_vec, n_slices,
+                                   (const int4 *)eo, (float4 *)y);
+  return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
 template <bool kBf16, int KB>
@@ -209,7 +216,7 @@ extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_tuning(
   int *f[] = {&g_tune.dispatch_impl, &g_tune.dispatch_u, &g_tune.dispatch_cta_per_sm,
               &g_tune.dispatch_stages, &g_tune.dispatch_warps, &g_tune.combine_impl,
               &g_tune.combine_u, &g_tune.combine_cta_per_sm, &g_tune.combine_depth,
-              &g_tune.combine_threads};
+              &g_tune.combine_threads, &g_tune.pdl};
   if (key >= 0 && key < (int)(sizeof(f) / sizeof(f[0]))) *f[key] = value;
 }
 
@@ -227,7 +234,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const for
   if (mb_begin == mb_end) return FOREMOE_OK;
   const int32_t *inv_l = inv + (size_t)layer * d.T * d.K;
   cudaStream_t st = (cudaStream_t)stream;
-  if (g_tune.dispatch_impl == 1) {
+  if (g_tune.dispatch_impl == 1) {   // default (-1, 0): register-staged rows
     rc = launch_dispatch_tma(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
     if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
   }
@@ -253,7 +260,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine(const fore
   if (mb_begin == mb_end) return FOREMOE_OK;
   const size_t lo = (size_t)layer * d.T * d.K;
   cudaStream_t st = (cudaStream_t)stream;
-  if (g_tune.combine_impl == 1) {
+  if (g_tune.combine_impl != 0) {    // default: cp.async shared-memory ring
     rc = launch_combine_async(d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
     if (rc != FOREMOE_ERR_INVALID_ARG) return rc;
   }

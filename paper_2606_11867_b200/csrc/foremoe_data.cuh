@@ -18,6 +18,7 @@ struct DataTuning {
   int combine_cta_per_sm = 0;
   int combine_depth = 0;         // impl 1: stages in flight per thread (0 = auto)
   int combine_threads = 0;       // impl 1: threads per CTA (0 = auto)
+  int pdl = 1;                   // programmatic dependent launch on the data-path kernels
 };
 extern DataTuning g_tune;
 
@@ -50,6 +51,24 @@ __device__ __forceinline__ float bf16_hi(int v) { return __int_as_float(v & 0xff
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) {
   return (uint32_t)__cvta_generic_to_shared(p);
+}
+
+// Programmatic dependent launch: the kernel may be scheduled while the previous kernel of the
+// stream drains (hides launch latency and the ramp); it touches no global memory before pdl_wait().
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kern)(KArgs...), int grid, int block, size_t smem, cudaStream_t st,
+                              Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block);
+  cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = g_tune.pdl ? 1 : 0;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
 template <typename Kern>

@@ -45,6 +45,8 @@ k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb
                int mb_end, int K, int row_bytes, int NS, const char *__restrict__ x,
                int32_t *__restrict__ perm, char *__restrict__ buf) {
   extern __shared__ __align__(128) unsigned char smem[];
+  pdl_wait();
+  pdl_launch_dependents();
   const int n_warps = blockDim.x >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   unsigned char *rows = smem + (size_t)warp * NS * row_bytes;

@@ -341,7 +341,7 @@ def run_ours(args, cfg) -> None:
             traffic = json.load(open(tp)).get(f"config{cfg.cfg_id}", {}).get(dom)
         except Exception:
             traffic = None
-    roofline = {"bound": "hbm", "kernel": f"foremoe_{dom} (k_{dom}_rows)",
+    roofline = {"bound": "hbm", "kernel": f"foremoe_{dom}",
                 "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "bytes_per_launch": bpt[dom] * max(wl.tok), "avg_launch_ms": kern[dom]["avg_ms"],

@@ -178,15 +178,18 @@ static int launch_k(int D, const Dims &d, int threads, const int32_t *inv_l, con
 int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
                          const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
                          cudaStream_t st) {
-  int threads = g_tune.combine_threads > 0 ? g_tune.combine_threads : 256;
-  if (g_tune.combine_threads <= 0 && (size_t)2 * d.K * threads * 16 > 96 * 1024) threads = 128;
+  // one CTA per SM with up to 512 threads and D >= 2 stages filling <= 190 KB of shared memory
+  // (sweep: profiles/r01_sweeps.md): bytes in flight per SM = D * K * threads * 16
+  const size_t budget = 190 * 1024;
+  int threads = g_tune.combine_threads > 0 ? g_tune.combine_threads : 512;
+  if (g_tune.combine_threads <= 0)
+    while (threads > 64 && (size_t)2 * d.K * threads * 16 > budget) threads >>= 1;
   int D = g_tune.combine_depth;
   if (D <= 0) {
-    // fill ~96 KB per CTA (two CTAs per SM): D * K * threads * 16 bytes
     const int cand[] = {8, 6, 4, 3, 2};
     D = 2;
     for (int c : cand)
-      if ((size_t)c * d.K * threads * 16 <= 96 * 1024) { D = c; break; }
+      if ((size_t)c * d.K * threads * 16 <= (threads >= 512 ? 128 * 1024 : budget)) { D = c; break; }
   }
   if (d.act_dtype == FOREMOE_ACT_BF16)
     return launch_k<true>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);

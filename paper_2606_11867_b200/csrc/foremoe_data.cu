@@ -155,9 +155,9 @@ static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *m
                            int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
   static int occ = 0;
   if (!occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
-  // 16 CTAs per SM although only `occ` are resident: the store path runs ~10 % faster with fresh
+  // 32 CTAs per SM although only `occ` are resident: the store path runs ~10 % faster with fresh
   // CTAs streaming in than with a strictly persistent grid (profiles/r01_sweeps.md)
-  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : (occ > 16 ? occ : 16);
+  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : (occ > 32 ? occ : 32);
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   const cudaError_t e = launch_pdl(k_dispatch_rows<U>, num_sms() * per_sm, 256, 0, st, inv_l, mb_off,
                                    mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)x, perm,

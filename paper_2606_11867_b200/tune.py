@@ -1,0 +1,149 @@
+"""Sweep the launch parameters of foremoe_dispatch / foremoe_combine on one config (GPU only).
+
+    python -m paper_2606_11867_b200.tune --config 2 --layers 2 [--quick]
+
+Prints one JSON line per variant: mean CUDA-event time per launch (us), algorithmic GB/s, and
+whether the variant's perm / buf / y are bit-identical to the default kernels' outputs.  Also
+prints torch fill / copy rates at the instance's size as calibration.  The defaults in
+csrc/foremoe_data.cu and csrc/foremoe_combine_async.cu were chosen from this tool's output
+(profiles/r01_sweeps.md).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2606_11867_b200 import binding as fm
+from paper_2606_11867_b200 import synth
+
+KEYS = ["dispatch_impl", "dispatch_u", "dispatch_cta_per_sm", "dispatch_stages", "dispatch_warps",
+        "combine_impl", "combine_u", "combine_cta_per_sm", "combine_depth", "combine_threads", "pdl"]
+DEFAULTS = {"dispatch_impl": -1, "combine_impl": -1, "pdl": 1}
+
+
+def set_tuning(**kw) -> None:
+    """foremoe_debug_set_tuning: sweeps only; unspecified keys return to their defaults."""
+    lib = fm.lib()
+    lib.foremoe_debug_set_tuning.restype = None
+    for i, k in enumerate(KEYS):
+        lib.foremoe_debug_set_tuning(i, int(kw.get(k, DEFAULTS.get(k, 0))))
+
+
+DISPATCH_VARIANTS = [
+    {}, {"dispatch_cta_per_sm": 4}, {"dispatch_cta_per_sm": 8}, {"dispatch_cta_per_sm": 16},
+    {"dispatch_cta_per_sm": 64}, {"dispatch_u": 4}, {"dispatch_u": 2, "dispatch_cta_per_sm": 64},
+    {"dispatch_impl": 1}, {"dispatch_impl": 1, "dispatch_warps": 4, "dispatch_stages": 3, "dispatch_cta_per_sm": 14},
+]
+COMBINE_VARIANTS = [
+    {}, {"combine_impl": 0}, {"combine_impl": 0, "combine_u": 2},
+    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256},
+    {"combine_impl": 1, "combine_depth": 4, "combine_threads": 128},
+    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256},
+    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 2},
+]
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--layers", type=int, default=2)
+    ap.add_argument("--samples", type=int, default=None, help="fewer samples (config 3: 32)")
+    ap.add_argument("--quick", action="store_true")
+    args = ap.parse_args()
+    import bench
+    cfg = synth.config(args.config).scaled(L=args.layers, n_samples=args.samples)
+    dev = torch.device("cuda:0")
+    wl = bench.Workload(cfg, dev)
+    wl.plan.plan()
+    torch.cuda.synchronize()
+    bpt = bench.bytes_per_token(cfg)
+    tok = max(wl.tok)
+
+    def timeit(which: str, reps: int = 2):
+        ev = []
+        for r in range(reps + 1):
+            for (l, i) in wl.instances:
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                if which == "dispatch":
+                    a.record(); wl.plan.dispatch(l, i, i + 1, wl.x[i], wl.perm, wl.buf); b.record()
+                else:
+                    wl.plan.dispatch(l, i, i + 1, wl.x[i], wl.perm, wl.buf)
+                    a.record(); wl.plan.combine(l, i, i + 1, wl.buf, wl.y); b.record()
+                if r > 0:
+                    ev.append((a, b, wl.tok[i]))
+        torch.cuda.synchronize()
+        ms = np.array([a.elapsed_time(b) for a, b, _ in ev])
+        n = np.array([t for _, _, t in ev], dtype=np.float64)
+        return round(float(ms.mean() * 1e3), 1), round(float((n * bpt[which]).sum() / (ms.sum() * 1e-3) / 1e9), 1)
+
+    def loop_time(reps: int = 2):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for r in range(reps + 1):
+            if r == 1:
+                a.record()
+            for (l, i) in wl.instances:
+                wl.plan.dispatch(l, i, i + 1, wl.x[i], wl.perm, wl.buf)
+                wl.plan.combine(l, i, i + 1, wl.buf, wl.y)
+        b.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / reps
+        return round(ms * 1e3 / len(wl.instances), 1), round(sum(wl.tok) * cfg.L * (bpt["dispatch"] + bpt["combine"]) / ms / 1e6, 1)
+
+    set_tuning()
+    l0, i0 = wl.instances[len(wl.instances) // 2]
+    wl.plan.dispatch(l0, i0, i0 + 1, wl.x[i0], wl.perm, wl.buf)
+    wl.plan.combine(l0, i0, i0 + 1, wl.buf, wl.y)
+    ref = (wl.perm.clone(), wl.buf.clone(), wl.y.clone())
+
+    def same(kw) -> bool:
+        set_tuning(**kw)
+        wl.perm.fill_(-9); wl.buf.zero_(); wl.y.zero_()
+        wl.plan.dispatch(l0, i0, i0 + 1, wl.x[i0], wl.perm, wl.buf)
+        wl.plan.combine(l0, i0, i0 + 1, wl.buf, wl.y)
+        torch.cuda.synchronize()
+        return bool(torch.equal(wl.perm, ref[0]) and torch.equal(wl.buf.view(torch.uint8), ref[1].view(torch.uint8))
+                    and torch.equal(wl.y.view(torch.int32), ref[2].view(torch.int32)))
+
+    print(json.dumps({"workload": bench.workload_name(cfg), "tokens_per_instance": tok,
+                      "bytes_per_token": bpt}), flush=True)
+    # calibration: plain torch fill / copy of the instance's buf size
+    nbytes = wl.buf.numel() * wl.buf.element_size()
+    other = torch.empty_like(wl.buf)
+    for name, fn, moved in (("torch fill_", lambda: wl.buf.view(torch.int32).fill_(1), nbytes),
+                            ("torch copy_", lambda: other.copy_(wl.buf), 2 * nbytes)):
+        ts = []
+        for r in range(8):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            if r >= 2:
+                ts.append(a.elapsed_time(b))
+        print(json.dumps({"calibration": name, "bytes": moved, "us": round(float(np.mean(ts)) * 1e3, 1),
+                          "gbs": round(moved / float(np.mean(ts)) / 1e6, 1)}), flush=True)
+    del other
+    dv = DISPATCH_VARIANTS[:3] if args.quick else DISPATCH_VARIANTS
+    cv = COMBINE_VARIANTS[:3] if args.quick else COMBINE_VARIANTS
+    for kw in dv:
+        ok = same(kw); set_tuning(**kw)
+        us, gbs = timeit("dispatch")
+        print(json.dumps({"dispatch": kw or "default", "identical": ok, "us": us, "gbs": gbs}), flush=True)
+    for kw in cv:
+        ok = same(kw); set_tuning(**kw)
+        us, gbs = timeit("combine")
+        print(json.dumps({"combine": kw or "default", "identical": ok, "us": us, "gbs": gbs}), flush=True)
+    for kw in ({}, {"pdl": 0}):
+        set_tuning(**kw)
+        us, gbs = loop_time()
+        print(json.dumps({"loop dispatch+combine": kw or "default", "us_per_instance": us, "gbs": gbs}), flush=True)
+    set_tuning()
+
+
+if __name__ == "__main__":
+    main()

@@ -12,11 +12,46 @@ namespace foremoe {
 //
 // Tiles are fixed token ranges of one layer; a tile may straddle micro-step boundaries, so it is
 // walked segment by segment, each segment counted into a shared-memory histogram and flushed to
-// hist[i][l][:] with one global atomic per non-zero bin.  Warp aggregation: lanes holding the same
-// expert id elect a leader that adds the group's population once (match.any), so a hot expert
-// costs one shared atomic per warp instead of a serialised same-bank burst.
+// hist[i][l][:] with one global atomic per non-zero bin.
+// kMode 0: one shared atomic per pair, 4-byte coalesced loads.
+// kMode 1: warp-aggregated: lanes holding the same expert id elect a leader that adds the group's
+//          population once (match.any) -- one shared atomic per distinct id and warp.
+// kMode 2: one shared atomic per pair, 16-byte loads (4 pairs per lane), 4 loads in flight (default:
+//          fastest on every config incl. the all-one-expert worst case, profiles/r01_hist.md).
 // =============================================================================================
-template <bool kWarpAgg>
+// Count the ids src[0..n) into the shared-memory histogram sh[E]: one shared atomic per pair,
+// 16-byte loads (head / tail handled 4 bytes at a time), 4 loads in flight per thread.
+// Returns FOREMOE_FAULT_ID_RANGE if an id outside [0, E) was seen (it is not counted).
+__device__ __forceinline__ int count_ids(const int32_t *__restrict__ src, int n, int32_t *sh, int E) {
+  int fault = 0;
+  auto count = [&](int e) {
+    if ((unsigned)e < (unsigned)E) atomicAdd(&sh[e], 1); else fault = FOREMOE_FAULT_ID_RANGE;
+  };
+  const int tid = threadIdx.x, nt = blockDim.x;
+  int head = (int)(((16 - ((uintptr_t)src & 15)) & 15) >> 2);
+  if (head > n) head = n;
+  if (tid < head) count(__ldg(src + tid));
+  const int4 *v4 = (const int4 *)(src + head);
+  const int nv = (n - head) >> 2;
+  int v = tid;
+  for (; v + 3 * nt < nv; v += 4 * nt) {
+    const int4 a = __ldg(v4 + v), b = __ldg(v4 + v + nt);
+    const int4 c = __ldg(v4 + v + 2 * nt), d = __ldg(v4 + v + 3 * nt);
+    count(a.x); count(a.y); count(a.z); count(a.w);
+    count(b.x); count(b.y); count(b.z); count(b.w);
+    count(c.x); count(c.y); count(c.z); count(c.w);
+    count(d.x); count(d.y); count(d.z); count(d.w);
+  }
+  for (; v < nv; v += nt) {
+    const int4 a = __ldg(v4 + v);
+    count(a.x); count(a.y); count(a.z); count(a.w);
+  }
+  const int done = head + (nv << 2);
+  if (tid < n - done) count(__ldg(src + done + tid));
+  return fault;
+}
+
+template <int kMode>
 __global__ void __launch_bounds__(256)
 k_load_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off, int L, int T, int K,
             int E, int n_mb, int tile_tokens, int tiles_per_layer, int32_t *__restrict__ hist,
@@ -52,19 +87,23 @@ k_load_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off,
       const int seg_end = min(t1, __ldg(mb_off + i + 1));
       for (int e = tid; e < E; e += blockDim.x) sh[e] = 0;
       __syncthreads();
-      const int p1 = seg_end * K;
-      // uniform trip count so that every lane takes part in match.any
-      for (int p = t0 * K + tid - lane; p < p1; p += blockDim.x) {
-        const int pp = p + lane;
-        int e = pp < p1 ? __ldg(lids + pp) : -1;
-        const bool ok = (unsigned)e < (unsigned)E;
-        if (pp < p1 && !ok) fault = FOREMOE_FAULT_ID_RANGE;
-        if (kWarpAgg) {
-          const unsigned key = ok ? (unsigned)e : (0x80000000u | lane);
-          const unsigned grp = __match_any_sync(0xffffffffu, key);
-          if (ok && lane == __ffs(grp) - 1) atomicAdd(&sh[e], __popc(grp));
-        } else {
-          if (ok) atomicAdd(&sh[e], 1);
+      const int p0 = t0 * K, p1 = seg_end * K;
+      if (kMode == 2) {
+        fault |= count_ids(lids + p0, p1 - p0, sh, E);
+      } else {
+        // uniform trip count so that every lane takes part in match.any
+        for (int p = p0 + tid - lane; p < p1; p += blockDim.x) {
+          const int pp = p + lane;
+          int e = pp < p1 ? __ldg(lids + pp) : -1;
+          const bool ok = (unsigned)e < (unsigned)E;
+          if (pp < p1 && !ok) fault = FOREMOE_FAULT_ID_RANGE;
+          if (kMode == 1) {
+            const unsigned key = ok ? (unsigned)e : (0x80000000u | lane);
+            const unsigned grp = __match_any_sync(0xffffffffu, key);
+            if (ok && lane == __ffs(grp) - 1) atomicAdd(&sh[e], __popc(grp));
+          } else {
+            if (ok) atomicAdd(&sh[e], 1);
+          }
         }
       }
       __syncthreads();
@@ -216,12 +255,7 @@ k_chunk_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off
   if (!locate_chunk(chunk_off, mb_off, n_mb, tpc, c, &ci)) return;
   for (int e = threadIdx.x; e < E; e += blockDim.x) sh[e] = 0;
   __syncthreads();
-  const int32_t *src = ids + ((size_t)l * T + ci.t0) * K;
-  const int np = (ci.t1 - ci.t0) * K;
-  for (int p = threadIdx.x; p < np; p += blockDim.x) {
-    const int e = __ldg(src + p);
-    if ((unsigned)e < (unsigned)E) atomicAdd(&sh[e], 1);
-  }
+  (void)count_ids(ids + ((size_t)l * T + ci.t0) * K, (ci.t1 - ci.t0) * K, sh, E);
   __syncthreads();
   int32_t *dst = chunk_cnt + ((size_t)l * max_chunks + c) * E;
   for (int e = threadIdx.x; e < E; e += blockDim.x) dst[e] = sh[e];
@@ -639,7 +673,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_workspace_bytes(co
   return FOREMOE_OK;
 }
 
-static int g_hist_variant = 1;   // 1 = warp-aggregated (default), 0 = plain shared atomics
+static int g_hist_variant = 2;   // kMode of k_load_hist (sweeps only)
 extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_hist_variant(int v) { g_hist_variant = v; }
 
 extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const foremoe_shape_t *shape, const int32_t *ids,
@@ -659,12 +693,15 @@ extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const fo
     const long long n_tiles = (long long)tiles_per_layer * d.L;
     const int grid = (int)(n_tiles < (long long)num_sms() * 8 ? n_tiles : (long long)num_sms() * 8);
     const size_t smem = sizeof(int32_t) * d.E;
-    if (g_hist_variant)
-      k_load_hist<true><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb,
-                                                 tile_tokens, tiles_per_layer, hist, dev_status);
+    if (g_hist_variant == 1)
+      k_load_hist<1><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
+                                              tiles_per_layer, hist, dev_status);
+    else if (g_hist_variant == 0)
+      k_load_hist<0><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
+                                              tiles_per_layer, hist, dev_status);
     else
-      k_load_hist<false><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb,
-                                                  tile_tokens, tiles_per_layer, hist, dev_status);
+      k_load_hist<2><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
+                                              tiles_per_layer, hist, dev_status);
   }
   if (step_hist) {
     const int LE = d.L * d.E;

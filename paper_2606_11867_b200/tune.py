@@ -52,17 +52,50 @@ COMBINE_VARIANTS = [
 ]
 
 
+def hist_sweep(wl, cfg) -> None:
+    """foremoe_load_hist with each k_load_hist mode on the config's trace and on the worst case
+    for shared atomics (every pair selects expert 0); results are checked against each other."""
+    lib = fm.lib()
+    lib.foremoe_debug_set_hist_variant.restype = None
+    sp = wl.plan
+    names = {0: "plain atomics, 4-byte loads", 1: "warp-aggregated (match.any)",
+             2: "plain atomics, 16-byte loads"}
+    pairs = cfg.L * cfg.T * cfg.K
+    for label, ids in (("config trace", sp.ids), ("all pairs -> expert 0", torch.zeros_like(sp.ids))):
+        ref = None
+        for mode in (0, 1, 2):
+            lib.foremoe_debug_set_hist_variant(mode)
+            ts = []
+            for r in range(6):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                fm.load_hist(sp.shape, ids, sp.mb_off, sp.hist, sp.step_hist, sp.status)
+                b.record(); torch.cuda.synchronize()
+                if r >= 2:
+                    ts.append(a.elapsed_time(b))
+            same = True if ref is None else bool(torch.equal(ref, sp.hist))
+            ref = sp.hist.clone() if ref is None else ref
+            ms = float(np.mean(ts))
+            print(json.dumps({"hist": label, "mode": mode, "what": names[mode], "ms": round(ms, 3),
+                              "ids_gbs": round(pairs * 4 / ms / 1e6, 1), "identical": same}), flush=True)
+    lib.foremoe_debug_set_hist_variant(2)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--layers", type=int, default=2)
     ap.add_argument("--samples", type=int, default=None, help="fewer samples (config 3: 32)")
     ap.add_argument("--quick", action="store_true")
+    ap.add_argument("--hist", action="store_true", help="sweep the k_load_hist modes instead")
     args = ap.parse_args()
     import bench
     cfg = synth.config(args.config).scaled(L=args.layers, n_samples=args.samples)
     dev = torch.device("cuda:0")
     wl = bench.Workload(cfg, dev)
+    if args.hist:
+        hist_sweep(wl, cfg)
+        return
     wl.plan.plan()
     torch.cuda.synchronize()
     bpt = bench.bytes_per_token(cfg)

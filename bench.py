@@ -350,6 +350,17 @@ def run_ours(args, cfg) -> None:
                 "whole_path_frac_of_nominal_8TBs": value / world * bpt["total"] / 1e9 / NOMINAL_HBM_GBS,
                 "kernels": kern}
     clocks = clk.summary()
+    # load balance of the plan (not timed): per instance max rank load / mean rank load, against the
+    # natural placement (expert e on rank e // Nb, no replicas) -- PAPER.md:503-507 reports this ratio
+    rl = wl.plan.rank_load.float()
+    live = rl.sum(-1) > 0
+    ratio = (rl.max(-1).values / rl.mean(-1).clamp(min=1e-9))[live]
+    nat = wl.plan.hist.float().view(cfg.n_mb, cfg.L, cfg.P, cfg.Nb).sum(-1)
+    nratio = (nat.max(-1).values / nat.mean(-1).clamp(min=1e-9))[live]
+    balance = {"lmax_over_lmean": {"max": float(ratio.max()), "mean": float(ratio.mean()),
+                                   "median": float(ratio.median())},
+               "natural_placement": {"max": float(nratio.max()), "mean": float(nratio.mean()),
+                                     "median": float(nratio.median())}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -360,7 +371,7 @@ def run_ours(args, cfg) -> None:
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
                    "bytes_per_routed_token": bpt["total"]},
-        "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
+        "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
     if not args.no_e2e:
         line["e2e"] = run_e2e(args, cfg, wl, dev)

@@ -271,21 +271,21 @@ k_chunk_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off
 // then quota / rank_load / slot_off and the pair-lookup tables are written by all threads.
 // =============================================================================================
 struct QuotaSmem {
-  int32_t *c, *q, *load, *se, *act, *hptr, *hslot, *rslot, *R, *nact, *visited, *par_rank,
+  int32_t *c, *q, *load, *se, *act, *hptr, *hslot, *ahs, *rk, *rslot, *R, *nact, *visited, *par_rank,
       *par_from, *par_to, *queue, *soff;
 };
+// hptr/hslot: all slots of expert e (ascending); ahs[hptr[e] .. hptr[e] + nact[e]): its ACTIVE host
+// slots (ascending); rk[j] = rank of slot j.
 
 // One replicated expert: closed form of the unit-by-unit fill.  With host loads l_j (the expert's
 // own quota removed), lam = largest integer with sum_j max(0, lam - l_j) <= c; every host gets
 // max(0, lam - l_j); the remaining units go one each to the first hosts (ascending slot index)
-// among {l_j <= lam}.  Run by one lane.
-__device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e, int Ns) {
-  const int a0 = s.hptr[e], a1 = s.hptr[e + 1];
+// among {l_j <= lam}.  Serial version (one lane), used when an expert has more than 32 hosts.
+__device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e) {
+  const int a0 = s.hptr[e], a1 = a0 + s.nact[e];
   int cur = INT_MAX;
   for (int a = a0; a < a1; a++) {
-    const int j = s.hslot[a];
-    if (!s.act[j]) continue;
-    const int r = j / Ns;
+    const int j = s.ahs[a], r = s.rk[j];
     const int lj = s.load[r] - s.q[j];
     s.load[r] = lj;
     cur = min(cur, lj);
@@ -295,9 +295,7 @@ __device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e, int 
   for (;;) {
     int m = 0, nxt = INT_MAX;
     for (int a = a0; a < a1; a++) {
-      const int j = s.hslot[a];
-      if (!s.act[j]) continue;
-      const int lj = s.load[j / Ns];
+      const int lj = s.load[s.rk[s.ahs[a]]];
       if (lj <= cur) m++; else nxt = min(nxt, lj);
     }
     if (nxt == INT_MAX || rem < (int64_t)(nxt - cur) * m) {
@@ -310,9 +308,7 @@ __device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e, int 
   }
   int changed = 0;
   for (int a = a0; a < a1; a++) {
-    const int j = s.hslot[a];
-    if (!s.act[j]) continue;
-    const int r = j / Ns;
+    const int j = s.ahs[a], r = s.rk[j];
     const int lj = s.load[r];
     int g = 0;
     if (lj <= lam) {
@@ -323,6 +319,47 @@ __device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e, int 
     s.q[j] = g;
     s.load[r] = lj + g;
   }
+  return changed;
+}
+
+// Warp version of the same closed form (all 32 lanes call it; lane a owns the a-th active host).
+// f_a = sum_b max(0, l_a - l_b) is what it costs to raise every lower host to l_a; the water level
+// sits on top of the highest host load l* with f(l*) <= c:  lam = l* + (c - f(l*)) / m,
+// m = #{l_b <= l*}, and (c - f(l*)) % m units are left for the lowest slots among those m hosts.
+__device__ __forceinline__ int water_fill_expert_warp(const QuotaSmem &s, int e, int lane) {
+  const unsigned full = 0xffffffffu;
+  const int a0 = s.hptr[e], h = s.nact[e];
+  if (h > 32) {
+    int ch = 0;
+    if (lane == 0) ch = water_fill_expert(s, e);
+    __syncwarp();
+    return __shfl_sync(full, ch, 0);
+  }
+  const bool on = lane < h;
+  int j = 0, r = 0, qold = 0, l = INT_MAX;
+  if (on) { j = s.ahs[a0 + lane]; r = s.rk[j]; qold = s.q[j]; l = s.load[r] - qold; }
+  const int c = s.c[e];
+  long long f = 0;
+  for (int b = 0; b < h; b++) {
+    const int lb = __shfl_sync(full, l, b);
+    if (on && l > lb) f += l - lb;
+  }
+  const bool cand = on && f <= (long long)c;
+  const int lstar = __reduce_max_sync(full, cand ? l : INT_MIN);
+  const unsigned who = __ballot_sync(full, cand && l == lstar);
+  const int fstar = __shfl_sync(full, (int)f, __ffs(who) - 1);     // f(l*) <= c fits an int
+  const unsigned le = __ballot_sync(full, on && l <= lstar);
+  const int m = __popc(le);
+  const int rest = c - fstar;
+  const int lam = lstar + rest / m, rem = rest % m;
+  int g = 0;
+  if (on && l <= lstar) {
+    g = lam - l;
+    if (__popc(le & ((1u << lane) - 1u)) < rem) g++;
+  }
+  if (on) { s.q[j] = g; s.load[r] = l + g; }
+  const int changed = __any_sync(full, on && g != qold);
+  __syncwarp();
   return changed;
 }
 
@@ -344,10 +381,9 @@ __device__ __forceinline__ void augment_units(const QuotaSmem &s, int P, int Ns)
         if (j < 0) break;
         const int e = s.se[j];
         if (s.nact[e] < 2 || s.q[j] <= 0) continue;
-        for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
-          const int j2 = s.hslot[a];
-          if (!s.act[j2]) continue;
-          const int r2 = j2 / Ns;
+        const int a0 = s.hptr[e], a1 = a0 + s.nact[e];
+        for (int a = a0; a < a1; a++) {
+          const int j2 = s.ahs[a], r2 = s.rk[j2];
           if (s.visited[r2]) continue;
           s.visited[r2] = 1; s.par_rank[r2] = r; s.par_from[r2] = j; s.par_to[r2] = j2;
           s.queue[tail++] = r2;
@@ -393,6 +429,8 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   s.se = p; p += S;
   s.act = p; p += S;
   s.hslot = p; p += S;
+  s.ahs = p; p += S;
+  s.rk = p; p += S;
   s.rslot = p; p += S;
   s.soff = p; p += S + 1;
   s.load = p; p += P;
@@ -411,6 +449,7 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
     s.act[j] = pl_active[(size_t)pl * S + j];
     s.hslot[j] = pl_host_slot[(size_t)pl * S + j];
     s.rslot[j] = pl_rslot[(size_t)pl * S + j];
+    s.rk[j] = j / Ns;
     s.q[j] = 0;
   }
   for (int r = tid; r < P; r += nt) s.load[r] = 0;
@@ -420,7 +459,10 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   int fault = pl_fault[pl] ? FOREMOE_FAULT_SLOT_EXPERT : 0;
   for (int e = tid; e < E; e += nt) {
     int n = 0;
-    for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) n += s.act[s.hslot[a]];
+    for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
+      const int j = s.hslot[a];
+      if (s.act[j]) s.ahs[s.hptr[e] + n++] = j;
+    }
     s.nact[e] = n;
     if (s.c[e] < 0) fault |= FOREMOE_FAULT_ID_RANGE;
     if (s.c[e] > 0 && n == 0) fault |= FOREMOE_FAULT_NO_HOST;
@@ -458,10 +500,9 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
     // Phase A: forced load of singly hosted experts; collect the replicated set
     for (int e = tid; e < E; e += nt) {
       if (s.nact[e] == 1) {
-        for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
-          const int j = s.hslot[a];
-          if (s.act[j]) { s.q[j] = s.c[e]; atomicAdd(&s.load[j / Ns], s.c[e]); }
-        }
+        const int j = s.ahs[s.hptr[e]];
+        s.q[j] = s.c[e];
+        atomicAdd(&s.load[s.rk[j]], s.c[e]);
       } else if (s.nact[e] >= 2) {
         s.soff[atomicAdd(&nR_raw, 1)] = e;    // soff doubles as the unsorted list (|R| <= S/2)
       }
@@ -479,15 +520,15 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
       s.R[pos] = e;
     }
     __syncthreads();
-    if (tid == 0) {
-      // Phase B: Gauss-Seidel water-filling to a fixpoint
+    if (tid < 32) {
+      // Phase B: Gauss-Seidel water-filling to a fixpoint (warp 0, one lane per host)
       for (int pass = 0; pass < kMaxWaterPasses; pass++) {
         int changed = 0;
-        for (int a = 0; a < nR; a++) changed |= water_fill_expert(s, s.R[a], Ns);
+        for (int a = 0; a < nR; a++) changed |= water_fill_expert_warp(s, s.R[a], tid);
         if (!changed) break;
       }
       // Phase C: exactness cleanup
-      augment_units(s, P, Ns);
+      if (tid == 0) augment_units(s, P, Ns);
     }
   }
   if (tid >= 32) {
@@ -736,7 +777,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
   int32_t *inst_slot_adj = (int32_t *)(ws + w.inst_slot_adj);
   int32_t *inst_ok = (int32_t *)(ws + w.inst_ok), *chunk_cnt = (int32_t *)(ws + w.chunk_cnt);
 
-  const size_t smem_quota = sizeof(int32_t) * ((size_t)4 * d.E + 1 + (size_t)6 * d.S + 1 + (size_t)6 * d.P);
+  const size_t smem_quota = sizeof(int32_t) * ((size_t)4 * d.E + 1 + (size_t)8 * d.S + 1 + (size_t)6 * d.P);
   const size_t smem_pairs = sizeof(int32_t) * ((size_t)d.E + 1 + (size_t)3 * d.S + (size_t)kChunkWarps * d.E);
   const size_t smem_pl = sizeof(int32_t) * ((size_t)2 * d.S + d.E + 1);
   if (smem_quota > 200 * 1024 || smem_pairs > 200 * 1024 || smem_pl > 200 * 1024)

@@ -88,6 +88,7 @@ def main() -> None:
     ap.add_argument("--samples", type=int, default=None, help="fewer samples (config 3: 32)")
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--hist", action="store_true", help="sweep the k_load_hist modes instead")
+    ap.add_argument("--plan", action="store_true", help="time foremoe_load_hist / foremoe_assign only")
     args = ap.parse_args()
     import bench
     cfg = synth.config(args.config).scaled(L=args.layers, n_samples=args.samples)
@@ -95,6 +96,17 @@ def main() -> None:
     wl = bench.Workload(cfg, dev)
     if args.hist:
         hist_sweep(wl, cfg)
+        return
+    if args.plan:
+        for name, fn in (("foremoe_load_hist", wl.plan.load_hist), ("foremoe_assign", wl.plan.assign)):
+            ts = []
+            for r in range(5):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record(); torch.cuda.synchronize()
+                if r >= 2:
+                    ts.append(a.elapsed_time(b))
+            print(json.dumps({"call": name, "ms": round(float(np.mean(ts)), 3),
+                              "instances": cfg.L * cfg.n_mb, "pairs": cfg.L * cfg.T * cfg.K}), flush=True)
         return
     wl.plan.plan()
     torch.cuda.synchronize()

@@ -189,6 +189,35 @@ def test_max_skew_single_expert(cuda_device):
     G.check_data_path(sp, ref, x, [0], [0, 1], "max-skew")
 
 
+def test_expert_with_more_than_32_hosts(cuda_device):
+    """One expert replicated on all 40 ranks (serial water-fill path), a second one on 20 ranks
+    (warp path), the rest singly hosted."""
+    rng = np.random.default_rng(11)
+    E = P = 40
+    Nb, Nr, K, L = 1, 2, 4, 3
+    Ns = Nb + Nr
+    mb_sizes = [700, 64, 3000]
+    T = sum(mb_sizes)
+    mb_off = np.concatenate([[0], np.cumsum(mb_sizes)]).astype(np.int32)
+    p = np.full(E, 0.4 / (E - 2)); p[0] = 0.4; p[1] = 0.2
+    g = rng.gumbel(size=(L, T, E)) + np.log(p)[None, None, :]
+    ids = np.argsort(-g, axis=2)[:, :, :K].astype(np.int32)
+    w = rng.random((L, T, K), dtype=np.float32)
+    se = np.full((L, P * Ns), -1, dtype=np.int32)
+    for l in range(L):
+        for r in range(P):
+            se[l, r * Ns] = r
+            se[l, r * Ns + 1] = 0                      # expert 0 everywhere (rank 0: inactive duplicate)
+            if r % 2 == 0:
+                se[l, r * Ns + 2] = 1
+    ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+    assert ref["fault"] == 0
+    sp = G.gpu_plan(fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=T, n_mb=3, H=8,
+                             act_dtype=fm.ACT_FP32), ids, w, mb_off, se)
+    assert sp.faults() == 0
+    G.assert_plan_equal(sp, ref, "40-hosts")
+
+
 def test_per_microstep_placement(cuda_device):
     """placement_mb_stride = L*S: one placement per (micro-step, layer) (A^{(i)})."""
     rng = np.random.default_rng(3)

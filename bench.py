@@ -240,6 +240,22 @@ class Workload:
                 p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
                 p.combine(l, i, i + 1, self.buf, self.y)
 
+    def capture_graph(self):
+        """Capture the per-instance loop (dispatch + combine of every instance) into ONE CUDA graph:
+        for small micro-steps the loop is launch-bound on the host otherwise."""
+        self.step()                                   # all lazy one-time set-up happens before capture
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for (l, i) in self.instances:
+                self.plan.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
+                self.plan.combine(l, i, i + 1, self.buf, self.y)
+        self.graph = g
+
+    def step_graph(self):
+        self.plan.plan()
+        self.graph.replay()
+
     def release(self):
         self.plan = self.x = self.buf = self.y = self.perm = None
         torch.cuda.empty_cache()
@@ -313,17 +329,26 @@ def run_ours(args, cfg) -> None:
     bpt = bytes_per_token(cfg)
     peak, peak_src = measured_peak()
 
+    if args.graph:
+        wl.capture_graph()
     for _ in range(args.warmup):
         wl.step()
     torch.cuda.synchronize()
     assert wl.plan.faults() == 0
     probes = {"plan": [], "dispatch": [], "combine": []}
+    if args.graph:
+        # per-kernel probes cannot sit inside a graph: take them in one extra, untimed step
+        wl.step(probes, args.probe_stride)
+        torch.cuda.synchronize()
     multi.barrier(dev); torch.cuda.synchronize()
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
     with ClockSampler(physical_gpu_index(local_rank)) as clk:
         e0.record()
         for _ in range(args.steps):
-            wl.step(probes, args.probe_stride)
+            if args.graph:
+                wl.step_graph()
+            else:
+                wl.step(probes, args.probe_stride)
         e1.record()
         torch.cuda.synchronize()
     multi.barrier(dev)
@@ -370,7 +395,8 @@ def run_ours(args, cfg) -> None:
         "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
-                   "bytes_per_routed_token": bpt["total"]},
+                   "bytes_per_routed_token": bpt["total"],
+                   "launch": "cuda graph replay of the instance loop" if args.graph else "stream launches"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
     if not args.no_e2e:
@@ -401,6 +427,9 @@ def main() -> None:
                     help="CUDA-event brackets around every n-th instance's dispatch / combine launch")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-mb", type=int, default=8)
+    ap.add_argument("--graph", action="store_true",
+                    help="replay the per-instance loop as one CUDA graph (per-kernel probes are then "
+                         "taken in an extra untimed step)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

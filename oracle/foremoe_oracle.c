@@ -392,3 +392,158 @@ int oracle_plan(int L, int T, int K, int E, int P, int Ns, int n_mb, const int32
     }
   return fault;
 }
+
+/* ==========================================================================================
+ * NEXT row: placements computed from the foresight.
+ *
+ * O7 oracle_base_placement: Stage 1 at rank level (Alg. 1 lines 13-21, prose
+ *   :290): experts in descending aggregate load, each to the currently least-loaded rank ("LPT").
+ *   The output "fills the N_b base slots on every rank", so a rank is eligible only
+ *   while it has a free base slot (the listing omits this capacity; reading 21).
+ *   One machine (M = 1): the machine-level greedy of Alg. 1 lines 5-12 needs per-source loads and
+ *   the time-model coefficients K1, K2 the paper never gives -- out of scope.
+ *
+ * O8 oracle_microstep_placement: Alg. 3 Stages 2-3 (prose :840-842) for ONE
+ *   (micro-step, layer) instance, machines = M groups of R = P / M consecutive ranks; an expert
+ *   is local to the machine of its base rank.
+ *   Stage 2 (lines 4-10): local experts in descending micro-step load, each to the least-loaded
+ *     local rank with a free base slot; RL[r] += load.
+ *   Stage 3 (lines 12-16): R * N_r rounds per machine: e* = the locally heaviest expert, r* = the
+ *     local rank with the minimum current load; place a replica of e* on r* and update RL.
+ *   Readings: "heaviest" = largest load per copy c[e] / copies[e] (compared
+ *   exactly by cross-multiplication), ties lower id, among experts that still have an eligible
+ *   rank (free redundant slot, not hosting e* yet); an expert whose per-copy load is 0 is never
+ *   replicated (remaining slots stay empty, -1); "update RL" = every host of e* carries the exact
+ *   integer even split floor(c/n) (+1 for the first c mod n hosts in ascending slot index);
+ *   all ties between ranks go to the lowest rank.
+ * Both return fault bits (FAULT_SLOT_EXPERT: base placement unusable; FAULT_ID_RANGE: negative load).
+ * ========================================================================================== */
+static int heavier(const int64_t *c, int a, int b) {   /* a before b: descending load, ties ascending id */
+  if (c[a] != c[b]) return c[a] > c[b];
+  return a < b;
+}
+
+int oracle_base_placement(int E, int P, int Nb, int Nr, const int64_t *tot, int32_t *slot_expert) {
+  const int Ns = Nb + Nr, S = P * Ns;
+  int fault = 0;
+  for (int j = 0; j < S; j++) slot_expert[j] = -1;
+  if ((int64_t)P * Nb < E) return FAULT_SLOT_EXPERT;
+  int32_t *order = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int64_t *RL = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  int32_t *nb = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  if (!order || !RL || !nb) { free(order); free(RL); free(nb); return ORACLE_NO_MEM; }
+  for (int e = 0; e < E; e++) {
+    if (tot[e] < 0) fault |= FAULT_ID_RANGE;
+    order[e] = e;
+  }
+  for (int a = 1; a < E; a++) {          /* insertion sort: descending load, ties ascending id */
+    int32_t e = order[a];
+    int b = a;
+    while (b > 0 && heavier(tot, e, order[b - 1])) { order[b] = order[b - 1]; b--; }
+    order[b] = e;
+  }
+  for (int a = 0; a < E && !fault; a++) {
+    const int e = order[a];
+    int best = -1;
+    for (int r = 0; r < P; r++)
+      if (nb[r] < Nb && (best < 0 || RL[r] < RL[best])) best = r;   /* ties: lowest rank */
+    slot_expert[best * Ns + nb[best]] = e;
+    nb[best] += 1;
+    RL[best] += tot[e];
+  }
+  free(order); free(RL); free(nb);
+  return fault;
+}
+
+/* exact integer even split of c over n hosts: host idx (ascending slot order) carries this much */
+static int64_t even_share(int64_t c, int n, int idx) { return c / n + (idx < c % n ? 1 : 0); }
+
+int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_t *c32,
+                               const int32_t *base_se, int32_t *out_se) {
+  const int Ns = Nb + Nr, S = P * Ns;
+  int fault = 0;
+  for (int j = 0; j < S; j++) out_se[j] = -1;
+  if (M <= 0 || P % M != 0) return ORACLE_BAD_ARG;
+  const int R = P / M;
+  int64_t *c = (int64_t *)calloc((size_t)E, sizeof(int64_t));
+  int32_t *mach = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *order = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int64_t *RL = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  int32_t *nb = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int32_t *nr = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int32_t *copies = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *dead = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *hosts = (int32_t *)calloc((size_t)S + 1, sizeof(int32_t));   /* scratch: slots of e*, ascending */
+  if (!c || !mach || !order || !RL || !nb || !nr || !copies || !dead || !hosts) { fault = ORACLE_NO_MEM; goto done; }
+
+  for (int e = 0; e < E; e++) { c[e] = c32[e]; if (c32[e] < 0) fault |= FAULT_ID_RANGE; mach[e] = -1; }
+  for (int j = S - 1; j >= 0; j--) {       /* machine of e = machine of its lowest-indexed base slot */
+    const int32_t e = base_se[j];
+    if (e < -1 || e >= E) { fault |= FAULT_SLOT_EXPERT; continue; }
+    if (e >= 0) mach[e] = (j / Ns) / R;
+  }
+  for (int m = 0; m < M; m++) {
+    int n_local = 0;
+    for (int e = 0; e < E; e++) n_local += (mach[e] == m);
+    if (n_local > R * Nb) fault |= FAULT_SLOT_EXPERT;
+  }
+  for (int e = 0; e < E; e++) if (mach[e] < 0) fault |= FAULT_SLOT_EXPERT;
+  if (fault) goto done;
+
+  for (int e = 0; e < E; e++) order[e] = e;
+  for (int a = 1; a < E; a++) {
+    int32_t e = order[a];
+    int b = a;
+    while (b > 0 && heavier(c, e, order[b - 1])) { order[b] = order[b - 1]; b--; }
+    order[b] = e;
+  }
+  /* Stage 2: LPT relocation inside each machine (Alg. 3 lines 4-10) */
+  for (int a = 0; a < E; a++) {
+    const int e = order[a], m = mach[e];
+    int best = -1;
+    for (int r = m * R; r < (m + 1) * R; r++)
+      if (nb[r] < Nb && (best < 0 || RL[r] < RL[best])) best = r;
+    out_se[best * Ns + nb[best]] = e;
+    nb[best] += 1;
+    RL[best] += c[e];
+    copies[e] = 1;
+  }
+  /* Stage 3: replication, R * N_r rounds per machine (Alg. 3 lines 12-16) */
+  for (int m = 0; m < M; m++) {
+    for (int k = 0; k < R * Nr; k++) {
+      int estar = -1, rstar = -1;
+      for (;;) {
+        estar = -1;                       /* locally heaviest per copy, ties lower id, not ruled out */
+        for (int e = 0; e < E; e++) {
+          if (mach[e] != m || dead[e] || c[e] <= 0) continue;
+          if (estar < 0 || c[e] * copies[estar] > c[estar] * copies[e]) estar = e;
+        }
+        if (estar < 0) break;
+        rstar = -1;                       /* least-loaded eligible local rank, ties lowest rank */
+        for (int r = m * R; r < (m + 1) * R; r++) {
+          if (nr[r] >= Nr) continue;
+          int hosted = 0;
+          for (int j = r * Ns; j < (r + 1) * Ns; j++) hosted |= (out_se[j] == estar);
+          if (hosted) continue;
+          if (rstar < 0 || RL[r] < RL[rstar]) rstar = r;
+        }
+        if (rstar >= 0) break;
+        dead[estar] = 1;                  /* no eligible rank now => none later either */
+      }
+      if (estar < 0) break;
+      /* update RL: even split over n hosts -> even split over n + 1 hosts */
+      int n = 0;
+      for (int j = 0; j < S; j++) if (out_se[j] == estar) hosts[n++] = j;
+      for (int a = 0; a < n; a++) RL[hosts[a] / Ns] -= even_share(c[estar], n, a);
+      out_se[rstar * Ns + Nb + nr[rstar]] = estar;
+      nr[rstar] += 1;
+      copies[estar] += 1;
+      n = 0;
+      for (int j = 0; j < S; j++) if (out_se[j] == estar) hosts[n++] = j;
+      for (int a = 0; a < n; a++) RL[hosts[a] / Ns] += even_share(c[estar], n, a);
+    }
+  }
+done:
+  free(c); free(mach); free(order); free(RL); free(nb); free(nr); free(copies); free(dead); free(hosts);
+  return fault;
+}

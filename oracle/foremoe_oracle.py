@@ -133,3 +133,19 @@ def combine(inv: np.ndarray, w: np.ndarray, eo: np.ndarray, act_dtype: int,
                                      C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib().oracle_combine(n_tok, K, H, act_dtype, row_base, _p(inv), _p(w), _p(eo), _p(y))
     return y
+
+
+def base_placement(tot: np.ndarray, P: int, Nb: int, Nr: int):
+    """O7 for one layer: step totals int64 [E] -> slot_expert int32 [S], fault."""
+    tot = np.ascontiguousarray(tot, dtype=np.int64)
+    se = np.full(P * (Nb + Nr), -1, dtype=np.int32)
+    fault = lib().oracle_base_placement(tot.shape[0], P, Nb, Nr, _p(tot), _p(se))
+    return se, fault
+
+
+def microstep_placement(c: np.ndarray, base_se: np.ndarray, P: int, Nb: int, Nr: int, M: int = 1):
+    """O8 for one instance: micro-step loads int32 [E], base placement [S] -> slot_expert [S], fault."""
+    c, base_se = _i32(c), _i32(base_se)
+    se = np.full(P * (Nb + Nr), -1, dtype=np.int32)
+    fault = lib().oracle_microstep_placement(c.shape[0], P, Nb, Nr, M, _p(c), _p(base_se), _p(se))
+    return se, fault

@@ -1,0 +1,156 @@
+"""Pins for the placement oracles O7 (Stage 1 rank-level LPT, Alg. 1) and O8
+(Alg. 3 Stages 2-3): a hand-worked vector, closed forms, the greedy invariants
+checked from the OUTPUT alone, Eq.(6)/(7) structure, and the effect on Stage 4's max rank load."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import foremoe_oracle as orc
+from paper_2606_11867_b200 import synth
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _structure_ok(se, E, P, Nb, Nr, c=None, base_only=False):
+    Ns = Nb + Nr
+    se = se.reshape(P, Ns)
+    base = se[:, :Nb]
+    # Eq.(7) coverage + one base slot per expert; base slots filled front to back
+    ids, cnt = np.unique(base[base >= 0], return_counts=True)
+    assert (cnt == 1).all() and len(ids) == E
+    for r in range(P):
+        row = base[r]
+        k = int((row >= 0).sum())
+        assert (row[:k] >= 0).all() and (row[k:] == -1).all()
+        red = se[r, Nb:]
+        k = int((red >= 0).sum())
+        assert (red[:k] >= 0).all() and (red[k:] == -1).all()
+        live = se[r][se[r] >= 0]
+        assert len(set(live.tolist())) == len(live)          # never twice on one rank
+    if base_only:
+        assert (se[:, Nb:] == -1).all()
+    if c is not None:                                        # zero-load experts are never replicated
+        for e in se[:, Nb:].ravel():
+            assert e < 0 or c[e] > 0
+
+
+def test_golden_vector():
+    g = json.load(open(os.path.join(HERE, "golden", "placement_vectors.json")))
+    c = np.array(g["c"])
+    se, f = orc.base_placement(c, g["P"], g["Nb"], g["Nr"])
+    assert f == 0 and se.reshape(g["P"], -1).tolist() == g["base"]
+    for M, key in ((1, "microstep_M1"), (2, "microstep_M2")):
+        out, f = orc.microstep_placement(c, se, g["P"], g["Nb"], g["Nr"], M)
+        assert f == 0 and out.reshape(g["P"], -1).tolist() == g[key]
+
+
+def test_equal_loads_round_robin():
+    E, P, Nb, Nr = 12, 4, 3, 2
+    se, f = orc.base_placement(np.full(E, 5), P, Nb, Nr)
+    assert f == 0
+    exp = np.full((P, Nb + Nr), -1)
+    for r in range(P):
+        for b in range(Nb):
+            exp[r, b] = b * P + r
+    assert (se.reshape(P, -1) == exp).all()
+
+
+def test_one_slot_per_rank_is_sorted_order():
+    rng = np.random.default_rng(0)
+    c = rng.permutation(16) * 3 + 1
+    se, f = orc.base_placement(c, 16, 1, 0)
+    assert f == 0 and (se == np.argsort(-c, kind="stable")).all()
+
+
+def _check_lpt_invariant(c, se, P, Nb, Ns, ranks_of_machine):
+    """Replay in (load desc, id asc) order: at its turn every expert sits on a rank whose load was
+    minimal among the ranks of its machine that still had a free base slot, lowest rank on ties."""
+    order = sorted(range(len(c)), key=lambda e: (-int(c[e]), e))
+    where = {int(se[j]): j // Ns for j in range(len(se)) if se[j] >= 0 and j % Ns < Nb}
+    RL = np.zeros(P, dtype=np.int64)
+    nb = np.zeros(P, dtype=np.int64)
+    for e in order:
+        r = where[e]
+        cand = [q for q in ranks_of_machine(r) if nb[q] < Nb]
+        best = min(cand, key=lambda q: (RL[q], q))
+        assert r == best, (e, r, best)
+        RL[r] += c[e]
+        nb[r] += 1
+    return RL
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_instances_invariants(seed):
+    rng = np.random.default_rng(seed)
+    P = int(rng.choice([2, 4, 6, 8]))
+    Nb, Nr = int(rng.integers(1, 5)), int(rng.integers(0, 4))
+    E, Ns = P * Nb, Nb + Nr
+    tot = rng.integers(0, 1000, size=E) * rng.integers(0, 2, size=E)      # some zero loads
+    base, f = orc.base_placement(tot, P, Nb, Nr)
+    assert f == 0
+    _structure_ok(base, E, P, Nb, Nr, base_only=True)
+    _check_lpt_invariant(tot, base, P, Nb, Ns, lambda r: range(P))
+    c = rng.integers(0, 300, size=E).astype(np.int32) * rng.integers(0, 2, size=E).astype(np.int32)
+    for M in [m for m in (1, 2) if P % m == 0]:
+        R = P // M
+        out, f = orc.microstep_placement(c, base, P, Nb, Nr, M)
+        assert f == 0
+        _structure_ok(out, E, P, Nb, Nr, c=c)
+        RL = _check_lpt_invariant(c, out, P, Nb, Ns, lambda r: range((r // R) * R, (r // R + 1) * R))
+        # experts stay on the machine of their base rank; replicas too
+        mach = {int(base[j]): (j // Ns) // R for j in range(len(base)) if base[j] >= 0}
+        for j, e in enumerate(out):
+            if e >= 0:
+                assert mach[int(e)] == (j // Ns) // R
+        # first replica of each machine: the heaviest local expert, on the least-loaded other rank
+        if Nr > 0:
+            for m in range(M):
+                local = [e for e in range(E) if mach[e] == m and c[e] > 0]
+                if not local or R < 2:
+                    continue
+                e1 = min(local, key=lambda e: (-int(c[e]), e))
+                home = [j // Ns for j in range(len(out)) if out[j] == e1 and j % Ns < Nb][0]
+                cand = [r for r in range(m * R, (m + 1) * R) if r != home]
+                r1 = min(cand, key=lambda r: (RL[r], r))
+                assert out[r1 * Ns + Nb] == e1
+
+
+def test_replication_then_stage4_improves_balance():
+    """On a config-3-shaped trace (64 ranks x 1 replica slot is too coarse at step level) the
+    per-micro-step Stages 2-3 + Stage 4 bring max/mean rank load down on every instance."""
+    cfg = synth.config(3).scaled(L=1, n_samples=8, sample_len=1024, H=64)
+    ids, w, mb_off = synth.gen_trace(cfg, "cpu")
+    ids, mb_off = ids.numpy(), mb_off.numpy()
+    hist, step, f = orc.load_hist(ids, mb_off, cfg.E)
+    base, f = orc.base_placement(step[0], cfg.P, cfg.Nb, cfg.Nr)
+    assert f == 0
+    step_level = synth.gen_placement(cfg, step)[0]
+    better = 0
+    for i in range(cfg.n_mb):
+        _, rl0, _, _, f0 = orc.quota(hist[i, 0], step_level, cfg.P, cfg.Ns)
+        se, f1 = orc.microstep_placement(hist[i, 0], base, cfg.P, cfg.Nb, cfg.Nr, 1)
+        _, rl1, _, _, f2 = orc.quota(hist[i, 0], se, cfg.P, cfg.Ns)
+        assert f0 == 0 and f1 == 0 and f2 == 0
+        assert rl1.sum() == rl0.sum()
+        better += rl1.max() <= rl0.max()
+    assert better == cfg.n_mb
+
+
+def test_faults():
+    c = np.array([3, 2, 1, 1], dtype=np.int32)
+    base, f = orc.base_placement(np.array([3, 2, 1, 1]), 2, 2, 1)
+    assert f == 0
+    bad = base.copy()
+    bad[bad == 2] = -1                                   # expert 2 has no base slot
+    _, f = orc.microstep_placement(c, bad, 2, 2, 1, 1)
+    assert f & orc.FAULT_SLOT_EXPERT
+    bad = base.copy()
+    bad[0] = 9
+    _, f = orc.microstep_placement(c, bad, 2, 2, 1, 1)
+    assert f & orc.FAULT_SLOT_EXPERT
+    _, f = orc.microstep_placement(np.array([3, -1, 1, 1], dtype=np.int32), base, 2, 2, 1, 1)
+    assert f & orc.FAULT_ID_RANGE
+    _, f = orc.base_placement(np.array([1, 2, 3]), 1, 2, 0)       # more experts than base slots
+    assert f & orc.FAULT_SLOT_EXPERT

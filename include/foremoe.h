@@ -144,6 +144,39 @@ int foremoe_combine(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begi
                     const int32_t *mb_off, const int32_t *inv, const float *w,
                     const void *expert_out, float *y, int32_t *dev_status, void *stream);
 
+/*
+ * (NEXT) Stage 1 base placement at rank level for every layer: experts in
+ * descending step load (ties ascending id), each to the least-loaded rank that still has a free
+ * base slot (ties lowest rank) -- Alg. 1 lines 13-21 with the N_b capacity of
+ * PAPER.md:284; one machine (the machine-level greedy needs coefficients the paper never gives).
+ *   step_hist   [L][E] int64 from foremoe_load_hist.
+ *   slot_expert [L][S] int32 out: base slots filled front to back, redundant slots -1.
+ * Faults: ID_RANGE (negative load or load >= 2^31): that layer's output is all -1.
+ */
+int foremoe_base_placement(const foremoe_shape_t *shape, const int64_t *step_hist,
+                           int32_t *slot_expert, int32_t *dev_status, void *stream);
+
+/*
+ * (NEXT) Per-micro-step placement A^{(i)}: Alg. 3 Stages 2-3
+ * for every (micro-step, layer) instance.  Machines are M groups of
+ * R = P / M consecutive ranks; an expert is local to the machine of its base rank.
+ *   Stage 2: local experts in descending micro-step load, each to the least-loaded local rank with
+ *            a free base slot.
+ *   Stage 3: R * N_r rounds per machine: the locally heaviest expert (largest load per copy, exact;
+ *            ties lower id; zero-load experts never) gets a replica on the least-loaded local rank
+ *            with a free redundant slot that does not host it yet; rank loads carry the exact
+ *            integer even split over an expert's hosts (readings 21-25).
+ *   hist             [n_mb][L][E] from foremoe_load_hist.
+ *   base_slot_expert [L][S] (e.g. from foremoe_base_placement): defines each expert's machine.
+ *   slot_expert_mb   [n_mb][L][S] out: feed it to foremoe_assign with
+ *                    shape.placement_mb_stride = L * S.
+ * Faults: SLOT_EXPERT (base placement has a bad value, misses an expert, or overfills a machine),
+ * ID_RANGE (negative load): that instance's output is all -1.
+ */
+int foremoe_microstep_placement(const foremoe_shape_t *shape, int32_t M, const int32_t *hist,
+                                const int32_t *base_slot_expert, int32_t *slot_expert_mb,
+                                int32_t *dev_status, void *stream);
+
 /* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
  * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */
 int foremoe_step_host_arena_bytes(const foremoe_shape_t *shape, const int32_t *mb_off_h,

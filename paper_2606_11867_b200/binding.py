@@ -35,8 +35,8 @@ ACT_BF16 = 0
 ACT_FP32 = 1
 
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
-           "foremoe_dispatch", "foremoe_combine", "foremoe_step_host_arena_bytes",
-           "foremoe_step_host")
+           "foremoe_dispatch", "foremoe_combine", "foremoe_base_placement",
+           "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
 
 class ForeMoEError(RuntimeError):
@@ -105,6 +105,8 @@ def lib() -> C.CDLL:
         l.foremoe_assign.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
         l.foremoe_dispatch.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_combine.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+        l.foremoe_base_placement.argtypes = [sp, vp, vp, vp, vp]
+        l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
         l.foremoe_step_host.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
         for name in EXPORTS:
@@ -189,6 +191,21 @@ def combine(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, w
         C.byref(shape.c()), layer, mb_begin, mb_end, _dev(mb_off, torch.int32),
         _dev(inv, torch.int32), _dev(w, torch.float32), _dev(expert_out, shape.act_torch_dtype),
         _dev(y, torch.float32), _dev(dev_status, torch.int32), _stream()))
+
+
+def base_placement(shape: Shape, step_hist, slot_expert, dev_status=None) -> None:
+    """(f.4) Stage-1 rank-level LPT: step_hist int64 [L,E] -> slot_expert int32 [L,S]."""
+    _check("foremoe_base_placement", lib().foremoe_base_placement(
+        C.byref(shape.c()), _dev(step_hist, torch.int64), _dev(slot_expert, torch.int32),
+        _dev(dev_status, torch.int32), _stream()))
+
+
+def microstep_placement(shape: Shape, M: int, hist, base_slot_expert, slot_expert_mb,
+                        dev_status=None) -> None:
+    """(f.2) Alg. 3 Stages 2-3: hist [n_mb,L,E] + base [L,S] -> slot_expert_mb [n_mb,L,S]."""
+    _check("foremoe_microstep_placement", lib().foremoe_microstep_placement(
+        C.byref(shape.c()), M, _dev(hist, torch.int32), _dev(base_slot_expert, torch.int32),
+        _dev(slot_expert_mb, torch.int32), _dev(dev_status, torch.int32), _stream()))
 
 
 def step_host_arena_bytes(shape: Shape, mb_off_h) -> int:

@@ -1,0 +1,117 @@
+"""GPU parity of foremoe_base_placement / foremoe_microstep_placement against the oracle (O7 / O8),
+bit-exact, and the end-to-end effect: Stage 4 on the per-micro-step placements."""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import foremoe_oracle as orc
+from paper_2606_11867_b200 import binding as fm
+from paper_2606_11867_b200 import synth
+from tests import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_placements(shape, hist, step, M):
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    base = torch.full((shape.L, shape.S), -7, dtype=torch.int32, device=dev)
+    fm.base_placement(shape, torch.as_tensor(step, dtype=torch.int64).to(dev), base, st)
+    mb = torch.full((shape.n_mb, shape.L, shape.S), -7, dtype=torch.int32, device=dev)
+    fm.microstep_placement(shape, M, torch.as_tensor(hist, dtype=torch.int32).to(dev), base, mb, st)
+    torch.cuda.synchronize()
+    return base.cpu().numpy(), mb.cpu().numpy(), int(st.item())
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_instances(cuda_device, seed):
+    rng = np.random.default_rng(50 + seed)
+    P = [2, 4, 6, 8, 64, 40][seed]
+    Nb, Nr = [3, 2, 4, 16, 4, 1][seed], [1, 2, 0, 2, 1, 3][seed]
+    M = [1, 2, 3, 1, 8, 1][seed]
+    E, L, n_mb = P * Nb, 5, 6
+    shape = fm.Shape(L=L, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=n_mb, H=8, act_dtype=fm.ACT_FP32)
+    hist = (rng.integers(0, 500, size=(n_mb, L, E)) * rng.integers(0, 2, size=(n_mb, L, E))).astype(np.int32)
+    hist[1] = 7                                   # all-equal loads: pure tie-breaking
+    hist[2] = 0                                   # empty micro-step: nothing is replicated
+    step = hist.astype(np.int64).sum(0)
+    base, mb, fault = _gpu_placements(shape, hist, step, M)
+    assert fault == 0
+    for l in range(L):
+        ref, f = orc.base_placement(step[l], P, Nb, Nr)
+        assert f == 0 and (base[l] == ref).all(), ("base", l)
+        for i in range(n_mb):
+            ref2, f = orc.microstep_placement(hist[i, l], ref, P, Nb, Nr, M)
+            assert f == 0 and (mb[i, l] == ref2).all(), ("microstep", i, l)
+
+
+def test_golden_vector_on_gpu(cuda_device):
+    c = np.array([10, 9, 8, 7, 3, 2, 1, 1])
+    shape = fm.Shape(L=1, E=8, K=1, P=4, Nb=2, Nr=1, T=8, n_mb=1, H=8, act_dtype=fm.ACT_FP32)
+    base, mb, fault = _gpu_placements(shape, c.reshape(1, 1, 8).astype(np.int32), c.reshape(1, 8), 1)
+    assert fault == 0
+    assert base.reshape(4, 3).tolist() == [[0, 7, -1], [1, 6, -1], [2, 5, -1], [3, 4, -1]]
+    assert mb.reshape(4, 3).tolist() == [[0, 7, 1], [1, 6, 0], [2, 5, 3], [3, 4, 2]]
+
+
+def test_faults(cuda_device):
+    shape = fm.Shape(L=1, E=4, K=1, P=2, Nb=2, Nr=1, T=8, n_mb=2, H=8, act_dtype=fm.ACT_FP32)
+    hist = np.array([[[3, 2, 1, 1]], [[3, -2, 1, 1]]], dtype=np.int32)
+    dev = G.DEV
+    base = torch.tensor([[0, 3, -1, 1, 2, -1]], dtype=torch.int32, device=dev)
+    out = torch.full((2, 1, 6), -7, dtype=torch.int32, device=dev)
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    fm.microstep_placement(shape, 1, torch.from_numpy(hist).to(dev), base, out, st)
+    assert int(st.item()) == fm.FAULT_ID_RANGE
+    assert (out[1].cpu().numpy() == -1).all() and (out[0].cpu().numpy() >= -1).all()
+    st.zero_()
+    bad = base.clone(); bad[0, 1] = -1                      # expert 3 has no base slot
+    fm.microstep_placement(shape, 1, torch.from_numpy(hist).to(dev), bad, out, st)
+    assert int(st.item()) & fm.FAULT_SLOT_EXPERT
+    with pytest.raises(fm.ForeMoEError):
+        fm.microstep_placement(shape, 3, torch.from_numpy(hist).to(dev), base, out, st)   # P % M != 0
+
+
+@pytest.mark.parametrize("cfg_id,kw", [(3, dict(L=2, n_samples=16, sample_len=1500, H=256)),
+                                       (2, dict(L=2, n_samples=16, sample_len=800, H=256, mb_samples=4))])
+def test_stages_2_to_4_pipeline(cuda_device, cfg_id, kw):
+    """hist -> base placement -> per-micro-step placements -> assign (placement_mb_stride) ->
+    dispatch / combine: every array equals the oracle chain, and max rank load is no worse than with
+    the step-level placement on every instance."""
+    cfg = synth.config(cfg_id).scaled(**kw)
+    ids, w, mb_off = synth.gen_trace(cfg, "cpu")
+    ids, w, mb_off = ids.numpy(), w.numpy(), mb_off.numpy()
+    hist, step, f = orc.load_hist(ids, mb_off, cfg.E)
+    s0 = fm.shape_of(cfg)
+    base, mb, fault = _gpu_placements(s0, hist, step, 1)
+    assert fault == 0
+    shape = dataclasses.replace(s0, placement_mb_stride=s0.L * s0.S)
+    sp = G.gpu_plan(shape, ids, w, mb_off, mb)
+    assert sp.faults() == 0
+    step_level = synth.gen_placement(cfg, step)
+    K = cfg.K
+    for l in range(cfg.L):
+        b_ref, f = orc.base_placement(step[l], cfg.P, cfg.Nb, cfg.Nr)
+        assert (base[l] == b_ref).all()
+        for i in range(cfg.n_mb):
+            a, b = int(mb_off[i]), int(mb_off[i + 1])
+            se, f = orc.microstep_placement(hist[i, l], b_ref, cfg.P, cfg.Nb, cfg.Nr, 1)
+            assert f == 0 and (mb[i, l] == se).all()
+            q, rl, so, _, f = orc.quota(hist[i, l], se, cfg.P, cfg.Ns)
+            ps, inv, perm, f2 = orc.assign_instance(ids[l, a:b], se, q, so, cfg.E, base=a * K)
+            assert f == 0 and f2 == 0
+            assert (sp.quota[i, l].cpu().numpy() == q).all()
+            assert (sp.rank_load[i, l].cpu().numpy() == rl).all()
+            assert (sp.inv[l, a:b].cpu().numpy().ravel() == inv).all()
+            _, rl0, _, _, _ = orc.quota(hist[i, l], step_level[l], cfg.P, cfg.Ns)
+            assert rl.max() <= rl0.max()
+    # data path on the per-micro-step plan
+    ref = dict(perm=np.zeros((cfg.L, cfg.T * K), dtype=np.int32), inv=sp.inv.cpu().numpy())
+    for l in range(cfg.L):
+        for i in range(cfg.n_mb):
+            a, b = int(mb_off[i]) * K, int(mb_off[i + 1]) * K
+            ref["perm"][l, ref["inv"][l].ravel()[a:b]] = np.arange(a, b)
+    x = G.activations(cfg, mb_off, range(cfg.n_mb))
+    G.check_data_path(sp, ref, x, range(cfg.L), range(cfg.n_mb), "stages2-4")

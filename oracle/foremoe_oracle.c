@@ -28,6 +28,9 @@
  *   O3/O4 assign numpy.argsort(kind="stable"); bijection; per-slot counts equal quotas.
  *   O5 gather    numpy fancy indexing.
  *   O6 combine   float64 sum within the fp32 error bound; exact cases (w=1, w=1/K).
+ *   O7/O8 placement (Stage 1 LPT, Alg. 3 Stages 2-3): hand-worked vectors, closed forms, greedy
+ *                invariants replayed in Python, structure.  O9/O10 backward: torch.autograd,
+ *                adjoint identities, bf16 rounding cases (see the blocks further down).
  */
 #include <math.h>
 #include <stdint.h>
@@ -546,4 +549,79 @@ int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_
 done:
   free(c); free(mach); free(order); free(RL); free(nb); free(nr); free(copies); free(dead); free(hosts);
   return fault;
+}
+
+/* ==========================================================================================
+ * NEXT row: backward of the data path, the policy-update stage.
+ * "the backward pass triggers an additional gradient computation and additional MoE dispatch and
+ * MoE combine of gradients" (sec. 7.1, n1 = 3, n2 = 4); "the forward and backward
+ * passes of the same micro-step use the same reconfiguration plan" (PAPER.md:170 Fig. 7, :188),
+ * i.e. the SAME inv / w as the forward.  Forward: buf = gather(x) (O5), eo = expert(buf),
+ * y = combine(eo, w) (O6).  Given dy = dLoss/dy (fp32, like y), the chain rule gives
+ *
+ * O9 oracle_combine_bwd ("MoE dispatch of gradients": token order -> slot order)
+ *     d_eo[inv[t*K+k] - row_base][h] = round_act( w[t][k] * dy[t][h] )      one fp32 multiply, then
+ *                                      round-to-nearest-even to bf16 when act_dtype == 0
+ *     dw[t][k] = sum_h dy[t][h] * float(eo[inv[t*K+k] - row_base][h])       plain definition,
+ *                                      accumulated in fp64, rounded once to fp32
+ *   Readings: gradient rows have the activation dtype, the rounding decision is
+ *   taken on the fp32 product (the kernel's precision); dw is defined exactly (the GPU reduces in
+ *   fp32 in another order and is compared within H * 2^-24 * sum_h |dy * eo|); pairs with
+ *   inv < 0 are skipped (rows untouched, dw = 0).
+ *
+ * O10 oracle_dispatch_bwd ("MoE combine of gradients": slot order -> token order)
+ *     dx[t][h] = sum_{k=0}^{K-1} float(d_buf[inv[t*K+k] - row_base][h])     fp32 adds, k ascending
+ *   from 0.0f (the transpose of the row gather: token t was copied to its K rows) -- the same
+ *   fixed order as O6, which it equals with all weights 1.
+ * Pins (tests/test_oracle_backward.py): torch.autograd on a float64 forward built from
+ * index_select / einsum; the adjoint identities <C(eo), dy> = <eo, C^T(dy)>, <D(x), g> = <x, D^T(g)>;
+ * bf16 rounding against torch's conversion and against hand-picked tie cases; closed forms.
+ * ========================================================================================== */
+static uint16_t float_to_bf16_rne(float f) {
+  uint32_t u;
+  memcpy(&u, &f, sizeof u);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x0040u);   /* NaN stays NaN (quiet) */
+  uint32_t lsb = (u >> 16) & 1u;
+  u += 0x7fffu + lsb;                       /* round to nearest, ties to even */
+  return (uint16_t)(u >> 16);
+}
+
+int oracle_combine_bwd(int64_t n_tok, int K, int H, int act_dtype, int32_t row_base,
+                       const int32_t *inv, const float *w, const float *dy,
+                       const void *eo /* may be NULL with dw */, void *d_eo, float *dw /* may be NULL */) {
+  for (int64_t t = 0; t < n_tok; t++)
+    for (int k = 0; k < K; k++) {
+      if (inv[t * K + k] < 0) { if (dw) dw[t * K + k] = 0.0f; continue; }
+      int64_t row = (int64_t)inv[t * K + k] - row_base;
+      double dot = 0.0;
+      for (int h = 0; h < H; h++) {
+        float g = w[t * K + k] * dy[t * H + h];
+        if (act_dtype == 0) ((uint16_t *)d_eo)[row * H + h] = float_to_bf16_rne(g);
+        else ((float *)d_eo)[row * H + h] = g;
+        if (dw && eo) {
+          float v = act_dtype == 0 ? bf16_to_float(((const uint16_t *)eo)[row * H + h])
+                                   : ((const float *)eo)[row * H + h];
+          dot += (double)dy[t * H + h] * (double)v;
+        }
+      }
+      if (dw) dw[t * K + k] = (float)dot;
+    }
+  return 0;
+}
+
+int oracle_dispatch_bwd(int64_t n_tok, int K, int H, int act_dtype, int32_t row_base,
+                        const int32_t *inv, const void *d_buf, float *dx) {
+  for (int64_t t = 0; t < n_tok; t++)
+    for (int h = 0; h < H; h++) {
+      float acc = 0.0f;
+      for (int k = 0; k < K; k++) {
+        if (inv[t * K + k] < 0) continue;
+        int64_t row = (int64_t)inv[t * K + k] - row_base;
+        float v = act_dtype == 0 ? bf16_to_float(((const uint16_t *)d_buf)[row * H + h])
+                                 : ((const float *)d_buf)[row * H + h];
+        acc = acc + v;
+      }
+      dx[t * H + h] = acc;
+    }
+  return 0;
 }

@@ -149,3 +149,40 @@ def microstep_placement(c: np.ndarray, base_se: np.ndarray, P: int, Nb: int, Nr:
     se = np.full(P * (Nb + Nr), -1, dtype=np.int32)
     fault = lib().oracle_microstep_placement(c.shape[0], P, Nb, Nr, M, _p(c), _p(base_se), _p(se))
     return se, fault
+
+
+def combine_bwd(inv: np.ndarray, w: np.ndarray, dy: np.ndarray, eo: Optional[np.ndarray],
+                act_dtype: int, n_rows: int, row_base: int = 0, want_dw: bool = True,
+                d_eo_init: Optional[np.ndarray] = None):
+    """O9.  inv int32 [n_tok,K] layer-global rows, w fp32 [n_tok,K], dy fp32 [n_tok,H], eo
+    [n_rows,H] (uint16 bf16 bits / float32) or None -> d_eo [n_rows,H] (same dtype as eo; rows no
+    pair maps to keep d_eo_init or 0), dw fp32 [n_tok,K] (None if not wanted)."""
+    inv = _i32(inv)
+    w = np.ascontiguousarray(w, dtype=np.float32)
+    dy = np.ascontiguousarray(dy, dtype=np.float32)
+    n_tok, K = inv.shape
+    H = dy.shape[1]
+    dt = np.uint16 if act_dtype == 0 else np.float32
+    if eo is not None:
+        eo = np.ascontiguousarray(eo)
+        assert eo.dtype == dt and eo.shape == (n_rows, H)
+    d_eo = np.zeros((n_rows, H), dtype=dt) if d_eo_init is None else np.ascontiguousarray(d_eo_init, dtype=dt).copy()
+    dw = np.empty((n_tok, K), dtype=np.float32) if (want_dw and eo is not None) else None
+    f = lib().oracle_combine_bwd
+    f.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int32] + [C.c_void_p] * 6
+    f(n_tok, K, H, act_dtype, row_base, _p(inv), _p(w), _p(dy), _p(eo), _p(d_eo), _p(dw))
+    return d_eo, dw
+
+
+def dispatch_bwd(inv: np.ndarray, d_buf: np.ndarray, act_dtype: int, row_base: int = 0) -> np.ndarray:
+    """O10.  inv int32 [n_tok,K], d_buf [n_rows,H] (uint16 bf16 bits / float32) -> dx fp32 [n_tok,H]."""
+    inv = _i32(inv)
+    d_buf = np.ascontiguousarray(d_buf)
+    assert d_buf.dtype == (np.uint16 if act_dtype == 0 else np.float32)
+    n_tok, K = inv.shape
+    H = d_buf.shape[1]
+    dx = np.empty((n_tok, H), dtype=np.float32)
+    f = lib().oracle_dispatch_bwd
+    f.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int32] + [C.c_void_p] * 3
+    f(n_tok, K, H, act_dtype, row_base, _p(inv), _p(d_buf), _p(dx))
+    return dx

@@ -30,6 +30,7 @@ import torch
 from paper_2606_11867_b200 import multi, synth
 
 METRIC = "routed tokens/s (plan+dispatch+combine)"
+METRIC_UPDATE = "routed tokens/s (plan + forward dispatch/combine + backward combine_bwd/dispatch_bwd)"
 UNIT = "tokens/s"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json's "~8 TB/s" denominator, context only
 FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
@@ -38,9 +39,15 @@ FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallbac
 def bytes_per_token(cfg) -> dict:
     """Algorithmic bytes per routed token (DESIGN.md sec. 6 / SURVEY.md sec. 8(d))."""
     es = 2 if cfg.act_dtype == synth.ACT_BF16 else 4
-    return dict(plan=28 * cfg.K, dispatch=es * cfg.H * (1 + cfg.K) + 8 * cfg.K,
-                combine=cfg.H * (es * cfg.K + 4) + 8 * cfg.K,
-                total=28 * cfg.K + es * cfg.H * (1 + cfg.K) + cfg.H * (es * cfg.K + 4))
+    d = dict(plan=28 * cfg.K, dispatch=es * cfg.H * (1 + cfg.K) + 8 * cfg.K,
+             combine=cfg.H * (es * cfg.K + 4) + 8 * cfg.K,
+             total=28 * cfg.K + es * cfg.H * (1 + cfg.K) + cfg.H * (es * cfg.K + 4))
+    # backward (--stage update, DESIGN.md sec. 10): combine_bwd reads dy + K rows of eo, writes K
+    # gradient rows (+ inv, w, dw); dispatch_bwd reads K gradient rows, writes dx (+ inv)
+    d["combine_bwd"] = cfg.H * (4 + 2 * es * cfg.K) + 12 * cfg.K
+    d["dispatch_bwd"] = cfg.H * (es * cfg.K + 4) + 4 * cfg.K
+    d["total_update"] = d["total"] + d["combine_bwd"] + d["dispatch_bwd"]
+    return d
 
 
 def workload_name(cfg) -> str:
@@ -190,7 +197,7 @@ class Workload:
     """Device-resident inputs and outputs of one rank's step (inputs are seeded and synthetic:
     recipe in DESIGN.md sec. 4).  Nothing here is timed."""
 
-    def __init__(self, cfg, dev):
+    def __init__(self, cfg, dev, stage: str = "recompute"):
         from paper_2606_11867_b200 import binding as fm
         from paper_2606_11867_b200 import runner
         self.fm, self.cfg, self.dev = fm, cfg, dev
@@ -213,7 +220,34 @@ class Workload:
         self.perm = torch.empty((mx * s.K,), dtype=torch.int32, device=dev)
         self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
         self.routed_tokens = sum(tok) * s.L
-        self.launches_per_step = 2 + 5 + 2 * len(self.instances)
+        self.stage = stage
+        self.launches_per_step = 2 + 5 + (4 if stage == "update" else 2) * len(self.instances)
+        if stage == "update":          # forward + backward of every instance
+            self.dy = torch.randn((mx, s.H), dtype=torch.float32, device=dev,
+                                  generator=torch.Generator(device=dev).manual_seed(cfg.seed + 11))
+            self.d_buf = torch.empty_like(self.buf)
+            self.dx = torch.empty_like(self.y)
+            self.dw = torch.empty((s.L, s.T, s.K), dtype=torch.float32, device=dev)
+
+    def instance(self, l: int, i: int, ev=None):
+        """The data path of one instance; ev (optional) collects CUDA events between the calls."""
+        p = self.plan
+
+        def mark():
+            if ev is not None:
+                ev.append(torch.cuda.Event(enable_timing=True))
+                ev[-1].record()
+
+        mark()
+        p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
+        mark()
+        p.combine(l, i, i + 1, self.buf, self.y)
+        mark()
+        if self.stage == "update":
+            p.combine_bwd(l, i, i + 1, self.dy, self.buf, self.d_buf, self.dw)
+            mark()
+            p.dispatch_bwd(l, i, i + 1, self.d_buf, self.dx)
+            mark()
 
     def step(self, probes=None, stride: int = 0):
         """One pass of the whole path.  Layers outer, micro-steps inner: consecutive launches read
@@ -228,17 +262,12 @@ class Workload:
             probes["plan"].append((e0, e1, self.cfg.T * self.cfg.L))
         for n, (l, i) in enumerate(self.instances):
             if probes is not None and stride and n % stride == 0:
-                a = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
-                a[0].record()
-                p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
-                a[1].record()
-                p.combine(l, i, i + 1, self.buf, self.y)
-                a[2].record()
-                probes["dispatch"].append((a[0], a[1], self.tok[i]))
-                probes["combine"].append((a[1], a[2], self.tok[i]))
+                a = []
+                self.instance(l, i, a)
+                for j, name in enumerate(("dispatch", "combine", "combine_bwd", "dispatch_bwd")[:len(a) - 1]):
+                    probes[name].append((a[j], a[j + 1], self.tok[i]))
             else:
-                p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
-                p.combine(l, i, i + 1, self.buf, self.y)
+                self.instance(l, i)
 
     def capture_graph(self):
         """Capture the per-instance loop (dispatch + combine of every instance) into ONE CUDA graph:
@@ -248,8 +277,7 @@ class Workload:
         g = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g):
             for (l, i) in self.instances:
-                self.plan.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
-                self.plan.combine(l, i, i + 1, self.buf, self.y)
+                self.instance(l, i)
         self.graph = g
 
     def step_graph(self):
@@ -258,6 +286,7 @@ class Workload:
 
     def release(self):
         self.plan = self.x = self.buf = self.y = self.perm = None
+        self.dy = self.d_buf = self.dx = self.dw = None
         torch.cuda.empty_cache()
 
 
@@ -325,8 +354,10 @@ def run_ours(args, cfg) -> None:
     torch.cuda.set_device(dev)
     multi.init("nccl", dev)
     cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
-    wl = Workload(cfg, dev)
+    wl = Workload(cfg, dev, args.stage)
     bpt = bytes_per_token(cfg)
+    upd = args.stage == "update"
+    total_bpt = bpt["total_update"] if upd else bpt["total"]
     peak, peak_src = measured_peak()
 
     if args.graph:
@@ -335,7 +366,7 @@ def run_ours(args, cfg) -> None:
         wl.step()
     torch.cuda.synchronize()
     assert wl.plan.faults() == 0
-    probes = {"plan": [], "dispatch": [], "combine": []}
+    probes = {"plan": [], "dispatch": [], "combine": [], "combine_bwd": [], "dispatch_bwd": []}
     if args.graph:
         # per-kernel probes cannot sit inside a graph: take them in one extra, untimed step
         wl.step(probes, args.probe_stride)
@@ -359,6 +390,8 @@ def run_ours(args, cfg) -> None:
     launches = wl.launches_per_step * args.steps
     kern = probe_stats(probes, bpt)
     dom = "combine" if bpt["combine"] >= bpt["dispatch"] else "dispatch"
+    if upd:
+        dom = "combine_bwd"
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")      # written from the committed ncu capture
     if os.path.exists(tp):
@@ -370,9 +403,9 @@ def run_ours(args, cfg) -> None:
                 "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
                 "bytes_per_launch": bpt[dom] * max(wl.tok), "avg_launch_ms": kern[dom]["avg_ms"],
-                "whole_path_gbs": value / world * bpt["total"] / 1e9,
-                "whole_path_frac": value / world * bpt["total"] / 1e9 / peak,
-                "whole_path_frac_of_nominal_8TBs": value / world * bpt["total"] / 1e9 / NOMINAL_HBM_GBS,
+                "whole_path_gbs": value / world * total_bpt / 1e9,
+                "whole_path_frac": value / world * total_bpt / 1e9 / peak,
+                "whole_path_frac_of_nominal_8TBs": value / world * total_bpt / 1e9 / NOMINAL_HBM_GBS,
                 "kernels": kern}
     clocks = clk.summary()
     # load balance of the plan (not timed): per instance max rank load / mean rank load, against the
@@ -388,22 +421,22 @@ def run_ours(args, cfg) -> None:
                                      "median": float(nratio.median())}}
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRIC_UPDATE if upd else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if cfg.act_dtype == synth.ACT_BF16 else "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
-                   "bytes_per_routed_token": bpt["total"],
+                   "stage": args.stage, "bytes_per_routed_token": total_bpt,
                    "launch": "cuda graph replay of the instance loop" if args.graph else "stream launches"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
-    if not args.no_e2e:
+    if not args.no_e2e and not upd:
         line["e2e"] = run_e2e(args, cfg, wl, dev)
     else:
         wl.release()
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not upd:
         samp = OracleSample(cfg, 1, args.cpu_sample_mb)
         secs = samp.step()
         line["cpu_baseline"] = {"value": samp.routed_tokens / secs, "unit": UNIT, "cores": 1,
@@ -430,6 +463,9 @@ def main() -> None:
     ap.add_argument("--graph", action="store_true",
                     help="replay the per-instance loop as one CUDA graph (per-kernel probes are then "
                          "taken in an extra untimed step)")
+    ap.add_argument("--stage", default="recompute", choices=["recompute", "update"],
+                    help="recompute = the headline forward path; update = forward + backward of every "
+                         "instance (policy-update stage, PAPER.md:241; no e2e / oracle legs)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -177,6 +177,39 @@ int foremoe_microstep_placement(const foremoe_shape_t *shape, int32_t M, const i
                                 const int32_t *base_slot_expert, int32_t *slot_expert_mb,
                                 int32_t *dev_status, void *stream);
 
+/*
+ * (NEXT) Backward of the data path -- the policy-update stage: "the backward
+ * pass triggers an additional gradient computation and additional MoE dispatch and MoE combine of
+ * gradients" (sec. 7.1, n1 = 3, n2 = 4), on the SAME plan (inv, w) as the forward of
+ * the micro-step (PAPER.md:170 Fig. 7, :188).  Same range / row conventions as foremoe_combine.
+ *
+ * foremoe_combine_bwd -- backward of (a6), the "MoE dispatch of gradients" (token -> slot order):
+ *   dy            [T_range][H] fp32: gradient of the loss w.r.t. y.
+ *   expert_out    [T_range*K][H] the forward expert outputs (act dtype), or NULL if dw is NULL.
+ *   d_expert_out  [T_range*K][H] out (act dtype):
+ *                 d_expert_out[inv[l][t][k] - row0][h] = round_act(w[l][t][k] * dy[t - t0][h]):
+ *                 one fp32 multiply, then round-to-nearest-even to bf16 when act_dtype is bf16
+ *                 (reading 27; NaN payloads unspecified).  Rows no pair maps to
+ *                 (faulted pairs) are left untouched.
+ *   dw            [L][T][K] fp32 out (the whole array; the call writes layer / range), or NULL:
+ *                 dw[l][t][k] = sum_h dy[t - t0][h] * float(expert_out[inv[l][t][k] - row0][h]),
+ *                 reduced in fp32 (per-lane fma chains, then a fixed shuffle tree: deterministic,
+ *                 within H * 2^-24 * sum_h |dy * eo| of the exact sum); 0 for pairs with inv < 0.
+ *
+ * foremoe_dispatch_bwd -- backward of (a5), the "MoE combine of gradients" (slot -> token order):
+ *   d_buf [T_range*K][H] gradient w.r.t. the dispatched rows (act dtype);
+ *   dx    [T_range][H] fp32 out: dx[t - t0][h] = sum_k float(d_buf[inv[l][t][k] - row0][h]),
+ *         fp32 adds, k ascending from 0 (= foremoe_combine with unit weights, bit for bit).
+ */
+int foremoe_combine_bwd(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin, int32_t mb_end,
+                        const int32_t *mb_off, const int32_t *inv, const float *w, const float *dy,
+                        const void *expert_out, void *d_expert_out, float *dw, int32_t *dev_status,
+                        void *stream);
+
+int foremoe_dispatch_bwd(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin, int32_t mb_end,
+                         const int32_t *mb_off, const int32_t *inv, const void *d_buf, float *dx,
+                         int32_t *dev_status, void *stream);
+
 /* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
  * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */
 int foremoe_step_host_arena_bytes(const foremoe_shape_t *shape, const int32_t *mb_off_h,

@@ -35,7 +35,8 @@ ACT_BF16 = 0
 ACT_FP32 = 1
 
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
-           "foremoe_dispatch", "foremoe_combine", "foremoe_base_placement",
+           "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
+           "foremoe_base_placement",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
 
@@ -105,6 +106,8 @@ def lib() -> C.CDLL:
         l.foremoe_assign.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
         l.foremoe_dispatch.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_combine.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+        l.foremoe_combine_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        l.foremoe_dispatch_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         l.foremoe_base_placement.argtypes = [sp, vp, vp, vp, vp]
         l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
@@ -191,6 +194,25 @@ def combine(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, w
         C.byref(shape.c()), layer, mb_begin, mb_end, _dev(mb_off, torch.int32),
         _dev(inv, torch.int32), _dev(w, torch.float32), _dev(expert_out, shape.act_torch_dtype),
         _dev(y, torch.float32), _dev(dev_status, torch.int32), _stream()))
+
+
+def combine_bwd(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, w, dy, expert_out,
+                d_expert_out, dw=None, dev_status=None) -> None:
+    """(f.3) d_expert_out[T_range*K,H] = w * dy scattered to slot order; dw[L,T,K] = <dy, expert_out>."""
+    _check("foremoe_combine_bwd", lib().foremoe_combine_bwd(
+        C.byref(shape.c()), layer, mb_begin, mb_end, _dev(mb_off, torch.int32),
+        _dev(inv, torch.int32), _dev(w, torch.float32), _dev(dy, torch.float32),
+        _dev(expert_out, shape.act_torch_dtype), _dev(d_expert_out, shape.act_torch_dtype),
+        _dev(dw, torch.float32), _dev(dev_status, torch.int32), _stream()))
+
+
+def dispatch_bwd(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, d_buf, dx,
+                 dev_status=None) -> None:
+    """(f.3) dx[T_range,H] fp32 = sum of the K gradient rows of every token."""
+    _check("foremoe_dispatch_bwd", lib().foremoe_dispatch_bwd(
+        C.byref(shape.c()), layer, mb_begin, mb_end, _dev(mb_off, torch.int32),
+        _dev(inv, torch.int32), _dev(d_buf, shape.act_torch_dtype), _dev(dx, torch.float32),
+        _dev(dev_status, torch.int32), _stream()))
 
 
 def base_placement(shape: Shape, step_hist, slot_expert, dev_status=None) -> None:

@@ -46,7 +46,7 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
       const int tl = (int)(item / n_slices);
       const size_t p = (size_t)(rg.t_begin + tl) * K + lane;
       d_nxt = __ldg(inv_l + p);
-      w_nxt = __ldg(w_l + p);
+      w_nxt = w_l ? __ldg(w_l + p) : 1.f;   // w_l == nullptr: unit weights (dispatch backward)
     }
   };
   auto issue = [&](int n) {                // K cp.async of item n into stage n % D

@@ -80,7 +80,7 @@ k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
     if (lane < K) {
       d = __ldg(inv_l + p0 + lane);
       if (d >= 0) d -= rg.row0;
-      wv = __ldg(w_l + p0 + lane);
+      wv = w_l ? __ldg(w_l + p0 + lane) : 1.f;     // w_l == nullptr: unit weights (dispatch backward)
     }
     const int v0 = sl * (32 * U) + lane;
     float acc[U][kF];
@@ -216,7 +216,7 @@ extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_tuning(
   int *f[] = {&g_tune.dispatch_impl, &g_tune.dispatch_u, &g_tune.dispatch_cta_per_sm,
               &g_tune.dispatch_stages, &g_tune.dispatch_warps, &g_tune.combine_impl,
               &g_tune.combine_u, &g_tune.combine_cta_per_sm, &g_tune.combine_depth,
-              &g_tune.combine_threads, &g_tune.pdl};
+              &g_tune.combine_threads, &g_tune.pdl, &g_tune.bwd_depth, &g_tune.bwd_cta_per_sm};
   if (key >= 0 && key < (int)(sizeof(f) / sizeof(f[0]))) *f[key] = value;
 }
 
@@ -246,22 +246,22 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const for
   return launch_dispatch<1>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
 }
 
-extern "C" __attribute__((visibility("default"))) int foremoe_combine(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
-                               int32_t mb_end, const int32_t *mb_off, const int32_t *inv,
-                               const float *w, const void *expert_out, float *y,
-                               int32_t *dev_status, void *stream) {
-  (void)dev_status;
+// a6 and its unit-weight form: w == nullptr sums the K rows (fma(1, v, acc) = acc + v exactly)
+static int combine_entry(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
+                         int32_t mb_end, const int32_t *mb_off, const int32_t *inv, const float *w,
+                         const void *expert_out, float *y, void *stream) {
   Dims d;
   int rc = make_dims(shape, &d);
   if (rc) return rc;
   if ((rc = check_range(d, layer, mb_begin, mb_end))) return rc;
-  if (!mb_off || !inv || !w || !expert_out || !y || !aligned(expert_out, 16) || !aligned(y, 16))
+  if (!mb_off || !inv || !expert_out || !y || !aligned(expert_out, 16) || !aligned(y, 16))
     return FOREMOE_ERR_INVALID_ARG;
   if (mb_begin == mb_end) return FOREMOE_OK;
   const size_t lo = (size_t)layer * d.T * d.K;
+  const float *w_l = w ? w + lo : nullptr;
   cudaStream_t st = (cudaStream_t)stream;
   if (g_tune.combine_impl != 0) {    // default: cp.async shared-memory ring
-    rc = launch_combine_async(d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
+    rc = launch_combine_async(d, inv + lo, w_l, mb_off, mb_begin, mb_end, expert_out, y, st);
     if (rc != FOREMOE_ERR_INVALID_ARG) return rc;
   }
   const int groups = (d.K + 7) / 8;
@@ -269,6 +269,22 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine(const fore
   int U = g_tune.combine_u;
   if (U <= 0) U = (d.row_vec >= 64 && KB <= 4) ? 2 : 1;
   if (d.act_dtype == FOREMOE_ACT_BF16)
-    return launch_combine_kb<true>(KB, U, d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
-  return launch_combine_kb<false>(KB, U, d, inv + lo, w + lo, mb_off, mb_begin, mb_end, expert_out, y, st);
+    return launch_combine_kb<true>(KB, U, d, inv + lo, w_l, mb_off, mb_begin, mb_end, expert_out, y, st);
+  return launch_combine_kb<false>(KB, U, d, inv + lo, w_l, mb_off, mb_begin, mb_end, expert_out, y, st);
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_combine(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
+                               int32_t mb_end, const int32_t *mb_off, const int32_t *inv,
+                               const float *w, const void *expert_out, float *y,
+                               int32_t *dev_status, void *stream) {
+  (void)dev_status;
+  if (!w) return FOREMOE_ERR_INVALID_ARG;
+  return combine_entry(shape, layer, mb_begin, mb_end, mb_off, inv, w, expert_out, y, stream);
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_dispatch_bwd(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
+                                    int32_t mb_end, const int32_t *mb_off, const int32_t *inv,
+                                    const void *d_buf, float *dx, int32_t *dev_status, void *stream) {
+  (void)dev_status;
+  return combine_entry(shape, layer, mb_begin, mb_end, mb_off, inv, nullptr, d_buf, dx, stream);
 }

@@ -19,6 +19,8 @@ struct DataTuning {
   int combine_depth = 0;         // impl 1: stages in flight per thread (0 = auto)
   int combine_threads = 0;       // impl 1: threads per CTA (0 = auto)
   int pdl = 1;                   // programmatic dependent launch on the data-path kernels
+  int bwd_depth = 0;             // k_combine_bwd: stages in flight per thread (0 = auto)
+  int bwd_cta_per_sm = 0;        // 0 = occupancy
 };
 extern DataTuning g_tune;
 

@@ -56,6 +56,15 @@ class StepPlan:
         fm.combine(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, self.w, expert_out,
                    y, self.status)
 
+    def combine_bwd(self, layer: int, mb_begin: int, mb_end: int, dy, expert_out, d_expert_out,
+                    dw=None) -> None:
+        fm.combine_bwd(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, self.w, dy,
+                       expert_out, d_expert_out, dw, self.status)
+
+    def dispatch_bwd(self, layer: int, mb_begin: int, mb_end: int, d_buf, dx) -> None:
+        fm.dispatch_bwd(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, d_buf, dx,
+                        self.status)
+
     def faults(self) -> int:
         """Device fault bits raised so far (synchronises)."""
         return int(self.status.item())

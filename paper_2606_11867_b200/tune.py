@@ -26,7 +26,8 @@ from paper_2606_11867_b200 import binding as fm
 from paper_2606_11867_b200 import synth
 
 KEYS = ["dispatch_impl", "dispatch_u", "dispatch_cta_per_sm", "dispatch_stages", "dispatch_warps",
-        "combine_impl", "combine_u", "combine_cta_per_sm", "combine_depth", "combine_threads", "pdl"]
+        "combine_impl", "combine_u", "combine_cta_per_sm", "combine_depth", "combine_threads", "pdl",
+        "bwd_depth", "bwd_cta_per_sm"]
 DEFAULTS = {"dispatch_impl": -1, "combine_impl": -1, "pdl": 1}
 
 
@@ -49,7 +50,57 @@ COMBINE_VARIANTS = [
     {"combine_impl": 1, "combine_depth": 4, "combine_threads": 128},
     {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256},
     {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 2},
+    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 4},
+    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 8},
+    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256, "combine_cta_per_sm": 4},
+    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256, "combine_cta_per_sm": 8},
+    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256, "combine_cta_per_sm": 16},
+    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256, "combine_cta_per_sm": 8},
+    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256, "combine_cta_per_sm": 16},
 ]
+
+
+BWD_VARIANTS = [{}] + [{"bwd_depth": d, "bwd_cta_per_sm": c} for d in (2, 3) for c in (4, 8, 16, 32)]
+BWD_NODW_VARIANTS = [{}] + [{"bwd_depth": d, "bwd_cta_per_sm": c} for d in (2, 4) for c in (16, 32)]
+
+
+def bwd_sweep(wl, cfg, bench) -> None:
+    """foremoe_combine_bwd (with and without dw) and foremoe_dispatch_bwd per launch."""
+    bpt = bench.bytes_per_token(cfg)
+    es = 2 if cfg.act_dtype == synth.ACT_BF16 else 4
+    nodw = cfg.H * (4 + es * cfg.K) + 8 * cfg.K
+    wl.plan.plan()
+
+    def run(which, kw):
+        set_tuning(**kw)
+        ev = []
+        for r in range(3):
+            for (l, i) in wl.instances:
+                wl.plan.dispatch(l, i, i + 1, wl.x[i], wl.perm, wl.buf)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                if which == "combine_bwd":
+                    wl.plan.combine_bwd(l, i, i + 1, wl.dy, wl.buf, wl.d_buf, wl.dw)
+                elif which == "combine_bwd_nodw":
+                    wl.plan.combine_bwd(l, i, i + 1, wl.dy, None, wl.d_buf, None)
+                else:
+                    wl.plan.dispatch_bwd(l, i, i + 1, wl.buf, wl.dx)
+                b.record()
+                if r > 0:
+                    ev.append((a, b, wl.tok[i]))
+        torch.cuda.synchronize()
+        ms = np.array([a.elapsed_time(b) for a, b, _ in ev])
+        n = np.array([t for _, _, t in ev], dtype=np.float64)
+        per = nodw if which == "combine_bwd_nodw" else bpt[which]
+        print(json.dumps({which: kw or "default", "us": round(float(ms.mean() * 1e3), 1),
+                          "gbs": round(float((n * per).sum() / (ms.sum() * 1e-3) / 1e9), 1)}), flush=True)
+
+    for kw in BWD_VARIANTS:
+        run("combine_bwd", kw)
+    for kw in BWD_NODW_VARIANTS:
+        run("combine_bwd_nodw", kw)
+    run("dispatch_bwd", {})
+    set_tuning()
 
 
 def hist_sweep(wl, cfg) -> None:
@@ -89,11 +140,15 @@ def main() -> None:
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--hist", action="store_true", help="sweep the k_load_hist modes instead")
     ap.add_argument("--plan", action="store_true", help="time foremoe_load_hist / foremoe_assign only")
+    ap.add_argument("--bwd", action="store_true", help="sweep the backward kernels instead")
     args = ap.parse_args()
     import bench
     cfg = synth.config(args.config).scaled(L=args.layers, n_samples=args.samples)
     dev = torch.device("cuda:0")
-    wl = bench.Workload(cfg, dev)
+    wl = bench.Workload(cfg, dev, "update" if args.bwd else "recompute")
+    if args.bwd:
+        bwd_sweep(wl, cfg, bench)
+        return
     if args.hist:
         hist_sweep(wl, cfg)
         return

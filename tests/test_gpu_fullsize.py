@@ -10,7 +10,9 @@ The oracle cannot run a whole 1536-instance step in test time, so (tests/ rule o
   * every OTHER instance: properties that hold at any size, evaluated on the GPU with library
     routines (bincount, sort, cumsum, index_select): conservation Eq.(8), feasibility Eq.(9),
     offsets = prefix of quotas, rank loads = quota sums, inv is a bijection onto the instance's rows,
-    per-slot pair counts = quotas, stability, and max rank load within the water-filling bound.
+    per-slot pair counts = quotas, stability, and max rank load within the water-filling bound;
+  * backward (O9 / O10): first and last instance against the oracle (gradient rows and dx bit for
+    bit, dw within the derived bound), three random instances against torch library ops.
 """
 import numpy as np
 import pytest
@@ -188,3 +190,62 @@ def test_config4_size_sweep(cuda_device, mb_samples):
     layers = [0, cfg.L - 1]
     for l in layers:
         _oracle_checks(wl, [l], sorted({0, cfg.n_mb - 1, _most_imbalanced_mb(wl, l)}))
+
+
+def _backward_checks(wl, instances, oracle_instances):
+    """Backward of the data path at full size in the bench's launch configuration (Workload with
+    stage="update"): against the oracle (O9 / O10) on `oracle_instances`, against torch library
+    ops on the GPU (fp32 product -> bf16 conversion, fp64 einsum, index_select) on `instances`."""
+    sp, s = wl.plan, wl.shape
+    mb = wl.mb_off_h
+    bits = torch.int16 if s.act_dtype == 0 else torch.int32
+    for (l, i) in instances:
+        a, b = int(mb[i]), int(mb[i + 1])
+        n = b - a
+        if n == 0:
+            continue
+        sp.dispatch(l, i, i + 1, wl.x[i], wl.perm, wl.buf)
+        wl.d_buf.view(torch.uint8).fill_(0xAB)
+        sp.combine_bwd(l, i, i + 1, wl.dy, wl.buf, wl.d_buf, wl.dw)
+        sp.dispatch_bwd(l, i, i + 1, wl.d_buf, wl.dx)
+        torch.cuda.synchronize()
+        inv = (sp.inv[l, a:b].long() - a * s.K)                       # [n, K] local rows
+        w = sp.w[l, a:b]
+        for c0 in range(0, n, 2048):
+            c1 = min(n, c0 + 2048)
+            rows = inv[c0:c1].reshape(-1)
+            prod = (w[c0:c1, :, None] * wl.dy[c0:c1, None, :]).to(s.act_torch_dtype)    # fp32 multiply, RNE
+            assert torch.equal(wl.d_buf[rows].view(bits), prod.view(-1, s.H).view(bits)), ("d_eo", l, i)
+            eo = wl.buf[rows].double().view(c1 - c0, s.K, s.H)
+            dyd = wl.dy[c0:c1].double()
+            exact = torch.einsum("th,tkh->tk", dyd, eo)
+            bound = s.H * 2.0 ** -24 * torch.einsum("th,tkh->tk", dyd.abs(), eo.abs()) + 1e-30
+            assert ((wl.dw[l, a + c0:a + c1].double() - exact).abs() <= bound).all(), ("dw", l, i)
+            g = wl.d_buf[rows].double().view(c1 - c0, s.K, s.H)
+            bnd = s.K * 2.0 ** -24 * g.abs().sum(1) + 1e-30
+            assert ((wl.dx[c0:c1].double() - g.sum(1)).abs() <= bnd).all(), ("dx", l, i)
+        if (l, i) in oracle_instances:
+            inv_h = sp.inv[l, a:b].cpu().numpy()
+            d_ref, dw_ref = orc.combine_bwd(inv_h, w.cpu().numpy(), wl.dy[:n].cpu().numpy(),
+                                            G.to_bits(wl.buf[:n * s.K]), s.act_dtype, n * s.K,
+                                            row_base=a * s.K)
+            assert (G.to_bits(wl.d_buf[:n * s.K]) == d_ref).all(), ("d_eo vs oracle", l, i)
+            dx_ref = orc.dispatch_bwd(inv_h, d_ref, s.act_dtype, row_base=a * s.K)
+            assert (wl.dx[:n].cpu().numpy().view(np.uint32) == dx_ref.view(np.uint32)).all(), ("dx vs oracle", l, i)
+            err = np.abs(wl.dw[l, a:b].cpu().numpy().astype(np.float64) - dw_ref)
+            scale = np.abs(dw_ref).max()
+            assert err.max() <= 1e-4 * scale, ("dw vs oracle", l, i, float(err.max()), float(scale))
+
+
+@pytest.mark.parametrize("cfg_id", [2, 3, 5])
+def test_full_config_backward(cuda_device, cfg_id):
+    cfg = synth.config(cfg_id)
+    wl = bench.Workload(cfg, cuda_device, "update")
+    wl.plan.plan()
+    torch.cuda.synchronize()
+    assert wl.plan.faults() == 0
+    rng = np.random.default_rng(100 + cfg_id)
+    inst = [wl.instances[k] for k in rng.choice(len(wl.instances), size=3, replace=False)]
+    first, last = (0, 0), (cfg.L - 1, cfg.n_mb - 1)
+    _backward_checks(wl, [first, last] + inst, {first, last})
+    assert wl.plan.faults() == 0

@@ -625,3 +625,92 @@ int oracle_dispatch_bwd(int64_t n_tok, int K, int H, int act_dtype, int32_t row_
     }
   return 0;
 }
+
+/* ==========================================================================================
+ * NEXT row: per-source, multi-machine Stage 4.
+ *
+ * Inputs now carry the source of every token: w_{s,e} is a P x E matrix, the
+ * P ranks form M machines of R = P / M consecutive ranks, and C_{i,j} of Eq.(5)
+ * counts the tokens flowing from the ranks of machine i to the slots of machine j.
+ *
+ * O11 oracle_quota_local: token assignment with the placement fixed, by the paper's
+ * "locality-aware token assignment heuristic: tokens prefer same-machine replicas to avoid
+ * cross-machine traffic, and any leftover tokens are routed to minimize per-rank load"
+ * (sec. 8.2), made exact in the same way as O2 (readings 29-31):
+ *   - commodity (e, m) = the tokens of expert e whose source rank sits on machine m; only the
+ *     machine of the source matters for L_r (Eq.(4)) and C_{i,j} (Eq.(5)), so sources are
+ *     aggregated per machine: c[e][m] = sum_{s in ranks(m)} w_{s,e};
+ *   - allowed hosts of (e, m): the slots holding e on machine m if there is one ("prefer
+ *     same-machine replicas"), else every slot holding e ("leftover tokens");
+ *   - among all integer assignments that respect the allowed hosts, minimise L_max: this is O2
+ *     itself on a VIRTUAL instance with experts v = e * M + m, counts c[e][m] and virtual slots
+ *     (j, m) -> index j * M + m, N_s * M per rank, holding v when slot j is an allowed host of
+ *     (e, m) and -1 otherwise.  The reduction is written out below and oracle_quota (O2, pinned)
+ *     is called on it, so every tie-break of O2 carries over: commodities in descending count,
+ *     ties ascending v; units to the least-loaded rank, ties to the lowest virtual slot.
+ * Outputs: q_src[m][j] (tokens of source machine m sent to slot j), rank_load[r],
+ * traffic[i][j] = sum over slots of machine j of q_src[i][.] (diagonal = tokens that stay inside
+ * the machine; off-diagonal = C_{i,j} of Eq.(5)).
+ * Pins (tests/test_oracle_local.py): brute force over all integer splits within the allowed
+ * hosts on tiny instances; ceil(LP*) of Eq.(10) restricted to the allowed hosts (HiGHS); total
+ * cross-machine traffic equals its lower bound (tokens with no same-machine replica); M = 1 is O2;
+ * experts hosted on one machine only => same max load as O2 on the summed counts; hand-worked
+ * vectors in tests/golden/local_vectors.json.
+ * ========================================================================================== */
+int oracle_local_placement(int E, int P, int Ns, int M, const int32_t *slot_expert,
+                           int32_t *slot_expert_v /* [P*Ns*M] */) {
+  const int S = P * Ns;
+  if (M <= 0 || P % M != 0) return ORACLE_BAD_ARG;
+  const int R = P / M;
+  int fault = 0;
+  for (int j = 0; j < S; j++) {
+    const int32_t e = slot_expert[j];
+    if (e < -1 || e >= E) fault |= FAULT_SLOT_EXPERT;
+    for (int m = 0; m < M; m++) {
+      int32_t v = -1;
+      if (e >= 0 && e < E) {
+        const int mj = (j / Ns) / R;               /* machine of slot j */
+        int local_exists = 0;                      /* does machine m hold e at all? */
+        for (int j2 = 0; j2 < S; j2++)
+          if (slot_expert[j2] == e && (j2 / Ns) / R == m) local_exists = 1;
+        if (mj == m || !local_exists) v = e * M + m;
+      }
+      slot_expert_v[(size_t)j * M + m] = v;
+    }
+  }
+  return fault;
+}
+
+int oracle_quota_local(int E, int P, int Ns, int M, const int32_t *w_se /* [P][E] per-source counts */,
+                       const int32_t *slot_expert, int32_t *q_src /* [M][S] */,
+                       int32_t *rank_load /* [P] */, int32_t *traffic /* [M][M] */,
+                       int32_t *quota_v /* [S*M] or NULL */, int32_t *slot_off_v /* [S*M+1] or NULL */) {
+  const int S = P * Ns;
+  if (M <= 0 || P % M != 0) return ORACLE_BAD_ARG;
+  const int R = P / M;
+  int32_t *c_v = (int32_t *)calloc((size_t)E * M, sizeof(int32_t));
+  int32_t *se_v = (int32_t *)calloc((size_t)S * M, sizeof(int32_t));
+  int32_t *q_v = (int32_t *)calloc((size_t)S * M, sizeof(int32_t));
+  int32_t *so_v = (int32_t *)calloc((size_t)S * M + 1, sizeof(int32_t));
+  int fault;
+  if (!c_v || !se_v || !q_v || !so_v) { fault = ORACLE_NO_MEM; goto done; }
+  for (int s = 0; s < P; s++)                      /* aggregate the sources of a machine */
+    for (int e = 0; e < E; e++) c_v[e * M + s / R] += w_se[(size_t)s * E + e];
+  fault = oracle_local_placement(E, P, Ns, M, slot_expert, se_v);
+  if (fault < 0) goto done;
+  fault |= oracle_quota(E * M, P, Ns * M, c_v, se_v, q_v, rank_load, so_v, 3, NULL);
+  if (fault < 0) goto done;
+  for (int m = 0; m < M; m++)
+    for (int j = 0; j < S; j++) q_src[(size_t)m * S + j] = q_v[(size_t)j * M + m];
+  for (int i = 0; i < M; i++)
+    for (int mj = 0; mj < M; mj++) {
+      int64_t t = 0;
+      for (int j = mj * R * Ns; j < (mj + 1) * R * Ns; j++) t += q_src[(size_t)i * S + j];
+      traffic[i * M + mj] = (int32_t)t;
+    }
+  if (quota_v) memcpy(quota_v, q_v, sizeof(int32_t) * (size_t)S * M);
+  if (slot_off_v) memcpy(slot_off_v, so_v, sizeof(int32_t) * ((size_t)S * M + 1));
+done:
+  free(c_v); free(se_v); free(q_v); free(so_v);
+  return fault;
+}

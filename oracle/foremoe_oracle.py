@@ -186,3 +186,26 @@ def dispatch_bwd(inv: np.ndarray, d_buf: np.ndarray, act_dtype: int, row_base: i
     f.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int32] + [C.c_void_p] * 3
     f(n_tok, K, H, act_dtype, row_base, _p(inv), _p(d_buf), _p(dx))
     return dx
+
+
+def local_placement(slot_expert: np.ndarray, E: int, P: int, Ns: int, M: int):
+    """O11 reduction: real placement [S] -> virtual placement [S*M] (virtual expert e*M+m on virtual
+    slot j*M+m when slot j is an allowed host of commodity (e, m)), fault."""
+    se = _i32(slot_expert)
+    out = np.full(P * Ns * M, -1, dtype=np.int32)
+    fault = lib().oracle_local_placement(E, P, Ns, M, _p(se), _p(out))
+    return out, fault
+
+
+def quota_local(w_se: np.ndarray, slot_expert: np.ndarray, P: int, Ns: int, M: int):
+    """O11 for one instance: per-source counts int32 [P,E], placement [S] ->
+    dict(q_src [M,S], rank_load [P], traffic [M,M], quota_v [S*M], slot_off_v [S*M+1], fault)."""
+    w_se, se = _i32(w_se), _i32(slot_expert)
+    E, S = w_se.shape[1], P * Ns
+    out = dict(q_src=np.zeros((M, S), np.int32), rank_load=np.zeros(P, np.int32),
+               traffic=np.zeros((M, M), np.int32), quota_v=np.zeros(S * M, np.int32),
+               slot_off_v=np.zeros(S * M + 1, np.int32))
+    out["fault"] = lib().oracle_quota_local(E, P, Ns, M, _p(w_se), _p(se), _p(out["q_src"]),
+                                            _p(out["rank_load"]), _p(out["traffic"]),
+                                            _p(out["quota_v"]), _p(out["slot_off_v"]))
+    return out

@@ -197,7 +197,7 @@ class Workload:
     """Device-resident inputs and outputs of one rank's step (inputs are seeded and synthetic:
     recipe in DESIGN.md sec. 4).  Nothing here is timed."""
 
-    def __init__(self, cfg, dev, stage: str = "recompute"):
+    def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0):
         from paper_2606_11867_b200 import binding as fm
         from paper_2606_11867_b200 import runner
         self.fm, self.cfg, self.dev = fm, cfg, dev
@@ -211,6 +211,14 @@ class Workload:
         step_hist = self.plan.step_hist.cpu().numpy()
         self.se_h = synth.gen_placement(cfg, step_hist)
         self.plan.slot_expert.copy_(torch.from_numpy(self.se_h))
+        self.machines = machines
+        if machines:        # per-source, multi-machine Stage 4: commodity plan
+            self.tok_src_h = synth.gen_tok_src(cfg)
+            se_dev = self.plan.slot_expert
+            self.plan = None
+            self.plan = runner.LocalStepPlan(s, machines, ids, w, mb_off, se_dev,
+                                             torch.from_numpy(self.tok_src_h).to(dev))
+            self.real_shape, self.shape = s, self.plan.shape      # same K, H, T, n_mb; E, Nb, Nr x M
         tok = [int(self.mb_off_h[i + 1] - self.mb_off_h[i]) for i in range(s.n_mb)]
         self.tok = tok
         self.x = [synth.gen_activations(cfg, max(n, 1), i, str(dev)) for i, n in enumerate(tok)]
@@ -221,7 +229,7 @@ class Workload:
         self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
         self.routed_tokens = sum(tok) * s.L
         self.stage = stage
-        self.launches_per_step = 2 + 5 + (4 if stage == "update" else 2) * len(self.instances)
+        self.launches_per_step = 2 + 5 + (3 if machines else 0) + (4 if stage == "update" else 2) * len(self.instances)
         if stage == "update":          # forward + backward of every instance
             self.dy = torch.randn((mx, s.H), dtype=torch.float32, device=dev,
                                   generator=torch.Generator(device=dev).manual_seed(cfg.seed + 11))
@@ -354,7 +362,7 @@ def run_ours(args, cfg) -> None:
     torch.cuda.set_device(dev)
     multi.init("nccl", dev)
     cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
-    wl = Workload(cfg, dev, args.stage)
+    wl = Workload(cfg, dev, args.stage, args.machines)
     bpt = bytes_per_token(cfg)
     upd = args.stage == "update"
     total_bpt = bpt["total_update"] if upd else bpt["total"]
@@ -413,13 +421,23 @@ def run_ours(args, cfg) -> None:
     rl = wl.plan.rank_load.float()
     live = rl.sum(-1) > 0
     ratio = (rl.max(-1).values / rl.mean(-1).clamp(min=1e-9))[live]
-    nat = wl.plan.hist.float().view(cfg.n_mb, cfg.L, cfg.P, cfg.Nb).sum(-1)
+    hist_real = wl.plan.hist if not args.machines else wl.plan.hist.view(cfg.n_mb, cfg.L, cfg.E, args.machines).sum(-1)
+    nat = hist_real.float().view(cfg.n_mb, cfg.L, cfg.P, cfg.Nb).sum(-1)
     nratio = (nat.max(-1).values / nat.mean(-1).clamp(min=1e-9))[live]
     balance = {"lmax_over_lmean": {"max": float(ratio.max()), "mean": float(ratio.mean()),
                                    "median": float(ratio.median())},
                "natural_placement": {"max": float(nratio.max()), "mean": float(nratio.mean()),
                                      "median": float(nratio.median())}}
 
+    if args.machines:
+        tr = wl.plan.traffic.double()
+        tot = tr.sum((-1, -2)).clamp(min=1)
+        cross = (tot - tr.diagonal(dim1=-2, dim2=-1).sum(-1)) / tot
+        off = tr.clone()
+        off.diagonal(dim1=-2, dim2=-1).zero_()
+        balance["machines"] = args.machines
+        balance["cross_machine_fraction"] = {"mean": float(cross[live].mean()), "max": float(cross[live].max())}
+        balance["c_max_tokens"] = {"median": float(off.amax((-1, -2))[live].median()), "max": float(off.max())}
     line = {
         "metric": METRIC_UPDATE if upd else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
@@ -428,11 +446,11 @@ def run_ours(args, cfg) -> None:
         "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
-                   "stage": args.stage, "bytes_per_routed_token": total_bpt,
+                   "stage": args.stage, "machines": args.machines, "bytes_per_routed_token": total_bpt,
                    "launch": "cuda graph replay of the instance loop" if args.graph else "stream launches"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
-    if not args.no_e2e and not upd:
+    if not args.no_e2e and not upd and not args.machines:
         line["e2e"] = run_e2e(args, cfg, wl, dev)
     else:
         wl.release()
@@ -466,6 +484,9 @@ def main() -> None:
     ap.add_argument("--stage", default="recompute", choices=["recompute", "update"],
                     help="recompute = the headline forward path; update = forward + backward of every "
                          "instance (policy-update stage, PAPER.md:241; no e2e / oracle legs)")
+    ap.add_argument("--machines", type=int, default=0,
+                    help="M > 0: per-source, locality-aware Stage 4 over M machines of P/M ranks "
+                         "(commodity plan, SURVEY.md sec. 8(f).1); the data path is unchanged")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -58,6 +58,7 @@ extern "C" {
 #define FOREMOE_FAULT_SLOT_EXPERT 4       /* slot_expert value outside [-1, E)                */
 #define FOREMOE_FAULT_MB_OFF 8            /* mb_off not non-decreasing or not 0 .. T          */
 #define FOREMOE_FAULT_QUOTA_IN 16         /* caller quota violates Eq.(8)/(9) or is negative  */
+#define FOREMOE_FAULT_SOURCE 32           /* tok_src value outside [0, P)                     */
 
 #define FOREMOE_ACT_BF16 0
 #define FOREMOE_ACT_FP32 1
@@ -209,6 +210,51 @@ int foremoe_combine_bwd(const foremoe_shape_t *shape, int32_t layer, int32_t mb_
 int foremoe_dispatch_bwd(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin, int32_t mb_end,
                          const int32_t *mb_off, const int32_t *inv, const void *d_buf, float *dx,
                          int32_t *dev_status, void *stream);
+
+/*
+ * (NEXT) Per-source, multi-machine Stage 4.  Every token has a source rank
+ * (w_{s,e} is a P x E matrix); the P ranks form M machines of R = P / M
+ * consecutive ranks; C_{i,j} of Eq.(5) counts the tokens flowing from the ranks of
+ * machine i to the slots of machine j.  Token assignment follows the paper's locality-aware
+ * heuristic ("tokens prefer same-machine replicas to avoid cross-machine traffic,
+ * and any leftover tokens are routed to minimize per-rank load"), made exact like Stage 4 itself
+ * (readings 29-31): commodity (e, m) = tokens of expert e from sources on machine m; its
+ * allowed hosts are the slots holding e on machine m if there is one, else all slots holding e;
+ * among the assignments respecting the allowed hosts, L_max is minimised by the water-filling of
+ * foremoe_assign.  The three calls below build the VIRTUAL instance on which the four calls of the
+ * hot path then run unchanged:
+ *     virtual expert  v = e * M + m                 (E_v = E * M)
+ *     virtual slot    j * M + m  on the rank of j   (N_b,v = N_b * M, N_r,v = N_r * M, S_v = S * M)
+ *     shape_v = shape with E, Nb, Nr multiplied by M (placement_mb_stride too, if non-zero)
+ *   foremoe_source_ids      -> ids_v;   foremoe_local_placement -> slot_expert_v;
+ *   foremoe_load_hist(shape_v, ids_v)  -> hist_v[n_mb][L][E*M]: hist_v[..][e*M+m] = w_{m,e} summed over
+ *                                         the sources of machine m (with M = P: w_{s,e} itself);
+ *   foremoe_assign(shape_v, ids_v, hist_v, slot_expert_v) -> quota_v[n_mb][L][S*M] with
+ *       quota_v[..][j*M+m] = tokens of source machine m sent to slot j, rank_load (unchanged
+ *       meaning), pair_slot_v = (real slot) * M + (source machine), inv: rows grouped by rank, then
+ *       slot, then source machine, stable in (t, k) order;
+ *   foremoe_dispatch / foremoe_combine / *_bwd (shape_v): unchanged (they read K, H, T, inv only);
+ *   foremoe_traffic(quota_v) -> the M x M traffic matrix of every instance.
+ *
+ * foremoe_source_ids:  tok_src [T] int32 source rank of every token (the same for all layers);
+ *   ids_v [L][T][K] out = ids * M + tok_src[t] / R, or -1 for an id outside [0, E) (fault ID_RANGE)
+ *   or a source outside [0, P) (fault SOURCE).  ids_v may not alias ids.
+ * foremoe_local_placement: slot_expert [L][S] (or [n_mb][L][S] per placement_mb_stride) ->
+ *   slot_expert_v [.][S*M]: v on virtual slot j*M+m iff slot j holds e and (machine(j) == m or
+ *   machine m holds no copy of e), else -1.  Fault SLOT_EXPERT for values outside [-1, E).
+ * foremoe_traffic: traffic [n_mb][L][M][M] int32 out: traffic[..][i][j] = sum over the slots of
+ *   machine j of quota_v[..][slot*M + i]; off-diagonal = C_{i,j} of Eq.(5), diagonal = tokens that
+ *   stay inside machine i.  M <= 128.
+ * `shape` in all three calls is the REAL shape; M must divide P.
+ */
+int foremoe_source_ids(const foremoe_shape_t *shape, int32_t M, const int32_t *ids,
+                       const int32_t *tok_src, int32_t *ids_v, int32_t *dev_status, void *stream);
+
+int foremoe_local_placement(const foremoe_shape_t *shape, int32_t M, const int32_t *slot_expert,
+                            int32_t *slot_expert_v, int32_t *dev_status, void *stream);
+
+int foremoe_traffic(const foremoe_shape_t *shape, int32_t M, const int32_t *quota_v,
+                    int32_t *traffic, void *stream);
 
 /* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
  * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */

@@ -30,13 +30,14 @@ FAULT_NO_HOST = 2
 FAULT_SLOT_EXPERT = 4
 FAULT_MB_OFF = 8
 FAULT_QUOTA_IN = 16
+FAULT_SOURCE = 32
 
 ACT_BF16 = 0
 ACT_FP32 = 1
 
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
-           "foremoe_base_placement",
+           "foremoe_base_placement", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
 
@@ -109,6 +110,9 @@ def lib() -> C.CDLL:
         l.foremoe_combine_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_dispatch_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         l.foremoe_base_placement.argtypes = [sp, vp, vp, vp, vp]
+        l.foremoe_source_ids.argtypes = [sp, i32, vp, vp, vp, vp, vp]
+        l.foremoe_local_placement.argtypes = [sp, i32, vp, vp, vp, vp]
+        l.foremoe_traffic.argtypes = [sp, i32, vp, vp, vp]
         l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
         l.foremoe_step_host.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
@@ -228,6 +232,32 @@ def microstep_placement(shape: Shape, M: int, hist, base_slot_expert, slot_exper
     _check("foremoe_microstep_placement", lib().foremoe_microstep_placement(
         C.byref(shape.c()), M, _dev(hist, torch.int32), _dev(base_slot_expert, torch.int32),
         _dev(slot_expert_mb, torch.int32), _dev(dev_status, torch.int32), _stream()))
+
+
+def source_ids(shape: Shape, M: int, ids, tok_src, ids_v, dev_status=None) -> None:
+    """(f.1) ids_v[L,T,K] = ids * M + tok_src[t] // (P // M): commodity (expert, source machine) ids."""
+    _check("foremoe_source_ids", lib().foremoe_source_ids(
+        C.byref(shape.c()), M, _dev(ids, torch.int32), _dev(tok_src, torch.int32),
+        _dev(ids_v, torch.int32), _dev(dev_status, torch.int32), _stream()))
+
+
+def local_placement(shape: Shape, M: int, slot_expert, slot_expert_v, dev_status=None) -> None:
+    """(f.1) slot_expert [.,S] -> slot_expert_v [.,S*M]: allowed hosts of every commodity."""
+    _check("foremoe_local_placement", lib().foremoe_local_placement(
+        C.byref(shape.c()), M, _dev(slot_expert, torch.int32), _dev(slot_expert_v, torch.int32),
+        _dev(dev_status, torch.int32), _stream()))
+
+
+def traffic(shape: Shape, M: int, quota_v, traffic_out) -> None:
+    """(f.1) quota_v [n_mb,L,S*M] -> traffic [n_mb,L,M,M] (Eq.(5) off the diagonal)."""
+    _check("foremoe_traffic", lib().foremoe_traffic(
+        C.byref(shape.c()), M, _dev(quota_v, torch.int32), _dev(traffic_out, torch.int32), _stream()))
+
+
+def virtual_shape(shape: Shape, M: int) -> Shape:
+    """Shape of the commodity instance: E, Nb, Nr (and the placement stride) multiplied by M."""
+    return dataclasses.replace(shape, E=shape.E * M, Nb=shape.Nb * M, Nr=shape.Nr * M,
+                               placement_mb_stride=shape.placement_mb_stride * M)
 
 
 def step_host_arena_bytes(shape: Shape, mb_off_h) -> int:

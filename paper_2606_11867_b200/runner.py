@@ -68,3 +68,27 @@ class StepPlan:
     def faults(self) -> int:
         """Device fault bits raised so far (synchronises)."""
         return int(self.status.item())
+
+
+class LocalStepPlan(StepPlan):
+    """Per-source, multi-machine plan: the StepPlan of the commodity
+    instance (expert, source machine).  ``shape`` is the REAL shape, ``tok_src`` int32 [T] the source
+    rank of every token, ``M`` the number of machines.  Every attribute of StepPlan then refers to
+    the virtual instance (``hist`` [n_mb,L,E*M], ``quota`` [n_mb,L,S*M], ``pair_slot`` = slot*M +
+    source machine); ``inv`` / dispatch / combine are used exactly as before."""
+
+    def __init__(self, shape: fm.Shape, M: int, ids, w, mb_off, slot_expert, tok_src):
+        self.real_shape, self.M, self.real_ids, self.real_slot_expert, self.tok_src = \
+            shape, M, ids, slot_expert, tok_src
+        sv = fm.virtual_shape(shape, M)
+        dev = ids.device
+        ids_v = torch.empty_like(ids)
+        se_v = torch.empty(tuple(slot_expert.shape[:-1]) + (shape.S * M,), dtype=torch.int32, device=dev)
+        super().__init__(sv, ids_v, w, mb_off, se_v)
+        self.traffic = torch.empty((shape.n_mb, shape.L, M, M), dtype=torch.int32, device=dev)
+
+    def plan(self, quota_in: Optional[torch.Tensor] = None) -> None:
+        fm.source_ids(self.real_shape, self.M, self.real_ids, self.tok_src, self.ids, self.status)
+        fm.local_placement(self.real_shape, self.M, self.real_slot_expert, self.slot_expert, self.status)
+        super().plan(quota_in)
+        fm.traffic(self.real_shape, self.M, self.quota, self.traffic)

@@ -257,6 +257,20 @@ def gen_placement(cfg: TraceConfig, step_hist: np.ndarray) -> np.ndarray:
     return out
 
 
+def gen_tok_src(cfg: TraceConfig) -> np.ndarray:
+    """Source rank of every token (int32 [T]) for the per-source Stage 4:
+    every micro-step's token range is cut into P contiguous, near-equal shares, share s held by
+    logical rank s -- each EP rank contributes its part of the micro-batch to the dispatch
+    (PAPER.md:58, :204 "source rank s")."""
+    off = cfg.mb_off().astype(np.int64)
+    out = np.empty(cfg.T, dtype=np.int32)
+    for i in range(cfg.n_mb):
+        a, b = int(off[i]), int(off[i + 1])
+        if b > a:
+            out[a:b] = (np.arange(b - a, dtype=np.int64) * cfg.P // (b - a)).astype(np.int32)
+    return out
+
+
 def natural_placement(cfg: TraceConfig) -> np.ndarray:
     """The un-balanced default: expert e on rank e // Nb, no replicas (redundant slots empty)."""
     out = np.full((cfg.L, cfg.S), -1, dtype=np.int32)

@@ -249,3 +249,52 @@ def test_full_config_backward(cuda_device, cfg_id):
     first, last = (0, 0), (cfg.L - 1, cfg.n_mb - 1)
     _backward_checks(wl, [first, last] + inst, {first, last})
     assert wl.plan.faults() == 0
+
+
+@pytest.mark.parametrize("cfg_id,M", [(2, 2), (3, 8), (5, 4)])
+def test_full_config_local(cuda_device, cfg_id, M):
+    """Per-source, multi-machine Stage 4 at full size (bench.Workload with machines=M): invariants of
+    the commodity plan for every instance, the locality rule and Eq.(5) traffic by torch library ops,
+    O11 + O3/O4 on the first and last micro-step of layer 0, the data path on one instance."""
+    cfg = synth.config(cfg_id)
+    wl = bench.Workload(cfg, cuda_device, "recompute", M)
+    lp, sv = wl.plan, wl.shape
+    lp.plan()
+    torch.cuda.synchronize()
+    assert lp.faults() == 0 and sv.E == cfg.E * M
+    _properties_all_instances(wl)                      # Eq.(8)/(9), offsets, bijection, stability on commodities
+    R, S = cfg.P // M, cfg.S
+    dev = lp.ids.device
+    src_m = torch.from_numpy(wl.tok_src_h // R).to(dev).long()
+    se = lp.real_slot_expert.long()                    # [L, S]
+    mach_of_slot = (torch.arange(S, device=dev) // cfg.Ns) // R
+    for l in range(cfg.L):
+        ps = lp.pair_slot[l].long()                    # [T, K] = slot * M + source machine
+        assert torch.equal(se[l][(ps // M).view(-1)], lp.real_ids[l].long().view(-1))
+        assert torch.equal(ps % M, src_m[:, None].expand(-1, cfg.K))
+        # locality: a pair leaves its machine only if that machine holds no copy of its expert
+        holds = torch.zeros((cfg.E, M), dtype=torch.bool, device=dev)
+        ok = se[l] >= 0
+        holds[se[l][ok], mach_of_slot[ok]] = True
+        crosses = mach_of_slot[ps // M] != src_m[:, None]
+        assert not (crosses & holds[lp.real_ids[l].long(), src_m[:, None].expand(-1, cfg.K)]).any()
+    q = lp.quota.long().view(cfg.n_mb, cfg.L, M, R * cfg.Ns, M)      # [.., machine of slot, slot in machine, source]
+    assert torch.equal(lp.traffic.long(), q.sum(3).transpose(-1, -2))
+    ids_h = lp.real_ids[0].cpu().numpy()
+    for i in (0, cfg.n_mb - 1):
+        a, b = int(wl.mb_off_h[i]), int(wl.mb_off_h[i + 1])
+        key = np.repeat(wl.tok_src_h[a:b].astype(np.int64), cfg.K) * cfg.E + ids_h[a:b].reshape(-1)
+        w_se = np.bincount(key, minlength=cfg.P * cfg.E).reshape(cfg.P, cfg.E).astype(np.int32)
+        ref = orc.quota_local(w_se, wl.se_h[0], cfg.P, cfg.Ns, M)
+        assert ref["fault"] == 0
+        assert (lp.quota[i, 0].cpu().numpy() == ref["quota_v"]).all(), ("quota_v", i)
+        assert (lp.rank_load[i, 0].cpu().numpy() == ref["rank_load"]).all()
+        assert (lp.traffic[i, 0].cpu().numpy() == ref["traffic"]).all()
+        se_v, f = orc.local_placement(wl.se_h[0], cfg.E, cfg.P, cfg.Ns, M)
+        ids_v = (ids_h[a:b].astype(np.int64) * M + (wl.tok_src_h[a:b] // R)[:, None]).astype(np.int32)
+        ps, inv, perm, f2 = orc.assign_instance(ids_v, se_v, ref["quota_v"], ref["slot_off_v"], cfg.E * M,
+                                                base=a * cfg.K)
+        assert f == 0 and f2 == 0
+        assert (lp.pair_slot[0, a:b].cpu().numpy().ravel() == ps).all(), ("pair_slot_v", i)
+        assert (lp.inv[0, a:b].cpu().numpy().ravel() == inv).all(), ("inv", i)
+    _library_data_checks(wl, [wl.instances[0], wl.instances[-1]])

@@ -714,3 +714,155 @@ done:
   free(c_v); free(se_v); free(q_v); free(so_v);
   return fault;
 }
+
+/* ==========================================================================================
+ * NEXT row (second half): Alg. 2 Stage 2, expert relocation by swaps
+ * (sec. 8.2 prose; listing lines 4-12).
+ *
+ * O12 oracle_swap_relocation, ONE (micro-step, layer) instance.  Every expert sits in exactly one
+ * base slot (A^{(i)} <- A_base, line 2); rank loads RL[r] = L_r and traffic LT[i][j] = C_{i,j}
+ * (Eq.(4)/(5) with one host per expert) are initialised from the placement and the per-source-
+ * machine loads c[m][e] (line 3).  Each round (lines 5-12):
+ *   h = argmax_r RL[r]                                             "bottleneck rank" (ties: lowest rank)
+ *   for each r_l != h: "evaluate swapping a top-K heaviest expert on h with a top-K lightest
+ *   expert on r_l": window of `win` experts on each side (heaviest: descending load, ties
+ *   ascending id; lightest: ascending load, ties ascending id);
+ *   Delta = change of the layer-time objective  F = a * max_r RL[r] + b * max_{i != j} LT[i][j]
+ *   (Eq.(3) without its constants: a stands for n1*K1, b for n2*K2, caller-supplied integers --
+ *   the paper never prints them, reading 33);
+ *   the swap minimising Delta wins (ties: first in the order r_l ascending, then the heaviest-
+ *   window order, then the lightest-window order); "if Delta >= 0 then break"; else the two
+ *   experts exchange their slots and RL, LT are updated.
+ * At most max_rounds rounds ("maximum round count").  Redundant slots are copied
+ * unchanged from base_se (Stage 3 fills them later).
+ * stats (may be NULL): [0] rounds applied, [1..2] objective before / after (int64 as two int32 is
+ * avoided: written as int64_t stats[3]).
+ * Pins (tests/test_oracle_swap.py): hand-worked vectors (tests/golden/swap_vectors.json); the
+ * objective strictly decreases per applied swap (replayed from the placements with numpy);
+ * termination = no improving swap in the bottleneck's window (independent enumeration); structure;
+ * balanced input => unchanged; win covering all experts + P = 2 => each round takes the best of
+ * all swaps (brute force).
+ * ========================================================================================== */
+static int64_t swap_objective(int P, int M, int64_t a, int64_t b, const int64_t *RL, const int64_t *LT) {
+  int64_t lmax = 0, cmax = 0;
+  for (int r = 0; r < P; r++) if (RL[r] > lmax) lmax = RL[r];
+  for (int i = 0; i < M; i++)
+    for (int j = 0; j < M; j++)
+      if (i != j && LT[i * M + j] > cmax) cmax = LT[i * M + j];
+  return a * lmax + b * cmax;
+}
+
+int oracle_swap_relocation(int E, int P, int Nb, int Nr, int M, int win, int max_rounds, int64_t a,
+                           int64_t b, const int32_t *c_me /* [M][E] */, const int32_t *base_se,
+                           int32_t *out_se, int64_t *stats /* [3] or NULL */) {
+  const int Ns = Nb + Nr, S = P * Ns;
+  if (M <= 0 || P % M != 0 || win <= 0 || max_rounds < 0 || a < 0 || b < 0) return ORACLE_BAD_ARG;
+  const int R = P / M;
+  int fault = 0;
+  for (int j = 0; j < S; j++) out_se[j] = base_se[j];
+  int64_t *c = (int64_t *)calloc((size_t)E, sizeof(int64_t));
+  int32_t *slot_of = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int64_t *RL = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  int64_t *LT = (int64_t *)calloc((size_t)M * M, sizeof(int64_t));
+  int64_t *RL2 = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  int64_t *LT2 = (int64_t *)calloc((size_t)M * M, sizeof(int64_t));
+  int32_t *heavy = (int32_t *)calloc((size_t)Nb, sizeof(int32_t));
+  int32_t *light = (int32_t *)calloc((size_t)Nb, sizeof(int32_t));
+  if (!c || !slot_of || !RL || !LT || !RL2 || !LT2 || !heavy || !light) { fault = ORACLE_NO_MEM; goto done; }
+  for (int e = 0; e < E; e++) {
+    slot_of[e] = -1;
+    for (int m = 0; m < M; m++) {
+      if (c_me[(size_t)m * E + e] < 0) fault |= FAULT_ID_RANGE;
+      c[e] += c_me[(size_t)m * E + e];
+    }
+  }
+  for (int j = 0; j < S; j++) {
+    const int32_t e = base_se[j];
+    if (e < -1 || e >= E) { fault |= FAULT_SLOT_EXPERT; continue; }
+    if (e < 0 || j % Ns >= Nb) continue;                  /* only base slots take part */
+    if (slot_of[e] >= 0) fault |= FAULT_SLOT_EXPERT;      /* expert twice in base slots */
+    slot_of[e] = j;
+  }
+  for (int e = 0; e < E; e++) if (slot_of[e] < 0) fault |= FAULT_SLOT_EXPERT;
+  if (fault) goto done;
+  for (int e = 0; e < E; e++) {                           /* line 3 */
+    const int r = slot_of[e] / Ns;
+    RL[r] += c[e];
+    for (int i = 0; i < M; i++) LT[i * M + r / R] += c_me[(size_t)i * E + e];
+  }
+  const int64_t F0 = swap_objective(P, M, a, b, RL, LT);
+  int64_t F = F0;
+  int rounds = 0;
+  for (int round = 0; round < max_rounds; round++) {
+    int h = 0;
+    for (int r = 1; r < P; r++) if (RL[r] > RL[h]) h = r;
+    /* window on h: the `win` heaviest experts, descending load, ties ascending id */
+    int nh = 0;
+    for (int k = 0; k < win && k < Nb; k++) {
+      int best = -1;
+      for (int j = h * Ns; j < h * Ns + Nb; j++) {
+        const int e = out_se[j];
+        int taken = 0;
+        if (e < 0) continue;
+        for (int q = 0; q < nh; q++) taken |= (heavy[q] == e);
+        if (taken) continue;
+        if (best < 0 || c[e] > c[best] || (c[e] == c[best] && e < best)) best = e;
+      }
+      if (best < 0) break;
+      heavy[nh++] = best;
+    }
+    int64_t best_delta = 0;
+    int best_eh = -1, best_el = -1;
+    for (int rl = 0; rl < P; rl++) {
+      if (rl == h) continue;
+      int nl = 0;                                         /* the `win` lightest experts on r_l */
+      for (int k = 0; k < win && k < Nb; k++) {
+        int best = -1;
+        for (int j = rl * Ns; j < rl * Ns + Nb; j++) {
+          const int e = out_se[j];
+          int taken = 0;
+          if (e < 0) continue;
+          for (int q = 0; q < nl; q++) taken |= (light[q] == e);
+          if (taken) continue;
+          if (best < 0 || c[e] < c[best] || (c[e] == c[best] && e < best)) best = e;
+        }
+        if (best < 0) break;
+        light[nl++] = best;
+      }
+      for (int x = 0; x < nh; x++)
+        for (int y = 0; y < nl; y++) {
+          const int eh = heavy[x], el = light[y];
+          memcpy(RL2, RL, sizeof(int64_t) * (size_t)P);
+          memcpy(LT2, LT, sizeof(int64_t) * (size_t)M * M);
+          RL2[h] += c[el] - c[eh];
+          RL2[rl] += c[eh] - c[el];
+          for (int i = 0; i < M; i++) {
+            LT2[i * M + h / R] += (int64_t)c_me[(size_t)i * E + el] - c_me[(size_t)i * E + eh];
+            LT2[i * M + rl / R] += (int64_t)c_me[(size_t)i * E + eh] - c_me[(size_t)i * E + el];
+          }
+          const int64_t delta = swap_objective(P, M, a, b, RL2, LT2) - F;
+          if (delta < best_delta) { best_delta = delta; best_eh = eh; best_el = el; }   /* strict: first wins ties */
+        }
+    }
+    if (best_eh < 0) break;                               /* "if Delta >= 0 then break" */
+    {
+      const int jh = slot_of[best_eh], jl = slot_of[best_el];
+      const int rl = jl / Ns;
+      RL[h] += c[best_el] - c[best_eh];
+      RL[rl] += c[best_eh] - c[best_el];
+      for (int i = 0; i < M; i++) {
+        LT[i * M + h / R] += (int64_t)c_me[(size_t)i * E + best_el] - c_me[(size_t)i * E + best_eh];
+        LT[i * M + rl / R] += (int64_t)c_me[(size_t)i * E + best_eh] - c_me[(size_t)i * E + best_el];
+      }
+      out_se[jh] = best_el; out_se[jl] = best_eh;
+      slot_of[best_eh] = jl; slot_of[best_el] = jh;
+      F += best_delta;
+      rounds++;
+    }
+  }
+  if (stats) { stats[0] = rounds; stats[1] = F0; stats[2] = F; }
+done:
+  if (fault > 0) for (int j = 0; j < S; j++) out_se[j] = -1;
+  free(c); free(slot_of); free(RL); free(LT); free(RL2); free(LT2); free(heavy); free(light);
+  return fault;
+}

@@ -209,3 +209,17 @@ def quota_local(w_se: np.ndarray, slot_expert: np.ndarray, P: int, Ns: int, M: i
                                             _p(out["rank_load"]), _p(out["traffic"]),
                                             _p(out["quota_v"]), _p(out["slot_off_v"]))
     return out
+
+
+def swap_relocation(c_me: np.ndarray, base_se: np.ndarray, P: int, Nb: int, Nr: int, M: int = 1,
+                    win: int = 2, max_rounds: int = 16, a: int = 1, b: int = 0):
+    """O12 for one instance: per-source-machine loads int32 [M,E] (or [E] with M = 1), base
+    placement [S] -> relocated placement [S], stats (rounds, objective before, after), fault."""
+    c_me = _i32(c_me).reshape(M, -1)
+    base_se = _i32(base_se)
+    out = np.full(P * (Nb + Nr), -1, dtype=np.int32)
+    stats = np.zeros(3, dtype=np.int64)
+    f = lib().oracle_swap_relocation
+    f.argtypes = [C.c_int] * 7 + [C.c_int64, C.c_int64] + [C.c_void_p] * 4
+    fault = f(c_me.shape[1], P, Nb, Nr, M, win, max_rounds, a, b, _p(c_me), _p(base_se), _p(out), _p(stats))
+    return out, stats, fault

@@ -256,6 +256,30 @@ int foremoe_local_placement(const foremoe_shape_t *shape, int32_t M, const int32
 int foremoe_traffic(const foremoe_shape_t *shape, int32_t M, const int32_t *quota_v,
                     int32_t *traffic, void *stream);
 
+/*
+ * (NEXT, second half) Alg. 2 Stage 2: expert relocation by swaps
+ * (sec. 8.2; listing lines 4-12) for every (micro-step, layer)
+ * instance, starting from the base placement (every expert in exactly one base slot).  Each round:
+ * h = the most loaded rank (ties: lowest rank); for every other rank r_l the `win` heaviest experts
+ * on h (descending load, ties ascending id) x the `win` lightest experts on r_l (ascending load,
+ * ties ascending id); the swap with the smallest change Delta of the layer-time objective
+ *     F = a * max_r RL[r] + b * max_{i != j} LT[i][j]          (Eq.(3) without its constants;
+ *     a ~ n1*K1, b ~ n2*K2 are caller-supplied integers in [0, 2^20]: DESIGN.md reading 33)
+ * wins (ties: first in the order r_l ascending, heaviest-window order, lightest-window order);
+ * stop when Delta >= 0 or after max_rounds rounds; otherwise the two experts exchange slots.
+ *   hist_v           [n_mb][L][E*M]: load of expert e from the sources of machine m at e*M + m
+ *                    (foremoe_load_hist on foremoe_source_ids' output; with M = 1 the plain hist).
+ *   base_slot_expert [L][S]; redundant slots are copied through unchanged.
+ *   slot_expert_mb   [n_mb][L][S] out (feed it to foremoe_assign with placement_mb_stride = L*S).
+ *   rounds           [n_mb][L] out or NULL: swaps applied per instance.
+ * Faults: SLOT_EXPERT (base placement has a bad value, or an expert twice / missing in the base
+ * slots), ID_RANGE (negative load): that instance's output is all -1.
+ */
+int foremoe_swap_relocation(const foremoe_shape_t *shape, int32_t M, int32_t win, int32_t max_rounds,
+                            int64_t a, int64_t b, const int32_t *hist_v,
+                            const int32_t *base_slot_expert, int32_t *slot_expert_mb, int32_t *rounds,
+                            int32_t *dev_status, void *stream);
+
 /* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
  * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */
 int foremoe_step_host_arena_bytes(const foremoe_shape_t *shape, const int32_t *mb_off_h,

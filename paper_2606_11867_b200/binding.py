@@ -38,6 +38,7 @@ ACT_FP32 = 1
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
+           "foremoe_swap_relocation",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
 
@@ -113,6 +114,7 @@ def lib() -> C.CDLL:
         l.foremoe_source_ids.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_local_placement.argtypes = [sp, i32, vp, vp, vp, vp]
         l.foremoe_traffic.argtypes = [sp, i32, vp, vp, vp]
+        l.foremoe_swap_relocation.argtypes = [sp, i32, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp]
         l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
         l.foremoe_step_host.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
@@ -252,6 +254,15 @@ def traffic(shape: Shape, M: int, quota_v, traffic_out) -> None:
     """(f.1) quota_v [n_mb,L,S*M] -> traffic [n_mb,L,M,M] (Eq.(5) off the diagonal)."""
     _check("foremoe_traffic", lib().foremoe_traffic(
         C.byref(shape.c()), M, _dev(quota_v, torch.int32), _dev(traffic_out, torch.int32), _stream()))
+
+
+def swap_relocation(shape: Shape, M: int, win: int, max_rounds: int, a: int, b: int, hist_v,
+                    base_slot_expert, slot_expert_mb, rounds=None, dev_status=None) -> None:
+    """(f.2) Alg. 2 Stage 2: hist_v [n_mb,L,E*M] + base [L,S] -> slot_expert_mb [n_mb,L,S]."""
+    _check("foremoe_swap_relocation", lib().foremoe_swap_relocation(
+        C.byref(shape.c()), M, win, max_rounds, a, b, _dev(hist_v, torch.int32),
+        _dev(base_slot_expert, torch.int32), _dev(slot_expert_mb, torch.int32),
+        _dev(rounds, torch.int32), _dev(dev_status, torch.int32), _stream()))
 
 
 def virtual_shape(shape: Shape, M: int) -> Shape:

@@ -115,3 +115,92 @@ def test_stages_2_to_4_pipeline(cuda_device, cfg_id, kw):
             ref["perm"][l, ref["inv"][l].ravel()[a:b]] = np.arange(a, b)
     x = G.activations(cfg, mb_off, range(cfg.n_mb))
     G.check_data_path(sp, ref, x, range(cfg.L), range(cfg.n_mb), "stages2-4")
+
+
+# ------------------------------------------------------------------ Alg. 2 Stage 2 (swap relocation, O12)
+def _swap_gpu(shape, M, win, rounds, a, b, hist_v, base):
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    out = torch.full((shape.n_mb, shape.L, shape.S), -7, dtype=torch.int32, device=dev)
+    nr = torch.full((shape.n_mb, shape.L), -7, dtype=torch.int32, device=dev)
+    fm.swap_relocation(shape, M, win, rounds, a, b, torch.as_tensor(hist_v, dtype=torch.int32).to(dev),
+                       torch.as_tensor(base, dtype=torch.int32).to(dev), out, nr, st)
+    torch.cuda.synchronize()
+    return out.cpu().numpy(), nr.cpu().numpy(), int(st.item())
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_swap_relocation_random(cuda_device, seed):
+    rng = np.random.default_rng(70 + seed)
+    P, M, Nb, Nr = [(2, 1, 2, 1), (4, 2, 4, 1), (8, 2, 16, 2), (8, 8, 4, 0), (64, 8, 4, 1), (32, 4, 16, 4),
+                    (6, 3, 5, 2), (40, 1, 3, 1)][seed]
+    win = [2, 1, 4, 3, 2, 40, 2, 3][seed]
+    a, b = [(1, 0), (1, 1), (3, 2), (0, 1), (1, 1), (2, 1), (1, 5), (1, 0)][seed]
+    E, L, n_mb, Ns = P * Nb, 3, 5, Nb + Nr
+    shape = fm.Shape(L=L, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=n_mb, H=8, act_dtype=fm.ACT_FP32)
+    hist_v = (rng.integers(0, 400, size=(n_mb, L, E, M)) * (rng.random((n_mb, L, E, M)) < 0.8)).astype(np.int32)
+    hist_v[1] = 9                                     # all equal: nothing to gain, pure tie handling
+    hist_v[2, :, : E // 2] = 0                        # many zero loads
+    base = np.full((L, P * Ns), -1, dtype=np.int32)
+    for l in range(L):
+        perm = rng.permutation(E)
+        for r in range(P):
+            base[l, r * Ns:r * Ns + Nb] = perm[r * Nb:(r + 1) * Nb]
+            base[l, r * Ns + Nb:(r + 1) * Ns] = -1
+    out, nr, fault = _swap_gpu(shape, M, win, 24, a, b, hist_v.reshape(n_mb, L, E * M), base)
+    assert fault == 0
+    moved = 0
+    for i in range(n_mb):
+        for l in range(L):
+            ref, st, f = orc.swap_relocation(hist_v[i, l].T.copy(), base[l], P, Nb, Nr, M, win, 24, a, b)
+            assert f == 0 and (out[i, l] == ref).all(), ("swap", i, l)
+            assert nr[i, l] == st[0]
+            moved += int(st[0])
+    assert moved > 0
+    # fewer rounds allowed: the prefix of the same sequence
+    out2, nr2, _ = _swap_gpu(shape, M, win, 1, a, b, hist_v.reshape(n_mb, L, E * M), base)
+    ref, st, f = orc.swap_relocation(hist_v[0, 0].T.copy(), base[0], P, Nb, Nr, M, win, 1, a, b)
+    assert (out2[0, 0] == ref).all() and nr2[0, 0] == st[0]
+
+
+def test_swap_relocation_golden_and_faults(cuda_device):
+    shape = fm.Shape(L=1, E=4, K=1, P=2, Nb=2, Nr=1, T=8, n_mb=1, H=8, act_dtype=fm.ACT_FP32)
+    base = np.array([[0, 1, -1, 2, 3, -1]], dtype=np.int32)
+    out, nr, fault = _swap_gpu(shape, 1, 2, 8, 1, 0, np.array([[[9, 8, 1, 2]]]), base)
+    assert fault == 0 and out.reshape(2, 3).tolist() == [[3, 1, -1], [2, 0, -1]] and nr.item() == 1
+    hv = np.array([[5, 0, 6, 1], [1, 2, 0, 7]]).T.reshape(1, 1, 8)            # [e*M + m]
+    out, nr, fault = _swap_gpu(shape, 2, 2, 8, 0, 1, hv, base)
+    assert fault == 0 and out.reshape(2, 3).tolist() == [[0, 2, -1], [1, 3, -1]] and nr.item() == 1
+    bad = base.copy(); bad[0, 1] = 0
+    out, nr, fault = _swap_gpu(shape, 1, 2, 8, 1, 0, np.array([[[9, 8, 1, 2]]]), bad)
+    assert fault & fm.FAULT_SLOT_EXPERT and (out == -1).all()
+    out, nr, fault = _swap_gpu(shape, 1, 2, 8, 1, 0, np.array([[[9, -8, 1, 2]]]), base)
+    assert fault & fm.FAULT_ID_RANGE and (out == -1).all()
+    with pytest.raises(fm.ForeMoEError):
+        _swap_gpu(shape, 3, 2, 8, 1, 0, np.zeros((1, 1, 12)), base)           # 3 does not divide P
+    with pytest.raises(fm.ForeMoEError):
+        _swap_gpu(shape, 1, 0, 8, 1, 0, np.zeros((1, 1, 4)), base)            # empty window
+
+
+def test_swap_then_stage4_on_config_trace(cuda_device):
+    """End to end on a config-2-shaped trace: load_hist -> base placement -> swap relocation ->
+    foremoe_assign on the per-micro-step placements; the max rank load never gets worse than with
+    the base placement alone, and the plan stays consistent with the oracle."""
+    cfg = synth.config(2).scaled(L=2, n_samples=16, sample_len=512, H=64, mb_samples=4)
+    ids, w, mb_off, _ = G.make_case(cfg)
+    shape = fm.shape_of(cfg)
+    hist, step, _ = orc.load_hist(ids, mb_off, cfg.E)
+    base = np.stack([orc.base_placement(step[l], cfg.P, cfg.Nb, cfg.Nr)[0] for l in range(cfg.L)])
+    out, nr, fault = _swap_gpu(shape, 1, 4, 32, 1, 0, hist, base)
+    assert fault == 0
+    sp0 = G.gpu_plan(shape, ids, w, mb_off, base)
+    shape_mb = dataclasses.replace(shape, placement_mb_stride=shape.L * shape.S)
+    sp1 = G.gpu_plan(shape_mb, ids, w, mb_off, out)
+    assert sp0.faults() == 0 and sp1.faults() == 0
+    m0 = sp0.rank_load.max(-1).values.cpu().numpy()
+    m1 = sp1.rank_load.max(-1).values.cpu().numpy()
+    assert (m1 <= m0).all() and (m1 < m0).any()
+    for i in range(cfg.n_mb):
+        for l in range(cfg.L):
+            q, rl, so, _, f = orc.quota(hist[i, l], out[i, l], cfg.P, cfg.Ns)
+            assert f == 0 and (sp1.quota[i, l].cpu().numpy() == q).all()

@@ -103,6 +103,56 @@ def bwd_sweep(wl, cfg, bench) -> None:
     set_tuning()
 
 
+def planner_times(wl, cfg, M: int) -> None:
+    """Whole-step times of the planner stages that run ahead of the data path (all instances of the
+    step in one launch each): Stage 1, Alg. 3 Stages 2-3, Alg. 2 Stage 2, and Stage 4 on the result."""
+    import dataclasses
+    s, dev = wl.shape, wl.dev
+    p = wl.plan
+    p.load_hist()
+    base = torch.empty((s.L, s.S), dtype=torch.int32, device=dev)
+    mbp = torch.empty((s.n_mb, s.L, s.S), dtype=torch.int32, device=dev)
+    swp = torch.empty_like(mbp)
+    rounds = torch.empty((s.n_mb, s.L), dtype=torch.int32, device=dev)
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    s_mb = dataclasses.replace(s, placement_mb_stride=s.L * s.S)
+    ws_mb = torch.empty(fm.workspace_bytes(s_mb) + 16, dtype=torch.uint8, device=dev)   # one table set per instance
+
+    def assign_mb(se_mb):
+        fm.assign(s_mb, p.ids, p.mb_off, p.hist, se_mb, None, p.quota, p.rank_load, p.slot_off, p.pair_slot,
+                  p.inv, ws_mb, st)
+
+    def ratio():
+        rl = p.rank_load.float()
+        r = (rl.max(-1).values / rl.mean(-1).clamp(min=1e-9))
+        return {"median": round(float(r.median()), 4), "mean": round(float(r.mean()), 4), "max": round(float(r.max()), 4)}
+
+    calls = [
+        ("foremoe_load_hist", p.load_hist, None),
+        ("foremoe_assign (step-level placement from the harness)", p.assign, ratio),
+        ("foremoe_base_placement (Stage 1)", lambda: fm.base_placement(s, p.step_hist, base, st), None),
+        (f"foremoe_microstep_placement (Alg. 3 Stages 2-3, M={M})", lambda: fm.microstep_placement(s, M, p.hist, base, mbp, st), None),
+        ("foremoe_assign on Alg. 3 placements", lambda: assign_mb(mbp), ratio),
+        ("foremoe_swap_relocation (Alg. 2 Stage 2, M=1, win=4, <=32 rounds, a=1 b=0)",
+         lambda: fm.swap_relocation(s, 1, 4, 32, 1, 0, p.hist, base, swp, rounds, st), None),
+        ("foremoe_assign on swap-relocated placements (no replicas)", lambda: assign_mb(swp), ratio),
+    ]
+    for name, fn, after in calls:
+        ts = []
+        for r in range(5):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            if r >= 2:
+                ts.append(a.elapsed_time(b))
+        line = {"call": name, "ms": round(float(np.mean(ts)), 3), "instances": cfg.L * cfg.n_mb}
+        if after:
+            line["lmax_over_lmean"] = after()
+        if "swap_relocation" in name:
+            line["rounds"] = {"mean": round(float(rounds.float().mean()), 2), "max": int(rounds.max())}
+        print(json.dumps(line), flush=True)
+    assert int(st.item()) == 0, int(st.item())
+
+
 def hist_sweep(wl, cfg) -> None:
     """foremoe_load_hist with each k_load_hist mode on the config's trace and on the worst case
     for shared atomics (every pair selects expert 0); results are checked against each other."""
@@ -135,19 +185,27 @@ def hist_sweep(wl, cfg) -> None:
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, default=2)
-    ap.add_argument("--layers", type=int, default=2)
+    ap.add_argument("--layers", type=int, default=2, help="0 = all layers of the config")
     ap.add_argument("--samples", type=int, default=None, help="fewer samples (config 3: 32)")
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--hist", action="store_true", help="sweep the k_load_hist modes instead")
     ap.add_argument("--plan", action="store_true", help="time foremoe_load_hist / foremoe_assign only")
     ap.add_argument("--bwd", action="store_true", help="sweep the backward kernels instead")
+    ap.add_argument("--planner", action="store_true", help="time the planner stages (placement, relocation, Stage 4)")
+    ap.add_argument("--machines", type=int, default=1, help="--planner: machines for Alg. 3")
     args = ap.parse_args()
     import bench
-    cfg = synth.config(args.config).scaled(L=args.layers, n_samples=args.samples)
+    cfg = synth.config(args.config)
+    if args.layers > 0 or args.samples:
+        cfg = cfg.scaled(L=args.layers if args.layers > 0 else None, n_samples=args.samples)
     dev = torch.device("cuda:0")
     wl = bench.Workload(cfg, dev, "update" if args.bwd else "recompute")
     if args.bwd:
         bwd_sweep(wl, cfg, bench)
+        return
+    if args.planner:
+        print(json.dumps({"workload": bench.workload_name(cfg)}), flush=True)
+        planner_times(wl, cfg, args.machines)
         return
     if args.hist:
         hist_sweep(wl, cfg)

@@ -197,7 +197,7 @@ class Workload:
     """Device-resident inputs and outputs of one rank's step (inputs are seeded and synthetic:
     recipe in DESIGN.md sec. 4).  Nothing here is timed."""
 
-    def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0):
+    def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0, planner: str = "stage4"):
         from paper_2606_11867_b200 import binding as fm
         from paper_2606_11867_b200 import runner
         self.fm, self.cfg, self.dev = fm, cfg, dev
@@ -211,8 +211,12 @@ class Workload:
         step_hist = self.plan.step_hist.cpu().numpy()
         self.se_h = synth.gen_placement(cfg, step_hist)
         self.plan.slot_expert.copy_(torch.from_numpy(self.se_h))
-        self.machines = machines
-        if machines:        # per-source, multi-machine Stage 4: commodity plan
+        self.machines, self.planner = machines, planner
+        if planner == "full":   # Stages 1-4 on the device: the harness placement above is not used
+            self.plan = None
+            self.plan = runner.PlannerStepPlan(s, max(machines, 1), ids, w, mb_off)
+            self.shape = self.plan.shape
+        elif machines:        # per-source, multi-machine Stage 4: commodity plan
             self.tok_src_h = synth.gen_tok_src(cfg)
             se_dev = self.plan.slot_expert
             self.plan = None
@@ -229,7 +233,8 @@ class Workload:
         self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
         self.routed_tokens = sum(tok) * s.L
         self.stage = stage
-        self.launches_per_step = 2 + 5 + (3 if machines else 0) + (4 if stage == "update" else 2) * len(self.instances)
+        self.launches_per_step = (2 + 5 + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
+                                  + (4 if stage == "update" else 2) * len(self.instances))
         if stage == "update":          # forward + backward of every instance
             self.dy = torch.randn((mx, s.H), dtype=torch.float32, device=dev,
                                   generator=torch.Generator(device=dev).manual_seed(cfg.seed + 11))
@@ -362,7 +367,7 @@ def run_ours(args, cfg) -> None:
     torch.cuda.set_device(dev)
     multi.init("nccl", dev)
     cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
-    wl = Workload(cfg, dev, args.stage, args.machines)
+    wl = Workload(cfg, dev, args.stage, args.machines, args.planner)
     bpt = bytes_per_token(cfg)
     upd = args.stage == "update"
     total_bpt = bpt["total_update"] if upd else bpt["total"]
@@ -421,7 +426,7 @@ def run_ours(args, cfg) -> None:
     rl = wl.plan.rank_load.float()
     live = rl.sum(-1) > 0
     ratio = (rl.max(-1).values / rl.mean(-1).clamp(min=1e-9))[live]
-    hist_real = wl.plan.hist if not args.machines else wl.plan.hist.view(cfg.n_mb, cfg.L, cfg.E, args.machines).sum(-1)
+    hist_real = wl.plan.hist if (not args.machines or args.planner == "full") else wl.plan.hist.view(cfg.n_mb, cfg.L, cfg.E, args.machines).sum(-1)
     nat = hist_real.float().view(cfg.n_mb, cfg.L, cfg.P, cfg.Nb).sum(-1)
     nratio = (nat.max(-1).values / nat.mean(-1).clamp(min=1e-9))[live]
     balance = {"lmax_over_lmean": {"max": float(ratio.max()), "mean": float(ratio.mean()),
@@ -429,7 +434,7 @@ def run_ours(args, cfg) -> None:
                "natural_placement": {"max": float(nratio.max()), "mean": float(nratio.mean()),
                                      "median": float(nratio.median())}}
 
-    if args.machines:
+    if args.machines and args.planner != "full":
         tr = wl.plan.traffic.double()
         tot = tr.sum((-1, -2)).clamp(min=1)
         cross = (tot - tr.diagonal(dim1=-2, dim2=-1).sum(-1)) / tot
@@ -446,11 +451,11 @@ def run_ours(args, cfg) -> None:
         "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
-                   "stage": args.stage, "machines": args.machines, "bytes_per_routed_token": total_bpt,
+                   "stage": args.stage, "machines": args.machines, "planner": args.planner, "bytes_per_routed_token": total_bpt,
                    "launch": "cuda graph replay of the instance loop" if args.graph else "stream launches"},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
-    if not args.no_e2e and not upd and not args.machines:
+    if not args.no_e2e and not upd and not args.machines and args.planner != "full":
         line["e2e"] = run_e2e(args, cfg, wl, dev)
     else:
         wl.release()
@@ -487,6 +492,10 @@ def main() -> None:
     ap.add_argument("--machines", type=int, default=0,
                     help="M > 0: per-source, locality-aware Stage 4 over M machines of P/M ranks "
                          "(commodity plan, SURVEY.md sec. 8(f).1); the data path is unchanged")
+    ap.add_argument("--planner", default="stage4", choices=["stage4", "full"],
+                    help="stage4 = the headline path (step-level placement is an input, Stage 4 on the GPU); "
+                         "full = Stage 1 + Alg. 3 Stages 2-3 + Stage 4 all on the GPU inside the timed step "
+                         "(--machines M then restricts relocation / replication to machines of P/M ranks)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

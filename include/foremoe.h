@@ -280,6 +280,23 @@ int foremoe_swap_relocation(const foremoe_shape_t *shape, int32_t M, int32_t win
                             const int32_t *base_slot_expert, int32_t *slot_expert_mb, int32_t *rounds,
                             int32_t *dev_status, void *stream);
 
+/*
+ * (NEXT) Stage 3 alone: replication on per-micro-step placements whose base
+ * slots are already final -- the output of foremoe_swap_relocation -- with Alg. 3's choice rule
+ * (readings 22-25), so that Alg. 2's relocation by swaps, replication
+ * and Stage 4 compose.  (Alg. 2's own replica score, an "estimated drop" under a locality-aware
+ * assignment, is not defined precisely enough to restate: DESIGN.md reading 36.)
+ *   hist                  [n_mb][L][E] micro-step loads.
+ *   placed_slot_expert_mb [n_mb][L][S]: every expert exactly once in the base slots; the
+ *                         redundant slots of the input are not read.
+ *   slot_expert_mb        [n_mb][L][S] out (may alias the input): base slots copied, redundant
+ *                         slots filled by R * N_r rounds per machine, -1 where nothing is left.
+ * Faults: SLOT_EXPERT, ID_RANGE as in foremoe_microstep_placement (instance output all -1).
+ */
+int foremoe_replication(const foremoe_shape_t *shape, int32_t M, const int32_t *hist,
+                        const int32_t *placed_slot_expert_mb, int32_t *slot_expert_mb,
+                        int32_t *dev_status, void *stream);
+
 /* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
  * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */
 int foremoe_step_host_arena_bytes(const foremoe_shape_t *shape, const int32_t *mb_off_h,

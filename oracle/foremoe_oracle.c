@@ -461,8 +461,8 @@ int oracle_base_placement(int E, int P, int Nb, int Nr, const int64_t *tot, int3
 /* exact integer even split of c over n hosts: host idx (ascending slot order) carries this much */
 static int64_t even_share(int64_t c, int n, int idx) { return c / n + (idx < c % n ? 1 : 0); }
 
-int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_t *c32,
-                               const int32_t *base_se, int32_t *out_se) {
+static int microstep_impl(int E, int P, int Nb, int Nr, int M, const int32_t *c32,
+                          const int32_t *base_se, int32_t *out_se, int relocate) {
   const int Ns = Nb + Nr, S = P * Ns;
   int fault = 0;
   for (int j = 0; j < S; j++) out_se[j] = -1;
@@ -481,6 +481,7 @@ int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_
 
   for (int e = 0; e < E; e++) { c[e] = c32[e]; if (c32[e] < 0) fault |= FAULT_ID_RANGE; mach[e] = -1; }
   for (int j = S - 1; j >= 0; j--) {       /* machine of e = machine of its lowest-indexed base slot */
+    if (!relocate && j % Ns >= Nb) continue;   /* O13 does not read the input's redundant slots */
     const int32_t e = base_se[j];
     if (e < -1 || e >= E) { fault |= FAULT_SLOT_EXPERT; continue; }
     if (e >= 0) mach[e] = (j / Ns) / R;
@@ -500,8 +501,24 @@ int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_
     while (b > 0 && heavier(c, e, order[b - 1])) { order[b] = order[b - 1]; b--; }
     order[b] = e;
   }
+  if (!relocate) {
+    /* O13: the relocation was done by someone else (Alg. 2 Stage 2 swaps, O12): every expert stays in
+     * the base slot it was given; the input must hold each expert exactly once in the base slots */
+    for (int e = 0; e < E; e++) {
+      int n = 0, at = -1;
+      for (int j = 0; j < S; j++)
+        if (base_se[j] == e && j % Ns < Nb) { n++; if (at < 0) at = j; }
+      if (n != 1) { fault |= FAULT_SLOT_EXPERT; continue; }
+      out_se[at] = e;
+      mach[e] = (at / Ns) / R;                 /* the input's redundant slots are ignored */
+      nb[at / Ns] += 1;
+      RL[at / Ns] += c[e];
+      copies[e] = 1;
+    }
+    if (fault) { for (int j = 0; j < S; j++) out_se[j] = -1; goto done; }
+  }
   /* Stage 2: LPT relocation inside each machine (Alg. 3 lines 4-10) */
-  for (int a = 0; a < E; a++) {
+  for (int a = 0; a < E && relocate; a++) {
     const int e = order[a], m = mach[e];
     int best = -1;
     for (int r = m * R; r < (m + 1) * R; r++)
@@ -549,6 +566,21 @@ int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_
 done:
   free(c); free(mach); free(order); free(RL); free(nb); free(nr); free(copies); free(dead); free(hosts);
   return fault;
+}
+
+int oracle_microstep_placement(int E, int P, int Nb, int Nr, int M, const int32_t *c32,
+                               const int32_t *base_se, int32_t *out_se) {
+  return microstep_impl(E, P, Nb, Nr, M, c32, base_se, out_se, 1);
+}
+
+/* O13 oracle_replication: Stage 3 alone (Alg. 3 lines 12-16 / the replication loop of Alg. 2 lines
+ * 14-19 with Alg. 3's choice rule, readings 22-25) on a placement whose base slots are already
+ * final -- e.g. the output of O12 -- so that swaps (Alg. 2 Stage 2) + replication + Stage 4 compose.
+ * Redundant slots of the input are ignored and rebuilt.  Pins: equals O8 when fed O8's own Stage-2
+ * result; structure; first replica = heaviest expert on the least-loaded other rank. */
+int oracle_replication(int E, int P, int Nb, int Nr, int M, const int32_t *c32,
+                       const int32_t *placed_se, int32_t *out_se) {
+  return microstep_impl(E, P, Nb, Nr, M, c32, placed_se, out_se, 0);
 }
 
 /* ==========================================================================================

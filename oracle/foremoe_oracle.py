@@ -223,3 +223,12 @@ def swap_relocation(c_me: np.ndarray, base_se: np.ndarray, P: int, Nb: int, Nr: 
     f.argtypes = [C.c_int] * 7 + [C.c_int64, C.c_int64] + [C.c_void_p] * 4
     fault = f(c_me.shape[1], P, Nb, Nr, M, win, max_rounds, a, b, _p(c_me), _p(base_se), _p(out), _p(stats))
     return out, stats, fault
+
+
+def replication(c: np.ndarray, placed_se: np.ndarray, P: int, Nb: int, Nr: int, M: int = 1):
+    """O13 for one instance: micro-step loads int32 [E], placement with final base slots [S] ->
+    slot_expert [S] with the redundant slots filled by Stage 3, fault."""
+    c, placed_se = _i32(c), _i32(placed_se)
+    se = np.full(P * (Nb + Nr), -1, dtype=np.int32)
+    fault = lib().oracle_replication(c.shape[0], P, Nb, Nr, M, _p(c), _p(placed_se), _p(se))
+    return se, fault

@@ -38,7 +38,7 @@ ACT_FP32 = 1
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
-           "foremoe_swap_relocation",
+           "foremoe_swap_relocation", "foremoe_replication",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
 
@@ -114,6 +114,7 @@ def lib() -> C.CDLL:
         l.foremoe_source_ids.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_local_placement.argtypes = [sp, i32, vp, vp, vp, vp]
         l.foremoe_traffic.argtypes = [sp, i32, vp, vp, vp]
+        l.foremoe_replication.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_swap_relocation.argtypes = [sp, i32, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp]
         l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
@@ -263,6 +264,13 @@ def swap_relocation(shape: Shape, M: int, win: int, max_rounds: int, a: int, b: 
         C.byref(shape.c()), M, win, max_rounds, a, b, _dev(hist_v, torch.int32),
         _dev(base_slot_expert, torch.int32), _dev(slot_expert_mb, torch.int32),
         _dev(rounds, torch.int32), _dev(dev_status, torch.int32), _stream()))
+
+
+def replication(shape: Shape, M: int, hist, placed_slot_expert_mb, slot_expert_mb, dev_status=None) -> None:
+    """(f.2) Stage 3 alone on per-micro-step placements with final base slots (may run in place)."""
+    _check("foremoe_replication", lib().foremoe_replication(
+        C.byref(shape.c()), M, _dev(hist, torch.int32), _dev(placed_slot_expert_mb, torch.int32),
+        _dev(slot_expert_mb, torch.int32), _dev(dev_status, torch.int32), _stream()))
 
 
 def virtual_shape(shape: Shape, M: int) -> Shape:

@@ -19,13 +19,6 @@ namespace foremoe {
 
 namespace {
 
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
-
 // two fp32 -> packed bf16x2, round to nearest even (lo in bits 0..15)
 __device__ __forceinline__ int pack_bf16x2(float lo, float hi) {
   int r;

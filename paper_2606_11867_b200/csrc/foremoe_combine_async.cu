@@ -9,13 +9,6 @@
 
 namespace foremoe {
 
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
-
 // smem: data [D][K][threads] int4, then per warp [D][32] int32 rows and [D][32] float weights
 template <bool kBf16, int K_T, int D>
 __global__ void __launch_bounds__(512)

@@ -46,7 +46,8 @@ __device__ __forceinline__ int argmin_rank(const PlaceSmem &s, int r0, int R, in
   return best == ~0ull ? -1 : (int)(best & 0xffffffffu);
 }
 
-// mode 0: base placement from step totals (no replication); mode 1: Alg. 3 Stages 2-3.
+// mode 0: base placement from step totals (no replication); mode 1: Alg. 3 Stages 2-3;
+// mode 2: Stage 3 alone on a per-instance placement whose base slots are final (its redundant slots are not read).
 __global__ void __launch_bounds__(kPlaceThreads)
 k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restrict__ hist,
         const int32_t *__restrict__ base_se, int L, int E, int P, int Nb, int Nr, int M,
@@ -85,16 +86,21 @@ k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restri
   for (int r = tid; r < P; r += nt) { s.RL[r] = 0; s.nb[r] = 0; s.nr[r] = 0; }
   for (int m = tid; m < M; m += nt) s.cntm[m] = 0;
   __syncthreads();
-  if (mode == 1) {
+  if (mode >= 1) {
     // machine of e = machine of its lowest-indexed slot in the base placement
+    const int32_t *bse = base_se + (size_t)(mode == 2 ? prob : l) * S;
     for (int j = tid; j < S; j += nt) {
-      const int e = base_se[(size_t)l * S + j];
+      if (mode == 2 && j % Ns >= Nb) continue;
+      const int e = bse[j];
       if (e < -1 || e >= E) fault |= FOREMOE_FAULT_SLOT_EXPERT;
-      else if (e >= 0) atomicMin(&s.first[e], j);
+      else if (e >= 0) {
+        atomicMin(&s.first[e], j);
+        if (mode == 2) atomicAdd(&s.copies[e], 1);       // must end up exactly 1: once in the base slots
+      }
     }
     __syncthreads();
     for (int e = tid; e < E; e += nt) {
-      if (s.first[e] == INT_MAX) { fault |= FOREMOE_FAULT_SLOT_EXPERT; continue; }
+      if (s.first[e] == INT_MAX || (mode == 2 && s.copies[e] != 1)) { fault |= FOREMOE_FAULT_SLOT_EXPERT; continue; }
       s.mach[e] = (s.first[e] / Ns) / R;
       atomicAdd(&s.cntm[s.mach[e]], 1);
     }
@@ -130,9 +136,10 @@ k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restri
     for (int a = 0; a < E; a++) {
       const int e = s.order[a];
       if (s.mach[e] != m) continue;
-      const int best = argmin_rank(s, r0, R, lane, [&](int r) { return s.nb[r] < Nb; });
+      // mode 2: the expert keeps the base slot it was given
+      const int best = mode == 2 ? s.first[e] / Ns : argmin_rank(s, r0, R, lane, [&](int r) { return s.nb[r] < Nb; });
       if (lane == 0) {
-        const int j = best * Ns + s.nb[best];
+        const int j = mode == 2 ? s.first[e] : best * Ns + s.nb[best];
         s.out[j] = e;
         s.first[e] = j;                  // head of e's host list (ascending slot index)
         s.nb[best] += 1;
@@ -208,7 +215,7 @@ static int launch_place(int mode, const Dims &d, int M, const int64_t *step_hist
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute(k_place, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return FOREMOE_ERR_CUDA;
-  const int n_prob = mode == 0 ? d.L : d.n_inst;
+  const int n_prob = mode == 0 ? d.L : d.n_inst;   // modes 1, 2: one CTA per (micro-step, layer)
   k_place<<<n_prob, kPlaceThreads, smem, st>>>(mode, step_hist, hist, base_se, d.L, d.E, d.P, d.Nb,
                                                d.Nr, M, out_se, dev_status);
   return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
@@ -237,5 +244,17 @@ extern "C" __attribute__((visibility("default"))) int foremoe_microstep_placemen
   if (!hist || !base_slot_expert || !slot_expert_mb || M <= 0 || d.P % M != 0)
     return FOREMOE_ERR_INVALID_ARG;
   return launch_place(1, d, M, nullptr, hist, base_slot_expert, slot_expert_mb, dev_status,
+                      (cudaStream_t)stream);
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_replication(
+    const foremoe_shape_t *shape, int32_t M, const int32_t *hist, const int32_t *placed_slot_expert_mb,
+    int32_t *slot_expert_mb, int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!hist || !placed_slot_expert_mb || !slot_expert_mb || M <= 0 || d.P % M != 0)
+    return FOREMOE_ERR_INVALID_ARG;
+  return launch_place(2, d, M, nullptr, hist, placed_slot_expert_mb, slot_expert_mb, dev_status,
                       (cudaStream_t)stream);
 }

@@ -92,3 +92,26 @@ class LocalStepPlan(StepPlan):
         fm.local_placement(self.real_shape, self.M, self.real_slot_expert, self.slot_expert, self.status)
         super().plan(quota_in)
         fm.traffic(self.real_shape, self.M, self.quota, self.traffic)
+
+
+class PlannerStepPlan(StepPlan):
+    """All four planner stages on the device: Stage 1 (rank-level LPT from the step totals), Alg. 3
+    Stages 2-3 per (micro-step, layer) over ``M`` machines, Stage 4 on the per-micro-step placements
+    (PAPER.md:282-407, :787-846).  ``shape`` is the plain shape; the plan's own shape carries
+    ``placement_mb_stride = L * S``."""
+
+    def __init__(self, shape: fm.Shape, M: int, ids, w, mb_off):
+        import dataclasses
+        dev = ids.device
+        self.M = M
+        self.base_shape = shape
+        self.base_slot_expert = torch.empty((shape.L, shape.S), dtype=torch.int32, device=dev)
+        se_mb = torch.empty((shape.n_mb, shape.L, shape.S), dtype=torch.int32, device=dev)
+        super().__init__(dataclasses.replace(shape, placement_mb_stride=shape.L * shape.S), ids, w, mb_off, se_mb)
+
+    def plan(self, quota_in: Optional[torch.Tensor] = None) -> None:
+        self.load_hist()
+        fm.base_placement(self.base_shape, self.step_hist, self.base_slot_expert, self.status)
+        fm.microstep_placement(self.base_shape, self.M, self.hist, self.base_slot_expert, self.slot_expert,
+                               self.status)
+        self.assign(quota_in)

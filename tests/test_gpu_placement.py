@@ -204,3 +204,41 @@ def test_swap_then_stage4_on_config_trace(cuda_device):
         for l in range(cfg.L):
             q, rl, so, _, f = orc.quota(hist[i, l], out[i, l], cfg.P, cfg.Ns)
             assert f == 0 and (sp1.quota[i, l].cpu().numpy() == q).all()
+
+
+# ------------------------------------------------------------------ Stage 3 alone (O13) after the swaps
+@pytest.mark.parametrize("seed", range(5))
+def test_replication_after_swaps(cuda_device, seed):
+    rng = np.random.default_rng(90 + seed)
+    P, M, Nb, Nr = [(4, 1, 4, 1), (8, 2, 16, 2), (64, 8, 4, 1), (32, 1, 16, 4), (6, 3, 5, 2)][seed]
+    E, L, n_mb, Ns = P * Nb, 2, 4, Nb + Nr
+    shape = fm.Shape(L=L, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=n_mb, H=8, act_dtype=fm.ACT_FP32)
+    hist = (rng.integers(0, 400, size=(n_mb, L, E)) * (rng.random((n_mb, L, E)) < 0.8)).astype(np.int32)
+    hist[3] = 0
+    base = np.full((L, P * Ns), -1, dtype=np.int32)
+    for l in range(L):
+        perm = rng.permutation(E)
+        for r in range(P):
+            base[l, r * Ns:r * Ns + Nb] = perm[r * Nb:(r + 1) * Nb]
+    swapped, nr, fault = _swap_gpu(shape, 1, 3, 16, 1, 0, hist, base)
+    assert fault == 0
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    buf = torch.as_tensor(swapped).to(dev)
+    buf.view(n_mb, L, P, Ns)[..., Nb:] = -9                     # redundant slots of the input are not read
+    fm.replication(shape, M, torch.as_tensor(hist).to(dev), buf, buf, st)        # in place
+    torch.cuda.synchronize()
+    got = buf.cpu().numpy()
+    assert int(st.item()) == 0
+    for i in range(n_mb):
+        for l in range(L):
+            ref, f = orc.replication(hist[i, l], swapped[i, l], P, Nb, Nr, M)
+            assert f == 0 and (got[i, l] == ref).all(), ("replication", i, l)
+    # fault: an expert twice in the base slots of one instance -> that instance is all -1, others fine
+    bad = torch.as_tensor(swapped).to(dev)
+    bad[1, 0, 0] = bad[1, 0, 1]
+    out = torch.empty_like(bad)
+    fm.replication(shape, M, torch.as_tensor(hist).to(dev), bad, out, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) & fm.FAULT_SLOT_EXPERT
+    assert (out[1, 0] == -1).all() and (out[0, 0].cpu().numpy() == got[0, 0]).all()

@@ -154,3 +154,41 @@ def test_faults():
     assert f & orc.FAULT_ID_RANGE
     _, f = orc.base_placement(np.array([1, 2, 3]), 1, 2, 0)       # more experts than base slots
     assert f & orc.FAULT_SLOT_EXPERT
+
+
+# ------------------------------------------------------------------ O13: replication alone
+@pytest.mark.parametrize("seed", range(8))
+def test_replication_only_composes_with_stage2(seed):
+    """O13 on O8's own Stage-2 result (O8 run with N_r = 0, padded) must reproduce O8 in full; and the
+    first replica of every machine is the heaviest local expert on the least-loaded other rank."""
+    rng = np.random.default_rng(400 + seed)
+    P = int(rng.choice([2, 4, 6, 8]))
+    Nb, Nr = int(rng.integers(1, 5)), int(rng.integers(1, 4))
+    E, Ns = P * Nb, Nb + Nr
+    tot = rng.integers(1, 1000, size=E)
+    c = (rng.integers(0, 300, size=E) * rng.integers(0, 2, size=E)).astype(np.int32)
+    for M in [m for m in (1, 2) if P % m == 0]:
+        base, f = orc.base_placement(tot, P, Nb, Nr)
+        full, f1 = orc.microstep_placement(c, base, P, Nb, Nr, M)
+        base0, _ = orc.base_placement(tot, P, Nb, 0)
+        st2, f2 = orc.microstep_placement(c, base0, P, Nb, 0, M)           # Stage 2 only
+        padded = np.full(P * Ns, -1, dtype=np.int32)
+        padded.reshape(P, Ns)[:, :Nb] = st2.reshape(P, Nb)
+        padded.reshape(P, Ns)[:, Nb:] = rng.integers(-1, E, size=(P, Nr))  # garbage: must be ignored
+        rep, f3 = orc.replication(c, padded, P, Nb, Nr, M)
+        assert f == 0 and f1 == 0 and f2 == 0 and f3 == 0
+        assert (rep == full).all()
+        _structure_ok(rep, E, P, Nb, Nr, c=c)
+
+
+def test_replication_only_on_swapped_placement_and_faults():
+    c = np.array([9, 8, 1, 2], dtype=np.int32)
+    swapped, st, f = orc.swap_relocation(c, np.array([0, 1, -1, 2, 3, -1]), 2, 2, 1, 1, 2, 8)
+    assert f == 0 and swapped.tolist() == [3, 1, -1, 2, 0, -1]
+    rep, f = orc.replication(c, swapped, 2, 2, 1, 1)
+    # rank loads 10 | 10; heaviest per copy e0 (9) -> least-loaded rank not hosting it = rank 0;
+    # then e1 (8 vs e0 4.5 per copy) -> rank 1
+    assert f == 0 and rep.tolist() == [3, 1, 0, 2, 0, 1]
+    bad = swapped.copy(); bad[0] = 1                                       # e1 twice, e3 missing
+    rep, f = orc.replication(c, bad, 2, 2, 1, 1)
+    assert f & orc.FAULT_SLOT_EXPERT and (rep == -1).all()

@@ -17,7 +17,6 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
                 int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
   constexpr int kF = kBf16 ? 8 : 4;
   const int K = K_T > 0 ? K_T : K_rt;
-  pdl_wait();
   pdl_launch_dependents();
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -66,7 +65,8 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
     cp_async_commit();
   };
 
-  fetch_meta(0);
+  fetch_meta(0);                           // inv / w / mb_off only: the plan's own arrays (see k_dispatch_rows)
+  pdl_wait();                              // expert_out is read and y written after the wait
   for (int n = 0; n < D - 1; n++) issue(n);
   for (int j = 0; j < n_my; j++) {
     issue(j + D - 1);

@@ -898,3 +898,80 @@ done:
   free(c); free(slot_of); free(RL); free(LT); free(RL2); free(LT2); free(heavy); free(light);
   return fault;
 }
+
+/* ==========================================================================================
+ * O14 oracle_base_placement_machines: Stage 1 in full, Alg. 1 for ONE layer.
+ *   lines 1-3   wbar_e = sum_s wbar_{s,e}; experts in descending wbar_e (ties ascending id);
+ *               ML[m] = MC[m] = 0;
+ *   lines 5-12  machine-level placement: for each expert in that order,
+ *                 Delta_{m,e} = sum_{s: machine(s) != m} wbar_{s,e}   (tokens reaching e from other machines)
+ *                 score(m,e)  = a * (ML[m] + wbar_e) + b * (MC[m] + Delta_{m,e})   (a ~ n1*K1, b ~ n2*K2)
+ *                 m* = argmin score over the machines that still have a free base slot (capacity
+ *                 R * N_b; ties lowest m); ML[m*] += wbar_e; MC[m*] += Delta_{m*,e};
+ *   lines 13-21 rank-level placement: inside each machine, its experts in descending wbar_e to the
+ *               least-loaded local rank with a free base slot (LPT; O7's loop, ties lowest rank).
+ * Only the machine of a source matters for Delta, so the input is wbar aggregated per source
+ * machine: tot_me[m][e] (readings 21, 33, 37).  With M = 1 this is O7.
+ * Pins (tests/test_oracle_placement.py): M = 1 equals O7; the greedy choices replayed step by
+ * step in Python from the output; b = 0 => machines balanced as LPT with capacity; a = 0 => every
+ * expert on a machine minimising accumulated inbound traffic; hand-worked vector; structure.
+ * ========================================================================================== */
+int oracle_base_placement_machines(int E, int P, int Nb, int Nr, int M, int64_t a, int64_t b,
+                                   const int64_t *tot_me /* [M][E] */, int32_t *slot_expert) {
+  const int Ns = Nb + Nr, S = P * Ns;
+  int fault = 0;
+  for (int j = 0; j < S; j++) slot_expert[j] = -1;
+  if (M <= 0 || P % M != 0 || a < 0 || b < 0) return ORACLE_BAD_ARG;
+  if ((int64_t)P * Nb < E) return FAULT_SLOT_EXPERT;
+  const int R = P / M;
+  int64_t *tot = (int64_t *)calloc((size_t)E, sizeof(int64_t));
+  int32_t *order = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *mach = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int64_t *ML = (int64_t *)calloc((size_t)M, sizeof(int64_t));
+  int64_t *MC = (int64_t *)calloc((size_t)M, sizeof(int64_t));
+  int32_t *cnt = (int32_t *)calloc((size_t)M, sizeof(int32_t));
+  int64_t *RL = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  int32_t *nb = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  if (!tot || !order || !mach || !ML || !MC || !cnt || !RL || !nb) { fault = ORACLE_NO_MEM; goto done; }
+  for (int e = 0; e < E; e++) {
+    order[e] = e;
+    for (int m = 0; m < M; m++) {
+      if (tot_me[(size_t)m * E + e] < 0) fault |= FAULT_ID_RANGE;
+      tot[e] += tot_me[(size_t)m * E + e];                                        /* line 1 */
+    }
+  }
+  if (fault) goto done;
+  for (int x = 1; x < E; x++) {                                                   /* line 2 */
+    int32_t e = order[x];
+    int y = x;
+    while (y > 0 && heavier(tot, e, order[y - 1])) { order[y] = order[y - 1]; y--; }
+    order[y] = e;
+  }
+  for (int x = 0; x < E; x++) {                                                   /* lines 5-12 */
+    const int e = order[x];
+    int best = -1;
+    int64_t best_score = 0;
+    for (int m = 0; m < M; m++) {
+      if (cnt[m] >= R * Nb) continue;
+      const int64_t delta = tot[e] - tot_me[(size_t)m * E + e];
+      const int64_t score = a * (ML[m] + tot[e]) + b * (MC[m] + delta);
+      if (best < 0 || score < best_score) { best = m; best_score = score; }
+    }
+    mach[e] = best;
+    cnt[best] += 1;
+    ML[best] += tot[e];
+    MC[best] += tot[e] - tot_me[(size_t)best * E + e];
+  }
+  for (int x = 0; x < E; x++) {                                                   /* lines 13-21 */
+    const int e = order[x], m = mach[e];
+    int best = -1;
+    for (int r = m * R; r < (m + 1) * R; r++)
+      if (nb[r] < Nb && (best < 0 || RL[r] < RL[best])) best = r;
+    slot_expert[best * Ns + nb[best]] = e;
+    nb[best] += 1;
+    RL[best] += tot[e];
+  }
+done:
+  free(tot); free(order); free(mach); free(ML); free(MC); free(cnt); free(RL); free(nb);
+  return fault;
+}

@@ -232,3 +232,13 @@ def replication(c: np.ndarray, placed_se: np.ndarray, P: int, Nb: int, Nr: int, 
     se = np.full(P * (Nb + Nr), -1, dtype=np.int32)
     fault = lib().oracle_replication(c.shape[0], P, Nb, Nr, M, _p(c), _p(placed_se), _p(se))
     return se, fault
+
+
+def base_placement_machines(tot_me: np.ndarray, P: int, Nb: int, Nr: int, M: int, a: int = 1, b: int = 0):
+    """O14 for one layer: step totals per source machine int64 [M,E] -> slot_expert int32 [S], fault."""
+    tot_me = np.ascontiguousarray(tot_me, dtype=np.int64).reshape(M, -1)
+    se = np.full(P * (Nb + Nr), -1, dtype=np.int32)
+    f = lib().oracle_base_placement_machines
+    f.argtypes = [C.c_int] * 5 + [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
+    fault = f(tot_me.shape[1], P, Nb, Nr, M, a, b, _p(tot_me), _p(se))
+    return se, fault

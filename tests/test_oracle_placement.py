@@ -192,3 +192,72 @@ def test_replication_only_on_swapped_placement_and_faults():
     bad = swapped.copy(); bad[0] = 1                                       # e1 twice, e3 missing
     rep, f = orc.replication(c, bad, 2, 2, 1, 1)
     assert f & orc.FAULT_SLOT_EXPERT and (rep == -1).all()
+
+
+# ------------------------------------------------------------------ O14: Alg. 1 in full (machine level + rank level)
+def _replay_alg1(tot_me, se, P, Nb, Nr, M, a, b):
+    """Re-derive every greedy choice of Alg. 1 from the OUTPUT: at its turn each expert sits on a machine
+    of minimal score among those with a free base slot (lowest m on ties), and inside the machine on the
+    least-loaded rank with a free base slot."""
+    Ns, R = Nb + Nr, P // M
+    E = tot_me.shape[1]
+    tot = tot_me.sum(0)
+    where = {int(se[j]): j // Ns for j in range(len(se)) if se[j] >= 0}
+    assert sorted(where) == list(range(E))
+    order = sorted(range(E), key=lambda e: (-int(tot[e]), e))
+    ML, MC, cnt = np.zeros(M, np.int64), np.zeros(M, np.int64), np.zeros(M, np.int64)
+    for e in order:
+        m_out = where[e] // R
+        scores = {m: a * (ML[m] + tot[e]) + b * (MC[m] + tot[e] - tot_me[m, e]) for m in range(M) if cnt[m] < R * Nb}
+        m_best = min(scores, key=lambda m: (scores[m], m))
+        assert m_out == m_best, (e, m_out, m_best)
+        ML[m_out] += tot[e]; MC[m_out] += tot[e] - tot_me[m_out, e]; cnt[m_out] += 1
+    RL, nb = np.zeros(P, np.int64), np.zeros(P, np.int64)
+    for e in order:
+        r = where[e]
+        cand = [q for q in range((r // R) * R, (r // R + 1) * R) if nb[q] < Nb]
+        assert r == min(cand, key=lambda q: (RL[q], q))
+        RL[r] += tot[e]; nb[r] += 1
+    return ML, MC
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_alg1_machines_replay(seed):
+    rng = np.random.default_rng(500 + seed)
+    P, M = [(4, 2), (8, 2), (8, 4), (6, 3), (16, 4), (8, 8)][seed % 6]
+    Nb, Nr = int(rng.integers(1, 5)), int(rng.integers(0, 3))
+    a, b = [(1, 0), (0, 1), (1, 1), (3, 2)][seed % 4]
+    E = P * Nb
+    tot_me = (rng.integers(0, 1000, size=(M, E)) * (rng.random((M, E)) < 0.7)).astype(np.int64)
+    se, f = orc.base_placement_machines(tot_me, P, Nb, Nr, M, a, b)
+    assert f == 0
+    _structure_ok(se, E, P, Nb, Nr, base_only=True)
+    _replay_alg1(tot_me, se, P, Nb, Nr, M, a, b)
+
+
+def test_alg1_special_cases():
+    rng = np.random.default_rng(7)
+    # M = 1 is O7
+    tot = rng.integers(0, 500, size=24)
+    se1, f1 = orc.base_placement_machines(tot.reshape(1, -1), 8, 3, 1, 1, 5, 9)
+    se7, f7 = orc.base_placement(tot, 8, 3, 1)
+    assert f1 == 0 and f7 == 0 and (se1 == se7).all()
+    # a = 0: only inbound traffic counts -> an expert whose tokens all come from one machine lands there
+    # (Delta = 0 on that machine, > 0 elsewhere) as long as it has room
+    P, M, Nb = 4, 2, 2
+    tot_me = np.array([[9, 0, 7, 0, 5, 0, 3, 0], [0, 8, 0, 6, 0, 4, 0, 2]], dtype=np.int64)
+    se, f = orc.base_placement_machines(tot_me, P, Nb, 0, M, 0, 1)
+    assert f == 0
+    mach = {int(e): (j // Nb) // 2 for j, e in enumerate(se)}
+    assert all(mach[e] == e % 2 for e in range(8))
+    # hand-worked, a = b = 1, M = 2 machines of 1 rank, N_b = 2: loads (m0, m1): e0 (6,0) e1 (1,4) e2 (0,4) e3 (3,0)
+    # order e0(6) e1(5) e2(4) e3(3); e0: score m0 = 6+0, m1 = 6+6 -> m0 (ML 6,0; MC 0,0)
+    # e1: m0 = (6+5)+(0+4) = 15, m1 = 5+1 = 6 -> m1 (ML 6,5; MC 0,1); e2: m0 = 10+4 = 14, m1 = 9+1+0 = 10 -> m1 (full)
+    # e3: only m0 has room -> m0.  ranks = machines: rank0 [e0, e3], rank1 [e1, e2]
+    tot_me = np.array([[6, 1, 0, 3], [0, 4, 4, 0]], dtype=np.int64)
+    se, f = orc.base_placement_machines(tot_me, 2, 2, 1, 2, 1, 1)
+    assert f == 0 and se.tolist() == [0, 3, -1, 1, 2, -1]
+    # faults
+    bad = tot_me.copy(); bad[0, 0] = -1
+    se, f = orc.base_placement_machines(bad, 2, 2, 1, 2, 1, 1)
+    assert f & orc.FAULT_ID_RANGE and (se == -1).all()

@@ -158,6 +158,21 @@ int foremoe_base_placement(const foremoe_shape_t *shape, const int64_t *step_his
                            int32_t *slot_expert, int32_t *dev_status, void *stream);
 
 /*
+ * (NEXT) Stage 1 in full -- Alg. 1 with M machines of
+ * R = P / M ranks: experts in descending step load; machine-level greedy (lines 5-12)
+ *     score(m, e) = a * (ML[m] + w_e) + b * (MC[m] + Delta_{m,e}),  Delta_{m,e} = w_e - w_{m,e}
+ * over the machines that still have a free base slot (capacity R * N_b; ties lowest m), with the
+ * caller-supplied integers a ~ n1*K1, b ~ n2*K2 in [0, 2^20] (readings 33, 37); then the
+ * rank-level LPT of foremoe_base_placement inside every machine (lines 13-21).
+ *   step_hist_v [L][E*M] int64: step load of expert e from the sources of machine m at e*M + m
+ *               (foremoe_load_hist's step_hist on foremoe_source_ids' output; M = 1: step_hist).
+ *   slot_expert [L][S] out.  M <= 64.  Faults: ID_RANGE (negative load): that layer is all -1.
+ */
+int foremoe_base_placement_machines(const foremoe_shape_t *shape, int32_t M, int64_t a, int64_t b,
+                                    const int64_t *step_hist_v, int32_t *slot_expert,
+                                    int32_t *dev_status, void *stream);
+
+/*
  * (NEXT) Per-micro-step placement A^{(i)}: Alg. 3 Stages 2-3
  * for every (micro-step, layer) instance.  Machines are M groups of
  * R = P / M consecutive ranks; an expert is local to the machine of its base rank.

@@ -37,7 +37,7 @@ ACT_FP32 = 1
 
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
-           "foremoe_base_placement", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
+           "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
            "foremoe_swap_relocation", "foremoe_replication",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
@@ -111,6 +111,7 @@ def lib() -> C.CDLL:
         l.foremoe_combine_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_dispatch_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         l.foremoe_base_placement.argtypes = [sp, vp, vp, vp, vp]
+        l.foremoe_base_placement_machines.argtypes = [sp, i32, C.c_int64, C.c_int64, vp, vp, vp, vp]
         l.foremoe_source_ids.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_local_placement.argtypes = [sp, i32, vp, vp, vp, vp]
         l.foremoe_traffic.argtypes = [sp, i32, vp, vp, vp]
@@ -226,6 +227,14 @@ def base_placement(shape: Shape, step_hist, slot_expert, dev_status=None) -> Non
     """(f.4) Stage-1 rank-level LPT: step_hist int64 [L,E] -> slot_expert int32 [L,S]."""
     _check("foremoe_base_placement", lib().foremoe_base_placement(
         C.byref(shape.c()), _dev(step_hist, torch.int64), _dev(slot_expert, torch.int32),
+        _dev(dev_status, torch.int32), _stream()))
+
+
+def base_placement_machines(shape: Shape, M: int, a: int, b: int, step_hist_v, slot_expert,
+                            dev_status=None) -> None:
+    """(f.4) Alg. 1 in full: step_hist_v int64 [L,E*M] -> slot_expert int32 [L,S]."""
+    _check("foremoe_base_placement_machines", lib().foremoe_base_placement_machines(
+        C.byref(shape.c()), M, a, b, _dev(step_hist_v, torch.int64), _dev(slot_expert, torch.int32),
         _dev(dev_status, torch.int32), _stream()))
 
 

@@ -50,8 +50,8 @@ __device__ __forceinline__ int argmin_rank(const PlaceSmem &s, int r0, int R, in
 // mode 2: Stage 3 alone on a per-instance placement whose base slots are final (its redundant slots are not read).
 __global__ void __launch_bounds__(kPlaceThreads)
 k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restrict__ hist,
-        const int32_t *__restrict__ base_se, int L, int E, int P, int Nb, int Nr, int M,
-        int32_t *__restrict__ out_se, int32_t *dev_status) {
+        const int32_t *__restrict__ base_se, int L, int E, int P, int Nb, int Nr, int M, long long a,
+        long long b, int32_t *__restrict__ out_se, int32_t *dev_status) {
   extern __shared__ int32_t sm[];
   const int Ns = Nb + Nr, S = P * Ns, R = P / M;
   const int prob = blockIdx.x;                 // layer (mode 0) or instance i * L + l (mode 1)
@@ -74,7 +74,16 @@ k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restri
 
   int fault = 0;
   for (int e = tid; e < E; e += nt) {
-    long long v = mode == 0 ? (long long)step_hist[(size_t)prob * E + e] : (long long)hist[(size_t)prob * E + e];
+    long long v = 0;
+    if (mode == 0) {               // step totals, per source machine at e*M + m (M = 1: the plain step_hist)
+      for (int m = 0; m < M; m++) {
+        const long long t = step_hist[((size_t)prob * E + e) * M + m];
+        if (t < 0) fault |= FOREMOE_FAULT_ID_RANGE;
+        v += t;
+      }
+    } else {
+      v = hist[(size_t)prob * E + e];
+    }
     if (v < 0 || v > INT_MAX) { fault |= FOREMOE_FAULT_ID_RANGE; v = 0; }
     s.c[e] = (int)v;
     s.mach[e] = mode == 0 ? 0 : -1;
@@ -129,6 +138,43 @@ k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restri
     s.order[pos] = e;
   }
   __syncthreads();
+
+  if (mode == 0 && M > 1) {
+    // Alg. 1 lines 5-12: machine-level greedy, experts in order, one lane per machine (M <= 64):
+    // score(m,e) = a*(ML[m] + w_e) + b*(MC[m] + Delta_{m,e}), Delta = w_e - w_{m,e}; machines with a
+    // free base slot only (capacity R*Nb); ties to the lowest machine
+    __shared__ long long ML[64], MC[64];
+    if (warp == 0) {
+      for (int m = lane; m < M; m += 32) { ML[m] = 0; MC[m] = 0; }
+      __syncwarp();
+      for (int x = 0; x < E; x++) {
+        const int e = s.order[x];
+        const long long we = s.c[e];
+        long long best = LLONG_MAX;
+        int bm = INT_MAX;
+        for (int m = lane; m < M; m += 32) {
+          if (s.cntm[m] >= R * Nb) continue;
+          const long long wme = step_hist[((size_t)prob * E + e) * M + m];
+          const long long sc = a * (ML[m] + we) + b * (MC[m] + we - wme);
+          if (sc < best) { best = sc; bm = m; }          // ascending m per lane: strict < keeps the lowest
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+          const long long ob = __shfl_xor_sync(kFull, best, o);
+          const int om = __shfl_xor_sync(kFull, bm, o);
+          if (ob < best || (ob == best && om < bm)) { best = ob; bm = om; }
+        }
+        if (lane == 0) {
+          s.mach[e] = bm;
+          s.cntm[bm] += 1;
+          ML[bm] += we;
+          MC[bm] += we - step_hist[((size_t)prob * E + e) * M + bm];
+        }
+        __syncwarp();
+      }
+    }
+    __syncthreads();
+  }
 
   for (int m = warp; m < M; m += nw) {
     const int r0 = m * R;
@@ -209,7 +255,8 @@ k_place(int mode, const int64_t *__restrict__ step_hist, const int32_t *__restri
 }
 
 static int launch_place(int mode, const Dims &d, int M, const int64_t *step_hist, const int32_t *hist,
-                        const int32_t *base_se, int32_t *out_se, int32_t *dev_status, cudaStream_t st) {
+                        const int32_t *base_se, int32_t *out_se, int32_t *dev_status, cudaStream_t st,
+                        long long a = 1, long long b = 0) {
   const size_t smem = sizeof(int32_t) * ((size_t)6 * d.E + (size_t)2 * d.S + (size_t)3 * d.P + M);
   if (smem > 200 * 1024) return FOREMOE_ERR_INVALID_ARG;
   if (smem > 48 * 1024 &&
@@ -217,7 +264,7 @@ static int launch_place(int mode, const Dims &d, int M, const int64_t *step_hist
     return FOREMOE_ERR_CUDA;
   const int n_prob = mode == 0 ? d.L : d.n_inst;   // modes 1, 2: one CTA per (micro-step, layer)
   k_place<<<n_prob, kPlaceThreads, smem, st>>>(mode, step_hist, hist, base_se, d.L, d.E, d.P, d.Nb,
-                                               d.Nr, M, out_se, dev_status);
+                                               d.Nr, M, a, b, out_se, dev_status);
   return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
@@ -257,4 +304,17 @@ extern "C" __attribute__((visibility("default"))) int foremoe_replication(
     return FOREMOE_ERR_INVALID_ARG;
   return launch_place(2, d, M, nullptr, hist, placed_slot_expert_mb, slot_expert_mb, dev_status,
                       (cudaStream_t)stream);
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_base_placement_machines(
+    const foremoe_shape_t *shape, int32_t M, int64_t a, int64_t b, const int64_t *step_hist_v,
+    int32_t *slot_expert, int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!step_hist_v || !slot_expert || M <= 0 || M > 64 || d.P % M != 0 || a < 0 || b < 0 ||
+      a > (1 << 20) || b > (1 << 20))
+    return FOREMOE_ERR_INVALID_ARG;
+  return launch_place(0, d, M, step_hist_v, nullptr, nullptr, slot_expert, dev_status, (cudaStream_t)stream,
+                      (long long)a, (long long)b);
 }

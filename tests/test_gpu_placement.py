@@ -242,3 +242,40 @@ def test_replication_after_swaps(cuda_device, seed):
     torch.cuda.synchronize()
     assert int(st.item()) & fm.FAULT_SLOT_EXPERT
     assert (out[1, 0] == -1).all() and (out[0, 0].cpu().numpy() == got[0, 0]).all()
+
+
+# ------------------------------------------------------------------ Alg. 1 in full (O14)
+@pytest.mark.parametrize("seed", range(6))
+def test_base_placement_machines(cuda_device, seed):
+    rng = np.random.default_rng(120 + seed)
+    P, M, Nb, Nr = [(4, 2, 2, 1), (8, 2, 16, 2), (64, 8, 4, 1), (32, 4, 16, 4), (6, 3, 5, 0), (64, 64, 4, 1)][seed]
+    a, b = [(1, 1), (1, 0), (3, 2), (0, 1), (1, 5), (2, 1)][seed]
+    E, L = P * Nb, 4
+    shape = fm.Shape(L=L, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=1, H=8, act_dtype=fm.ACT_FP32)
+    tot = (rng.integers(0, 5000, size=(L, E, M)) * (rng.random((L, E, M)) < 0.7)).astype(np.int64)
+    tot[1] = 11                                       # all equal: ties only
+    tot[2, :, 1:] = 0                                 # every token from machine 0
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    out = torch.full((L, shape.S), -7, dtype=torch.int32, device=dev)
+    fm.base_placement_machines(shape, M, a, b, torch.as_tensor(tot.reshape(L, E * M)).to(dev), out, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) == 0
+    got = out.cpu().numpy()
+    for l in range(L):
+        ref, f = orc.base_placement_machines(tot[l].T.copy(), P, Nb, Nr, M, a, b)
+        assert f == 0 and (got[l] == ref).all(), ("alg1", l)
+    # M = 1 through the same entry equals foremoe_base_placement
+    out1 = torch.empty_like(out)
+    out7 = torch.empty_like(out)
+    step = torch.as_tensor(tot.sum(-1)).to(dev)
+    fm.base_placement_machines(shape, 1, 1, 0, step, out1, st)
+    fm.base_placement(shape, step, out7, st)
+    torch.cuda.synchronize()
+    assert torch.equal(out1, out7)
+    neg = tot.reshape(L, E * M).copy(); neg[3, 5] = -2
+    fm.base_placement_machines(shape, M, a, b, torch.as_tensor(neg).to(dev), out, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) & fm.FAULT_ID_RANGE and (out[3] == -1).all() and (out[0].cpu().numpy() == got[0]).all()
+    with pytest.raises(fm.ForeMoEError):
+        fm.base_placement_machines(shape, M, -1, b, torch.as_tensor(neg).to(dev), out, st)

@@ -297,6 +297,34 @@ class Workload:
         self.plan.plan()
         self.graph.replay()
 
+    def setup_streams(self, n: int):
+        """Independent instances on `n` streams (each with its own perm / buf / y / gradient buffers):
+        the library is re-entrant per stream and (micro-step, layer) instances are independent
+        (PAPER.md:144, :417), so the ramp and drain of one launch overlap another stream's kernel."""
+        self.streams = [torch.cuda.Stream() for _ in range(n)]
+        names = ["perm", "buf", "y"] + (["d_buf", "dx"] if self.stage == "update" else [])
+        self.stream_bufs = [{k: (getattr(self, k) if j == 0 else torch.empty_like(getattr(self, k))) for k in names}
+                            for j in range(n)]
+
+    def step_streams(self):
+        main = torch.cuda.current_stream()
+        self.plan.plan()
+        ready = torch.cuda.Event()
+        ready.record(main)
+        for j, st in enumerate(self.streams):
+            st.wait_event(ready)
+            with torch.cuda.stream(st):
+                for k, v in self.stream_bufs[j].items():
+                    setattr(self, k, v)
+                for (l, i) in self.instances[j::len(self.streams)]:
+                    self.instance(l, i)
+        for k, v in self.stream_bufs[0].items():
+            setattr(self, k, v)
+        for st in self.streams:
+            done = torch.cuda.Event()
+            done.record(st)
+            main.wait_event(done)
+
     def release(self):
         self.plan = self.x = self.buf = self.y = self.perm = None
         self.dy = self.d_buf = self.dx = self.dw = None
@@ -375,13 +403,15 @@ def run_ours(args, cfg) -> None:
 
     if args.graph:
         wl.capture_graph()
+    if args.streams > 1:
+        wl.setup_streams(args.streams)
     for _ in range(args.warmup):
-        wl.step()
+        wl.step_streams() if args.streams > 1 else wl.step()
     torch.cuda.synchronize()
     assert wl.plan.faults() == 0
     probes = {"plan": [], "dispatch": [], "combine": [], "combine_bwd": [], "dispatch_bwd": []}
-    if args.graph:
-        # per-kernel probes cannot sit inside a graph: take them in one extra, untimed step
+    if args.graph or args.streams > 1:
+        # per-kernel probes cannot sit inside a graph / between concurrent streams: one extra, untimed step
         wl.step(probes, args.probe_stride)
         torch.cuda.synchronize()
     multi.barrier(dev); torch.cuda.synchronize()
@@ -391,6 +421,8 @@ def run_ours(args, cfg) -> None:
         for _ in range(args.steps):
             if args.graph:
                 wl.step_graph()
+            elif args.streams > 1:
+                wl.step_streams()
             else:
                 wl.step(probes, args.probe_stride)
         e1.record()
@@ -452,7 +484,9 @@ def run_ours(args, cfg) -> None:
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
                    "stage": args.stage, "machines": args.machines, "planner": args.planner, "bytes_per_routed_token": total_bpt,
-                   "launch": "cuda graph replay of the instance loop" if args.graph else "stream launches"},
+                   "launch": ("cuda graph replay of the instance loop" if args.graph else
+                              f"{args.streams} streams, independent instances interleaved" if args.streams > 1
+                              else "stream launches")},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
     if not args.no_e2e and not upd and not args.machines and args.planner != "full":
@@ -496,6 +530,8 @@ def main() -> None:
                     help="stage4 = the headline path (step-level placement is an input, Stage 4 on the GPU); "
                          "full = Stage 1 + Alg. 3 Stages 2-3 + Stage 4 all on the GPU inside the timed step "
                          "(--machines M then restricts relocation / replication to machines of P/M ranks)")
+    ap.add_argument("--streams", type=int, default=1,
+                    help="> 1: interleave the independent instances over that many CUDA streams")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

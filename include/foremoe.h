@@ -335,6 +335,20 @@ int foremoe_step_host(const foremoe_shape_t *shape, const int32_t *ids_h, const 
                       int32_t *quota_h, int32_t *rank_load_h, int32_t *slot_off_h, float *y_h,
                       void *arena, size_t arena_bytes, int32_t *status_h, void *stream);
 
+/*
+ * Sweeps only (paper_2606_11867_b200/tune.py; profiles/r01_sweeps.md, r01_hist.md, r01_backward.md):
+ * process-wide launch parameters of the data-path kernels and the histogram variant.  They select
+ * among kernels that compute bit-identical results; not part of the product contract, not
+ * thread-safe, defaults are restored by passing the default values again.
+ *   foremoe_debug_set_tuning: key = index into {dispatch_impl, dispatch_u, dispatch_cta_per_sm,
+ *     dispatch_stages, dispatch_warps, combine_impl, combine_u, combine_cta_per_sm, combine_depth,
+ *     combine_threads, pdl, bwd_depth, bwd_cta_per_sm}; unknown keys are ignored.
+ *   foremoe_debug_set_hist_variant: 0 = 4-byte loads, 1 = warp-aggregated (match.any), 2 = 16-byte
+ *     loads (default).
+ */
+void foremoe_debug_set_tuning(int key, int value);
+void foremoe_debug_set_hist_variant(int variant);
+
 #ifdef __cplusplus
 }
 #endif

@@ -29,6 +29,30 @@ def test_header_symbols_exported(libpath):
     assert lib.foremoe_version() >= 100
 
 
+def test_exported_symbols_are_exactly_the_declared_ones(libpath):
+    """Nothing is exported that include/foremoe.h does not declare (nm -D), debug setters included."""
+    import subprocess
+    hdr = open(os.path.join(ROOT, "include", "foremoe.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(?:int|void)\s+(foremoe_\w+)\s*\(", hdr))
+    out = subprocess.run(["nm", "-D", "--defined-only", libpath], capture_output=True, text=True, check=True).stdout
+    exported = {ln.split()[-1] for ln in out.splitlines() if " T " in ln and ln.split()[-1].startswith("foremoe_")}
+    assert exported == declared, (exported ^ declared)
+
+
+@pytest.mark.parametrize("lang,std", [("c", "c99"), ("c", "c11"), ("c++", "c++14")])
+def test_header_is_plain_c(tmp_path, lang, std):
+    """The boundary is a C ABI: the header compiles on its own as C and as C++ (no torch, no CUDA types)."""
+    import subprocess
+    src = tmp_path / ("t." + ("c" if lang == "c" else "cpp"))
+    src.write_text('#include "foremoe.h"\nint main(void) { foremoe_shape_t s; (void)s; return sizeof(s) == 44 ? 0 : 1; }\n')
+    exe = tmp_path / "t"
+    subprocess.run(["gcc" if lang == "c" else "g++", "-std=" + std, "-Wall", "-Wextra", "-Werror", "-pedantic",
+                    "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    assert subprocess.run([str(exe)]).returncode == 0          # 11 x int32: the ctypes mirror has the same size
+    assert C.sizeof(fm._CShape) == 44
+
+
 def test_workspace_bytes_and_invalid_shapes(libpath):
     s = fm.Shape(L=48, E=128, K=8, P=8, Nb=16, Nr=2, T=524288, n_mb=32, H=2048)
     n = fm.workspace_bytes(s)
@@ -52,6 +76,20 @@ def test_null_pointers_rejected_before_any_cuda_call(libpath):
     assert lib.foremoe_dispatch(C.byref(cs), 0, 0, 1, None, None, None, None, None, None, None) == fm.ERR_INVALID_ARG
     assert lib.foremoe_combine(C.byref(cs), 0, 0, 1, None, None, None, None, None, None, None) == fm.ERR_INVALID_ARG
     assert lib.foremoe_step_host(C.byref(cs), *([None] * 10), 0, None, None) == fm.ERR_INVALID_ARG
+    # the widened entry points check their arguments on the host as well
+    assert lib.foremoe_combine_bwd(C.byref(cs), 0, 0, 1, *([None] * 9)) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_dispatch_bwd(C.byref(cs), 0, 0, 1, *([None] * 6)) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_base_placement(C.byref(cs), None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_base_placement_machines(C.byref(cs), 2, 1, 1, None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_microstep_placement(C.byref(cs), 1, None, None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_replication(C.byref(cs), 1, None, None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_swap_relocation(C.byref(cs), 1, 2, 8, 1, 0, None, None, None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_source_ids(C.byref(cs), 2, None, None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_local_placement(C.byref(cs), 2, None, None, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_traffic(C.byref(cs), 2, None, None, None) == fm.ERR_INVALID_ARG
+    for M in (0, 3):                                  # M must divide P = 4
+        one = (C.c_int32 * 64)()
+        assert lib.foremoe_traffic(C.byref(cs), M, one, one, None) == fm.ERR_INVALID_ARG
 
 
 def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):

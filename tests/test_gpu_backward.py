@@ -183,3 +183,39 @@ def test_backward_host_errors(cuda_device):
         fm.combine_bwd(s, 0, 0, 1, sp.mb_off, sp.inv, sp.w, dy, None, d, dw)
     with pytest.raises(fm.ForeMoEError):                      # misaligned rows
         fm.combine_bwd(s, 0, 0, 1, sp.mb_off, sp.inv, sp.w, dy, eo, d.view(-1)[1:], None)
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_backward_skips_faulted_pairs(cuda_device, cfg_id):
+    """Pairs with an invalid expert id get inv = -1 in the plan (fault ID_RANGE): the backward leaves
+    the rows no pair maps to untouched, writes dw = 0 for them and sums only the valid rows into dx
+    (fp32 rows: K = 2; bf16 rows: K = 8 with several slices per row)."""
+    cfg = synth.config(1) if cfg_id == 1 else synth.config(2).scaled(L=1, n_samples=4, sample_len=300, H=1024, mb_samples=2)
+    ids, w, mb_off, se = G.make_case(cfg)
+    bad = ids.copy()
+    bad[0, 3, 1] = cfg.E + 3
+    bad[0, 40, 0] = -1
+    bad[0, int(mb_off[1]) + 7, cfg.K - 1] = 1 << 20
+    ref = G.oracle_plan(bad, mb_off, se, cfg.E, cfg.P, cfg.Ns)
+    sp = G.gpu_plan(fm.shape_of(cfg), bad, w, mb_off, se)
+    assert sp.faults() == fm.FAULT_ID_RANGE and ref["fault"] == orc.FAULT_ID_RANGE
+    G.assert_plan_equal(sp, ref, "bad-id")
+    assert (ref["inv"][0] < 0).sum() == 3
+    check_backward(sp, ref, [0], [0, 1], "bad-id-bwd")
+    # the skipped tokens too: dx sums the rows that exist (rows of d_eo the oracle and the GPU agree on)
+    s = sp.shape
+    a, b = 0, int(mb_off[1])
+    eo = _rows(s, b * s.K, 77)
+    dy = torch.randn((b, s.H), generator=torch.Generator().manual_seed(78)).to(G.DEV)
+    d_eo = torch.zeros_like(eo)
+    dw = torch.full((s.L, s.T, s.K), float("nan"), dtype=torch.float32, device=G.DEV)
+    dx = torch.empty((b, s.H), dtype=torch.float32, device=G.DEV)
+    sp.combine_bwd(0, 0, 1, dy, eo, d_eo, dw)
+    sp.dispatch_bwd(0, 0, 1, d_eo, dx)
+    torch.cuda.synchronize()
+    inv = ref["inv"][0, a:b]
+    d_ref, dw_ref = orc.combine_bwd(inv, w[0, a:b], dy.cpu().numpy(), G.to_bits(eo), s.act_dtype, b * s.K)
+    assert (G.to_bits(d_eo) == d_ref).all()
+    assert (dx.cpu().numpy().view(np.uint32) == orc.dispatch_bwd(inv, d_ref, s.act_dtype).view(np.uint32)).all()
+    dw_g = dw[0, a:b].cpu().numpy()
+    assert (dw_g[inv < 0] == 0).all() and (dw_ref[inv < 0] == 0).all()

@@ -273,6 +273,11 @@ k_chunk_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off
 struct QuotaSmem {
   int32_t *c, *q, *load, *se, *act, *hptr, *hslot, *ahs, *rk, *rslot, *R, *nact, *visited, *par_rank,
       *par_from, *par_to, *queue, *soff;
+  // Phase B bookkeeping: stamp[r] = event number of the last change of load[r]; seen[e] = event
+  // number at e's last fill.  A fill is a pure function of its hosts' loads (own quota removed) and
+  // c[e], so when no host rank was touched since e's last fill it would reproduce the same quotas:
+  // it is skipped.  The result is unchanged bit for bit; late passes cost almost nothing.
+  int32_t *stamp, *seen;
 };
 // hptr/hslot: all slots of expert e (ascending); ahs[hptr[e] .. hptr[e] + nact[e]): its ACTIVE host
 // slots (ascending); rk[j] = rank of slot j.
@@ -326,18 +331,26 @@ __device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e) {
 // f_a = sum_b max(0, l_a - l_b) is what it costs to raise every lower host to l_a; the water level
 // sits on top of the highest host load l* with f(l*) <= c:  lam = l* + (c - f(l*)) / m,
 // m = #{l_b <= l*}, and (c - f(l*)) % m units are left for the lowest slots among those m hosts.
-__device__ __forceinline__ int water_fill_expert_warp(const QuotaSmem &s, int e, int lane) {
+__device__ __forceinline__ int water_fill_expert_warp(const QuotaSmem &s, int e, int lane, int &event) {
   const unsigned full = 0xffffffffu;
   const int a0 = s.hptr[e], h = s.nact[e];
   if (h > 32) {
     int ch = 0;
     if (lane == 0) ch = water_fill_expert(s, e);
     __syncwarp();
-    return __shfl_sync(full, ch, 0);
+    ch = __shfl_sync(full, ch, 0);
+    if (ch) {                                    // conservative: every host rank counts as touched
+      event++;
+      for (int a = a0 + lane; a < a0 + h; a += 32) s.stamp[s.rk[s.ahs[a]]] = event;
+      __syncwarp();
+    }
+    return ch;
   }
   const bool on = lane < h;
   int j = 0, r = 0, qold = 0, l = INT_MAX;
-  if (on) { j = s.ahs[a0 + lane]; r = s.rk[j]; qold = s.q[j]; l = s.load[r] - qold; }
+  if (on) { j = s.ahs[a0 + lane]; r = s.rk[j]; }
+  if (__reduce_max_sync(full, on ? s.stamp[r] : 0) <= s.seen[e]) return 0;   // hosts untouched: same result
+  if (on) { qold = s.q[j]; l = s.load[r] - qold; }
   const int c = s.c[e];
   long long f = 0;
   for (int b = 0; b < h; b++) {
@@ -359,6 +372,11 @@ __device__ __forceinline__ int water_fill_expert_warp(const QuotaSmem &s, int e,
   }
   if (on) { s.q[j] = g; s.load[r] = l + g; }
   const int changed = __any_sync(full, on && g != qold);
+  if (changed) {
+    event++;
+    if (on && g != qold) s.stamp[r] = event;
+  }
+  if (lane == 0) s.seen[e] = event;
   __syncwarp();
   return changed;
 }
@@ -439,6 +457,8 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   s.par_from = p; p += P;
   s.par_to = p; p += P;
   s.queue = p; p += P;
+  s.stamp = p; p += P;
+  s.seen = p; p += E;
   __shared__ int nR_raw;
 
   for (int e = tid; e < E; e += nt) s.c[e] = hist[(size_t)inst * E + e];
@@ -452,7 +472,8 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
     s.rk[j] = j / Ns;
     s.q[j] = 0;
   }
-  for (int r = tid; r < P; r += nt) s.load[r] = 0;
+  for (int r = tid; r < P; r += nt) { s.load[r] = 0; s.stamp[r] = 1; }
+  for (int e = tid; e < E; e += nt) s.seen[e] = 0;
   if (tid == 0) nR_raw = 0;
   __syncthreads();
 
@@ -522,9 +543,10 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
     __syncthreads();
     if (tid < 32) {
       // Phase B: Gauss-Seidel water-filling to a fixpoint (warp 0, one lane per host)
+      int event = 1;
       for (int pass = 0; pass < kMaxWaterPasses; pass++) {
         int changed = 0;
-        for (int a = 0; a < nR; a++) changed |= water_fill_expert_warp(s, s.R[a], tid);
+        for (int a = 0; a < nR; a++) changed |= water_fill_expert_warp(s, s.R[a], tid, event);
         if (!changed) break;
       }
       // Phase C: exactness cleanup
@@ -777,7 +799,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
   int32_t *inst_slot_adj = (int32_t *)(ws + w.inst_slot_adj);
   int32_t *inst_ok = (int32_t *)(ws + w.inst_ok), *chunk_cnt = (int32_t *)(ws + w.chunk_cnt);
 
-  const size_t smem_quota = sizeof(int32_t) * ((size_t)4 * d.E + 1 + (size_t)8 * d.S + 1 + (size_t)6 * d.P);
+  const size_t smem_quota = sizeof(int32_t) * ((size_t)5 * d.E + 1 + (size_t)8 * d.S + 1 + (size_t)7 * d.P);
   const size_t smem_pairs = sizeof(int32_t) * ((size_t)d.E + 1 + (size_t)3 * d.S + (size_t)kChunkWarps * d.E);
   const size_t smem_pl = sizeof(int32_t) * ((size_t)2 * d.S + d.E + 1);
   if (smem_quota > 200 * 1024 || smem_pairs > 200 * 1024 || smem_pl > 200 * 1024)

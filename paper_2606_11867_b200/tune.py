@@ -1,6 +1,8 @@
 """Sweep the launch parameters of foremoe_dispatch / foremoe_combine on one config (GPU only).
 
     python -m paper_2606_11867_b200.tune --config 2 --layers 2 [--quick]
+    python -m paper_2606_11867_b200.tune --config 2 --layers 1 --samples 32 --bwd      # backward kernels
+    python -m paper_2606_11867_b200.tune --config 3 --layers 0 --planner [--machines M] # planner stages, full config
 
 Prints one JSON line per variant: mean CUDA-event time per launch (us), algorithmic GB/s, and
 whether the variant's perm / buf / y are bit-identical to the default kernels' outputs.  Also

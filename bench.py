@@ -494,7 +494,11 @@ def run_ours(args, cfg) -> None:
     else:
         wl.release()
     if rank == 0 and world == 1 and not args.no_cpu_baseline and not upd:
-        samp = OracleSample(cfg, 1, args.cpu_sample_mb)
+        n_samp = args.cpu_sample_mb
+        if n_samp <= 0:     # ~30 GB of algorithmic bytes = ~15 s for the single-threaded oracle
+            per_mb = bpt["total"] * max(1, cfg.T // cfg.n_mb)
+            n_samp = int(max(1, min(cfg.n_mb, round(30e9 / per_mb))))
+        samp = OracleSample(cfg, 1, n_samp)
         secs = samp.step()
         line["cpu_baseline"] = {"value": samp.routed_tokens / secs, "unit": UNIT, "cores": 1,
                                 "kind": "oracle", "sample": samp.desc, "seconds": secs}
@@ -516,7 +520,9 @@ def main() -> None:
     ap.add_argument("--probe-stride", type=int, default=8,
                     help="CUDA-event brackets around every n-th instance's dispatch / combine launch")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--cpu-sample-mb", type=int, default=8)
+    ap.add_argument("--cpu-sample-mb", type=int, default=0,
+                    help="micro-steps (x 1 layer) of the workload the oracle is timed on; 0 = as many as make "
+                         "about 15 s of CPU work (the oracle moves ~2 GB/s of algorithmic bytes on one core)")
     ap.add_argument("--graph", action="store_true",
                     help="replay the per-instance loop as one CUDA graph (per-kernel probes are then "
                          "taken in an extra untimed step)")

@@ -160,10 +160,19 @@ static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *m
                            int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
   static int occ = 0;
   if (!occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
-  // 32 CTAs per SM although only `occ` are resident: the store path runs ~10 % faster with fresh
-  // CTAs streaming in than with a strictly persistent grid (profiles/r01_sweeps.md)
-  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : (occ > 32 ? occ : 32);
+  // Oversubscribed grid, about one (token, slice) item per warp although only `occ` CTAs are
+  // resident per SM: the store path runs ~10 % faster with fresh CTAs streaming in than with a
+  // strictly persistent grid (profiles/r01_sweeps.md).  The item count of a launch is estimated
+  // from the mean micro-step of the shape (mb_off lives on the device): 4..128 CTAs per SM.
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
+  int per_sm = g_tune.dispatch_cta_per_sm;
+  if (per_sm <= 0) {
+    const long long items = (long long)(d.T / d.n_mb + 1) * n_slices;
+    const long long want = (items + 8LL * num_sms() - 1) / (8LL * num_sms());
+    per_sm = 4;
+    while (per_sm < want && per_sm < 128) per_sm <<= 1;
+    if (per_sm < occ) per_sm = occ;
+  }
   const cudaError_t e = launch_pdl(k_dispatch_rows<U>, num_sms() * per_sm, 256, 0, st, inv_l, mb_off,
                                    mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)x, perm,
                                    (int4 *)buf);
@@ -244,7 +253,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const for
     if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
   }
   int U = g_tune.dispatch_u;
-  if (U <= 0) U = d.row_vec >= 256 ? 8 : d.row_vec >= 128 ? 4 : d.row_vec >= 64 ? 2 : 1;
+  if (U <= 0) U = d.row_vec >= 64 ? 2 : 1;      // 1 KB slices: best or within 1 % of best on every config (sweep)
   if (U >= 8) return launch_dispatch<8>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
   if (U >= 4) return launch_dispatch<4>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
   if (U >= 2) return launch_dispatch<2>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);

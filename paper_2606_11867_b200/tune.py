@@ -41,9 +41,8 @@ def set_tuning(**kw) -> None:
         lib.foremoe_debug_set_tuning(i, int(kw.get(k, DEFAULTS.get(k, 0))))
 
 
-DISPATCH_VARIANTS = [
-    {}, {"dispatch_cta_per_sm": 4}, {"dispatch_cta_per_sm": 8}, {"dispatch_cta_per_sm": 16},
-    {"dispatch_cta_per_sm": 64}, {"dispatch_u": 4}, {"dispatch_u": 2, "dispatch_cta_per_sm": 64},
+DISPATCH_VARIANTS = [{}] + [{"dispatch_u": u, "dispatch_cta_per_sm": c} for u in (1, 2, 4, 8) for c in (16, 32, 64, 128)] + [
+    {"dispatch_cta_per_sm": 4}, {"dispatch_cta_per_sm": 8},
     {"dispatch_impl": 1}, {"dispatch_impl": 1, "dispatch_warps": 4, "dispatch_stages": 3, "dispatch_cta_per_sm": 14},
 ]
 COMBINE_VARIANTS = [

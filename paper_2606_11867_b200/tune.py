@@ -188,6 +188,7 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=2)
     ap.add_argument("--layers", type=int, default=2, help="0 = all layers of the config")
     ap.add_argument("--samples", type=int, default=None, help="fewer samples (config 3: 32)")
+    ap.add_argument("--mb-samples", type=int, default=None, help="config 4: samples per micro-step")
     ap.add_argument("--quick", action="store_true")
     ap.add_argument("--hist", action="store_true", help="sweep the k_load_hist modes instead")
     ap.add_argument("--plan", action="store_true", help="time foremoe_load_hist / foremoe_assign only")
@@ -196,7 +197,7 @@ def main() -> None:
     ap.add_argument("--machines", type=int, default=1, help="--planner: machines for Alg. 3")
     args = ap.parse_args()
     import bench
-    cfg = synth.config(args.config)
+    cfg = synth.config(args.config, mb_samples=args.mb_samples)
     if args.layers > 0 or args.samples:
         cfg = cfg.scaled(L=args.layers if args.layers > 0 else None, n_samples=args.samples)
     dev = torch.device("cuda:0")

@@ -197,10 +197,15 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
     attr_set = true;
   }
   if (!occ || occ_key != smem * 1024 + threads) { occ = occupancy_ctas(kern, threads, smem); occ_key = smem * 1024 + threads; }
-  // oversubscribed grid: 8 CTAs per SM (32 without the eo reads) although only `occ` are resident --
+  // oversubscribed grid: 8-16 CTAs per SM (32 without the eo reads) although only `occ` are resident --
   // fresh CTAs streaming in balance the tail and run 5-9 % faster than a strictly persistent grid
   // (sweep: profiles/r01_backward.md), the same effect as on the dispatch store path
-  const int dflt = !kDw ? 32 : (d.T / d.n_mb >= 24576 ? 16 : 8);
+  // size: about one token per warp (mean micro-step of the shape), rounded down to a power of two,
+  // at most 16 CTAs per SM with the eo reads (32 without)
+  const int cap = kDw ? 16 : 32;
+  const long long want = (long long)(d.T / d.n_mb + 1) / ((threads / 32) * (long long)num_sms());
+  int dflt = 1;
+  while (dflt * 2 <= want && dflt * 2 <= cap) dflt <<= 1;
   const int per_sm = g_tune.bwd_cta_per_sm > 0 ? g_tune.bwd_cta_per_sm : (occ > dflt ? occ : dflt);
   const int n_slices = (d.row_vec + 31) / 32;
   const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, threads, smem, st, inv_l, w_l, mb_off,

@@ -83,8 +83,18 @@ class Shape:
         return torch.bfloat16 if self.act_dtype == ACT_BF16 else torch.float32
 
     def c(self) -> _CShape:
-        return _CShape(self.L, self.E, self.K, self.P, self.Nb, self.Nr, self.T, self.n_mb,
-                       self.H, self.act_dtype, self.placement_mb_stride)
+        """The C struct (cached per field tuple: the per-instance calls of a step reuse it)."""
+        key = (self.L, self.E, self.K, self.P, self.Nb, self.Nr, self.T, self.n_mb, self.H,
+               self.act_dtype, self.placement_mb_stride)
+        hit = _shape_cache.get(key)
+        if hit is None:
+            if len(_shape_cache) > 256:
+                _shape_cache.clear()
+            hit = _shape_cache[key] = _CShape(*key)
+        return hit
+
+
+_shape_cache: dict = {}
 
 
 _lib = None
@@ -148,7 +158,14 @@ def _host(t: Optional[torch.Tensor], dtype=None) -> Optional[int]:
     return t.data_ptr()
 
 
+_raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+
+
 def _stream() -> int:
+    """cudaStream_t of torch's current stream on the current device (the raw getter avoids building a
+    Stream object per call: the per-instance calls of small micro-steps are host-bound)."""
+    if _raw_stream is not None:
+        return _raw_stream(torch.cuda.current_device())
     return torch.cuda.current_stream().cuda_stream
 
 

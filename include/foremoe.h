@@ -25,7 +25,9 @@
  * General rules
  *  - Every data pointer is a DEVICE pointer owned by the caller unless the argument is marked
  *    "host".  The foremoe_shape_t pointer is a host pointer, read during the call only.
- *  - The library allocates no device memory, keeps no global state and is re-entrant per stream.
+ *  - The library allocates no device memory and is re-entrant per stream.  Its only process state
+ *    is a set of memoised launch facts (SM count, occupancy, shared-memory opt-in), keyed by the
+ *    current device and refilled when it changes, and the sweep-only tuning at the end of this file.
  *    All entry points except foremoe_workspace_bytes / foremoe_version / foremoe_step_host
  *    enqueue work on `stream` (a cudaStream_t passed as void*) and return without synchronising.
  *  - Return value: FOREMOE_OK, or a negative host-detectable error (nothing was enqueued).

@@ -188,13 +188,14 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
   const size_t smem = (size_t)D * NV * threads * 16 + (size_t)(threads / 32) * D * 32 * 8;
   if (smem > 220 * 1024) return FOREMOE_ERR_INVALID_ARG;
   auto kern = k_combine_bwd<kBf16, K_T, D, kDw>;
-  static bool attr_set = false;
-  static int occ = 0;
+  static int occ = 0, cached_dev = -1;
   static size_t occ_key = 0;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess)
+  if (cache_stale(&cached_dev)) {
+    occ = 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) {
+      cached_dev = -1;
       return FOREMOE_ERR_CUDA;
-    attr_set = true;
+    }
   }
   if (!occ || occ_key != smem * 1024 + threads) { occ = occupancy_ctas(kern, threads, smem); occ_key = smem * 1024 + threads; }
   // oversubscribed grid: 8-16 CTAs per SM (32 without the eo reads) although only `occ` are resident --

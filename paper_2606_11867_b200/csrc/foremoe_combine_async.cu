@@ -124,14 +124,15 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
                       cudaStream_t st) {
   const size_t smem = (size_t)D * d.K * threads * 16 + (size_t)(threads / 32) * D * 32 * 8;
   if (smem > 220 * 1024) return FOREMOE_ERR_INVALID_ARG;
-  static size_t smem_set = 0;
-  static int occ = 0;
+  static int occ = 0, cached_dev = -1;
   static size_t occ_key = 0;
   auto kern = k_combine_async<kBf16, K_T, D>;
-  if (smem > smem_set) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess)
+  if (cache_stale(&cached_dev)) {
+    occ = 0;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) {
+      cached_dev = -1;
       return FOREMOE_ERR_CUDA;
-    smem_set = 220 * 1024;
+    }
   }
   if (!occ || occ_key != smem * 1024 + threads) { occ = occupancy_ctas(kern, threads, smem); occ_key = smem * 1024 + threads; }
   const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;

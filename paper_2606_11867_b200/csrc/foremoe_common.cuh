@@ -102,4 +102,16 @@ __device__ __forceinline__ int find_range(const int32_t *__restrict__ off, int n
 
 int num_sms();
 
+// The launchers memoise per-kernel launch facts (occupancy, the opt-in shared-memory attribute).
+// Both are per DEVICE: a cache remembers the device it was filled on and is refilled when the
+// calling thread's current device differs (one process per GPU is the normal case; this keeps a
+// process that drives several devices correct).  Returns true when the cache must be refilled.
+inline bool cache_stale(int *cached_dev) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return true;
+  if (*cached_dev == dev) return false;
+  *cached_dev = dev;
+  return true;
+}
+
 }  // namespace foremoe

@@ -158,8 +158,8 @@ DataTuning g_tune;
 template <int U>
 static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
                            int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
-  static int occ = 0;
-  if (!occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
+  static int occ = 0, cached_dev = -1;
+  if (cache_stale(&cached_dev) || !occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
   // Oversubscribed grid, about one (token, slice) item per warp although only `occ` CTAs are
   // resident per SM: the store path runs ~10 % faster with fresh CTAs streaming in than with a
   // strictly persistent grid (profiles/r01_sweeps.md).  The item count of a launch is estimated
@@ -183,8 +183,8 @@ template <bool kBf16, int KB, int U>
 static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
                           const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
                           cudaStream_t st) {
-  static int occ = 0;
-  if (!occ) occ = occupancy_ctas(k_combine_rows<kBf16, KB, U>, 256);
+  static int occ = 0, cached_dev = -1;
+  if (cache_stale(&cached_dev) || !occ) occ = occupancy_ctas(k_combine_rows<kBf16, KB, U>, 256);
   const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   const cudaError_t e = launch_pdl(k_combine_rows<kBf16, KB, U>, num_sms() * per_sm, 256, 0, st, inv_l,

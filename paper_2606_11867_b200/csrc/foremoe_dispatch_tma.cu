@@ -109,11 +109,11 @@ int launch_dispatch_tma(const Dims &d, const int32_t *inv_l, const int32_t *mb_o
   while (NS >= 3 && per_stage * warps * NS > budget) NS--;
   if (NS < 3) return FOREMOE_ERR_INVALID_ARG;       // rows too large for a ring: caller falls back
   const size_t smem = per_stage * warps * NS;
-  static size_t smem_set = 0;
-  if (smem > smem_set) {
-    if (cudaFuncSetAttribute(k_dispatch_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget) != cudaSuccess)
-      return FOREMOE_ERR_CUDA;
-    smem_set = budget;
+  static int cached_dev = -1;
+  if (cache_stale(&cached_dev) &&
+      cudaFuncSetAttribute(k_dispatch_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget) != cudaSuccess) {
+    cached_dev = -1;
+    return FOREMOE_ERR_CUDA;
   }
   const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : 1;
   k_dispatch_tma<<<num_sms() * per_sm, warps * 32, smem, st>>>(

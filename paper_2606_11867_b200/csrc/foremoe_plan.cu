@@ -712,12 +712,12 @@ using namespace foremoe;
 
 namespace foremoe {
 int num_sms() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+  static int n = 0, cached_dev = -1;
+  if (cache_stale(&cached_dev) || n == 0) {
+    if (cached_dev < 0 ||
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, cached_dev) != cudaSuccess || n <= 0) {
       n = 0;
+      cached_dev = -1;
       return 148;
     }
   }

@@ -26,6 +26,18 @@ __device__ __forceinline__ int pack_bf16x2(float lo, float hi) {
   return r;
 }
 
+// cp.async that copies nothing (zero-fills) when src_bytes == 0: absent rows and lanes beyond the
+// row need no branch (same scheme as k_combine_async)
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void *src, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ int4 lds16(uint32_t addr) {
+  int4 r;
+  asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
+  return r;
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -50,7 +62,9 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
   pdl_launch_dependents();
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  int4 *data = (int4 *)smem;                                            // [(s*NV + j)*nt + tid]
+  const uint32_t vstride = (uint32_t)nt * 16u, sstride = (uint32_t)NV * vstride;   // bytes; slot (s, j) of this thread:
+  const uint32_t data0 = smem_u32(smem) + (uint32_t)tid * 16u;                    // data0 + s*sstride + j*vstride
+  const uint32_t row_bytes = (uint32_t)row_vec * 16u;
   int32_t *dbuf = (int32_t *)(smem + (size_t)D * NV * nt * 16) + warp * D * 32;
   float *wbuf = (float *)(smem + (size_t)D * NV * nt * 16 + (size_t)(nt >> 5) * D * 32 * 4) + warp * D * 32;
 
@@ -74,27 +88,26 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
     if (i_tok < n_my) {
       const int s = i_n % D;
       const int tl = w0 + i_tok * W;
-      const int v = i_sl * 32 + lane;
+      uint32_t voff = (uint32_t)(i_sl * 32 + lane) * 16u;
+      const uint32_t sz = voff < row_bytes ? 16u : 0u;          // lanes beyond the row copy nothing
+      voff = sz ? voff : 0u;
       if (i_sl == 0) {
         d_cur = d_nxt >= 0 ? d_nxt - rg.row0 : -1;
         w_cur = w_nxt;
         fetch_meta(i_tok + 1);
       }
       if (lane < K) { dbuf[s * 32 + lane] = d_cur; wbuf[s * 32 + lane] = w_cur; }
-      if (v < row_vec) {
+      const uint32_t dst0 = data0 + (uint32_t)s * sstride;
+      const unsigned char *dsrc = (const unsigned char *)dy + ((unsigned long long)(unsigned)tl * row_bytes + voff) * DY;
 #pragma unroll
-        for (int j = 0; j < DY; j++)
-          cp_async16(smem_u32(data + ((size_t)(s * NV + j) * nt + tid)),
-                     dy + ((size_t)tl * row_vec + v) * DY + j);
-      }
+      for (int j = 0; j < DY; j++) cp_async16_zfill(dst0 + (uint32_t)j * vstride, dsrc + 16 * j, sz);
       if (kDw) {
 #pragma unroll
         for (int k = 0; k < KU; k++) {
           if (K_T == 0 && k >= K) break;
           const int dk = __shfl_sync(0xffffffffu, d_cur, k);
-          if (dk >= 0 && v < row_vec)
-            cp_async16(smem_u32(data + ((size_t)(s * NV + DY + k) * nt + tid)),
-                       eo + (size_t)dk * row_vec + v);
+          const unsigned long long off = (unsigned long long)(unsigned)max(dk, 0) * row_bytes + voff;
+          cp_async16_zfill(dst0 + (uint32_t)(DY + k) * vstride, (const unsigned char *)eo + off, dk >= 0 ? sz : 0u);
         }
       }
       i_n++;
@@ -122,11 +135,11 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
       if (v < row_vec) {
         float g[kF];
         {
-          const int4 a = data[(size_t)(s * NV) * nt + tid];
+          const int4 a = lds16(data0 + (uint32_t)s * sstride);
           g[0] = __int_as_float(a.x); g[1] = __int_as_float(a.y);
           g[2] = __int_as_float(a.z); g[3] = __int_as_float(a.w);
           if (kBf16) {
-            const int4 b = data[(size_t)(s * NV + 1) * nt + tid];
+            const int4 b = lds16(data0 + (uint32_t)s * sstride + vstride);
             g[4] = __int_as_float(b.x); g[5] = __int_as_float(b.y);
             g[6] = __int_as_float(b.z); g[7] = __int_as_float(b.w);
           }
@@ -138,7 +151,7 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
           const float wk = wbuf[s * 32 + k];
           if (dk < 0) continue;
           if (kDw) {
-            const int4 r = data[(size_t)(s * NV + DY + k) * nt + tid];
+            const int4 r = lds16(data0 + (uint32_t)s * sstride + (uint32_t)(DY + k) * vstride);
             float acc = part[k];
             if (kBf16) {
               acc = __fmaf_rn(g[0], bf16_lo(r.x), acc); acc = __fmaf_rn(g[1], bf16_hi(r.x), acc);
@@ -161,7 +174,7 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
             o.x = __float_as_int(__fmul_rn(wk, g[0])); o.y = __float_as_int(__fmul_rn(wk, g[1]));
             o.z = __float_as_int(__fmul_rn(wk, g[2])); o.w = __float_as_int(__fmul_rn(wk, g[3]));
           }
-          st16_stream(d_eo + (size_t)dk * row_vec + v, o);
+          st16_stream((unsigned char *)d_eo + ((unsigned long long)(unsigned)dk * row_bytes + (uint32_t)v * 16u), o);
         }
       }
       __syncwarp();                        // dbuf / wbuf of stage s free before it is refilled
@@ -263,14 +276,14 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine_bwd(
   const bool want_dw = dw != nullptr;
   float *dw_l = want_dw ? dw + lo : nullptr;
   cudaStream_t st = (cudaStream_t)stream;
-  // stages: 3 when they fit 128 KB per CTA (K = 8: 120 KB), else 2; without eo reads 2 is enough
   const int NV = (d.act_dtype == FOREMOE_ACT_BF16 ? 2 : 1) + (want_dw ? d.K : 0);
-  int threads = 256;
-  while (threads > 32 && (size_t)2 * NV * threads * 16 > 200 * 1024) threads >>= 1;   // large K
-  int D = g_tune.bwd_depth;
-  if (D <= 0) {
-    D = (want_dw && (size_t)3 * NV * threads * 16 <= 128 * 1024) ? 3 : 2;
-  }
+  // same sizing as k_combine_async: D = 3 stages, about 120 KB in flight per CTA (K = 8: 256 threads,
+  // K = 10: 192); without the eo reads only the dy slices are staged and 2 stages of 256 threads do
+  int D = g_tune.bwd_depth > 0 ? g_tune.bwd_depth : (want_dw ? 3 : 2);
+  int threads = want_dw ? (int)(120 * 1024 / ((size_t)D * NV * 16)) / 32 * 32 : 256;
+  threads = threads < 32 ? 32 : threads > 256 ? 256 : threads;
+  if (threads > 64) threads = threads / 64 * 64;
+  while (D > 2 && (size_t)D * NV * threads * 16 > 200 * 1024) D--;
   const bool bf = d.act_dtype == FOREMOE_ACT_BF16;
   if (bf && want_dw) return launch_k<true, true>(D, d, threads, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out, dw_l, st);
   if (bf) return launch_k<true, false>(D, d, threads, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out, dw_l, st);

@@ -9,101 +9,138 @@
 
 namespace foremoe {
 
-// smem: data [D][K][threads] int4, then per warp [D][32] int32 rows and [D][32] float weights
+// 16-byte cp.async whose source size is 0 when the row is absent: the destination is zero-filled
+// and no global access is made, so a skipped pair (inv < 0) or a lane beyond the row needs no branch
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void *src, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+
+// smem: data [D][K][threads] int4, then per warp [D][32] float weights (0 for a skipped pair).
+// Instruction budget matters here: under the board's power cap the SM clock drops to ~1.7 GHz and a
+// kernel that keeps the issue slots 60 % busy loses bandwidth with it.  Hence: no divisions in the
+// item loop (the (token, slice) cursors advance by a precomputed stride), 32-bit shared-memory byte
+// offsets, one 32x32+64-bit multiply-add per global address, zero-fill instead of per-row branches,
+// vector loads of the K weights.
 template <bool kBf16, int K_T, int D>
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(768)
 k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
                 const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K_rt, int row_vec,
                 int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
   constexpr int kF = kBf16 ? 8 : 4;
+  constexpr int KU = K_T > 0 ? K_T : 32;
   const int K = K_T > 0 ? K_T : K_rt;
   pdl_launch_dependents();
   extern __shared__ __align__(128) unsigned char smem[];
-  const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  int4 *data = (int4 *)smem;                                           // [(s*K + k)*nt + tid]
-  int32_t *dbuf = (int32_t *)(smem + (size_t)D * K * nt * 16) + warp * D * 32;
-  float *wbuf = (float *)(smem + (size_t)D * K * nt * 16 + (size_t)(nt >> 5) * D * 32 * 4) + warp * D * 32;
+  const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = nt >> 5;
+  const uint32_t kstride = (uint32_t)nt * 16u, sstride = (uint32_t)K * kstride;       // bytes
+  const uint32_t data0 = smem_u32(smem) + (uint32_t)tid * 16u;                        // + s*sstride + k*kstride
+  float *wbuf = (float *)(smem + (size_t)D * sstride) + warp * (D * 32);              // [D][32]
 
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
-  const long long W = (long long)gridDim.x * (nt >> 5);
-  const long long w0 = (long long)blockIdx.x * (nt >> 5) + warp;
+  const int W = (int)gridDim.x * nwarp;
+  const int w0 = (int)blockIdx.x * nwarp + warp;
   const int n_my = w0 < n_items ? (int)((n_items - w0 + W - 1) / W) : 0;
+  const int dW_t = W / n_slices, dW_s = W - dW_t * n_slices;        // cursor stride: one division per kernel
+  const uint32_t row_bytes = (uint32_t)row_vec * 16u;
+
+  // three cursors over this warp's items (token, slice): metadata fetch, copy issue, reduce
+  int m_tl = w0 / n_slices, m_sl = w0 - m_tl * n_slices;
+  int i_tl = m_tl, i_sl = m_sl, c_tl = m_tl, c_sl = m_sl;
+  int i_n = 0, i_s = 0, c_s = 0, m_n = 0;
+  auto advance = [&](int &tl, int &sl) {
+    sl += dW_s; tl += dW_t;
+    if (sl >= n_slices) { sl -= n_slices; tl++; }
+  };
 
   int d_nxt = -1;
   float w_nxt = 0.f;
-  auto fetch_meta = [&](int n) {           // inv / w of item n into registers (lanes < K)
-    if (n < n_my && lane < K) {
-      const long long item = w0 + (long long)n * W;
-      const int tl = (int)(item / n_slices);
-      const size_t p = (size_t)(rg.t_begin + tl) * K + lane;
+  auto fetch_meta = [&]() {                // inv / w of the next item into registers (lanes < K)
+    if (m_n < n_my && lane < K) {
+      const size_t p = (size_t)(rg.t_begin + m_tl) * K + lane;
       d_nxt = __ldg(inv_l + p);
-      w_nxt = w_l ? __ldg(w_l + p) : 1.f;   // w_l == nullptr: unit weights (dispatch backward)
+      w_nxt = w_l ? __ldg(w_l + p) : 1.f;  // w_l == nullptr: unit weights (dispatch backward)
     }
+    m_n++;
+    advance(m_tl, m_sl);
   };
-  auto issue = [&](int n) {                // K cp.async of item n into stage n % D
-    if (n < n_my) {
-      const int s = n % D;
-      const long long item = w0 + (long long)n * W;
-      const int tl = (int)(item / n_slices);
-      const int v = (int)(item - (long long)tl * n_slices) * 32 + lane;
-      int d = d_nxt;
-      if (lane < K) {
-        if (d >= 0) d -= rg.row0;
-        dbuf[s * 32 + lane] = d;
-        wbuf[s * 32 + lane] = w_nxt;
-      }
-      fetch_meta(n + 1);
+  auto issue = [&]() {                     // K cp.async of the next item into stage i_s
+    if (i_n < n_my) {
+      int d = -1;
+      float wv = 0.f;
+      if (lane < K && d_nxt >= 0) { d = d_nxt - rg.row0; wv = w_nxt; }
+      if (lane < K) wbuf[i_s * 32 + lane] = wv;
+      uint32_t voff = (uint32_t)(i_sl * 32 + lane) * 16u;
+      const uint32_t sz = voff < row_bytes ? 16u : 0u;      // lanes beyond the row copy nothing
+      voff = sz ? voff : 0u;
+      fetch_meta();
+      const uint32_t dst0 = data0 + (uint32_t)i_s * sstride;
 #pragma unroll
-      for (int k = 0; k < (K_T > 0 ? K_T : 32); k++) {
+      for (int k = 0; k < KU; k++) {
         if (K_T == 0 && k >= K) break;
         const int dk = __shfl_sync(0xffffffffu, d, k);
-        if (dk >= 0 && v < row_vec)
-          cp_async16(smem_u32(data + ((size_t)(s * K + k) * nt + tid)), eo + (size_t)dk * row_vec + v);
+        const unsigned long long off = (unsigned long long)(unsigned)max(dk, 0) * row_bytes + voff;
+        cp_async16_zfill(dst0 + (uint32_t)k * kstride, (const unsigned char *)eo + off, dk >= 0 ? sz : 0u);
       }
+      advance(i_tl, i_sl);
+      i_s = i_s + 1 == D ? 0 : i_s + 1;
     }
+    i_n++;
     cp_async_commit();
   };
 
-  fetch_meta(0);                           // inv / w / mb_off only: the plan's own arrays (see k_dispatch_rows)
+  fetch_meta();                            // inv / w / mb_off only: the plan's own arrays (see k_dispatch_rows)
   pdl_wait();                              // expert_out is read and y written after the wait
-  for (int n = 0; n < D - 1; n++) issue(n);
+  for (int n = 0; n < D - 1; n++) issue();
   for (int j = 0; j < n_my; j++) {
-    issue(j + D - 1);
+    issue();
     cp_async_wait<D - 1>();                // this thread's copies of item j have landed
-    __syncwarp();                          // dbuf / wbuf of item j visible to all lanes
-    const int s = j % D;
-    const long long item = w0 + (long long)j * W;
-    const int tl = (int)(item / n_slices);
-    const int v = (int)(item - (long long)tl * n_slices) * 32 + lane;
+    __syncwarp();                          // the weights of item j are visible to all lanes
+    const uint32_t ds = data0 + (uint32_t)c_s * sstride;
+    const float *ws = wbuf + c_s * 32;
+    float wk[KU];
+    if (K_T > 0 && K_T % 4 == 0) {
+#pragma unroll
+      for (int q = 0; q < KU / 4; q++) {
+        const float4 t = *(const float4 *)(ws + 4 * q);
+        wk[4 * q] = t.x; wk[4 * q + 1] = t.y; wk[4 * q + 2] = t.z; wk[4 * q + 3] = t.w;
+      }
+    } else if (K_T > 0 && K_T % 2 == 0) {
+#pragma unroll
+      for (int q = 0; q < KU / 2; q++) {
+        const float2 t = *(const float2 *)(ws + 2 * q);
+        wk[2 * q] = t.x; wk[2 * q + 1] = t.y;
+      }
+    }
     float acc[kF];
 #pragma unroll
     for (int f = 0; f < kF; f++) acc[f] = 0.f;
-    if (v < row_vec) {
 #pragma unroll
-      for (int k = 0; k < (K_T > 0 ? K_T : 32); k++) {
-        if (K_T == 0 && k >= K) break;
-        const int dk = dbuf[s * 32 + k];
-        const float wk = wbuf[s * 32 + k];
-        if (dk < 0) continue;
-        const int4 r = data[(size_t)(s * K + k) * nt + tid];
-        if (kBf16) {
-          acc[0] = __fmaf_rn(wk, bf16_lo(r.x), acc[0]);
-          acc[1] = __fmaf_rn(wk, bf16_hi(r.x), acc[1]);
-          acc[2] = __fmaf_rn(wk, bf16_lo(r.y), acc[2]);
-          acc[3] = __fmaf_rn(wk, bf16_hi(r.y), acc[3]);
-          acc[4] = __fmaf_rn(wk, bf16_lo(r.z), acc[4]);
-          acc[5] = __fmaf_rn(wk, bf16_hi(r.z), acc[5]);
-          acc[6] = __fmaf_rn(wk, bf16_lo(r.w), acc[6]);
-          acc[7] = __fmaf_rn(wk, bf16_hi(r.w), acc[7]);
-        } else {
-          acc[0] = __fmaf_rn(wk, __int_as_float(r.x), acc[0]);
-          acc[1] = __fmaf_rn(wk, __int_as_float(r.y), acc[1]);
-          acc[2] = __fmaf_rn(wk, __int_as_float(r.z), acc[2]);
-          acc[3] = __fmaf_rn(wk, __int_as_float(r.w), acc[3]);
-        }
+    for (int k = 0; k < KU; k++) {
+      if (K_T == 0 && k >= K) break;
+      const float w = (K_T > 0 && K_T % 2 == 0) ? wk[k] : ws[k];
+      int4 r;
+      asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(ds + (uint32_t)k * kstride));
+      if (kBf16) {
+        acc[0] = __fmaf_rn(w, bf16_lo(r.x), acc[0]);
+        acc[1] = __fmaf_rn(w, bf16_hi(r.x), acc[1]);
+        acc[2] = __fmaf_rn(w, bf16_lo(r.y), acc[2]);
+        acc[3] = __fmaf_rn(w, bf16_hi(r.y), acc[3]);
+        acc[4] = __fmaf_rn(w, bf16_lo(r.z), acc[4]);
+        acc[5] = __fmaf_rn(w, bf16_hi(r.z), acc[5]);
+        acc[6] = __fmaf_rn(w, bf16_lo(r.w), acc[6]);
+        acc[7] = __fmaf_rn(w, bf16_hi(r.w), acc[7]);
+      } else {
+        acc[0] = __fmaf_rn(w, __int_as_float(r.x), acc[0]);
+        acc[1] = __fmaf_rn(w, __int_as_float(r.y), acc[1]);
+        acc[2] = __fmaf_rn(w, __int_as_float(r.z), acc[2]);
+        acc[3] = __fmaf_rn(w, __int_as_float(r.w), acc[3]);
       }
-      float4 *dst = y + (size_t)tl * row_vec * (kF / 4) + (size_t)v * (kF / 4);
+    }
+    const int v = c_sl * 32 + lane;
+    if (v < row_vec) {
+      float4 *dst = y + ((size_t)c_tl * row_vec + v) * (kF / 4);
       int4 o;
       o.x = __float_as_int(acc[0]); o.y = __float_as_int(acc[1]);
       o.z = __float_as_int(acc[2]); o.w = __float_as_int(acc[3]);
@@ -114,7 +151,9 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
         st16_stream(dst + 1, o);
       }
     }
-    __syncwarp();                          // dbuf / wbuf of stage s free before it is refilled
+    advance(c_tl, c_sl);
+    c_s = c_s + 1 == D ? 0 : c_s + 1;
+    __syncwarp();                          // the stage's weights are free before it is refilled
   }
 }
 
@@ -122,7 +161,7 @@ template <bool kBf16, int K_T, int D>
 static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const float *w_l,
                       const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
                       cudaStream_t st) {
-  const size_t smem = (size_t)D * d.K * threads * 16 + (size_t)(threads / 32) * D * 32 * 8;
+  const size_t smem = (size_t)D * d.K * threads * 16 + (size_t)(threads / 32) * D * 32 * 4;
   if (smem > 220 * 1024) return FOREMOE_ERR_INVALID_ARG;
   static int occ = 0, cached_dev = -1;
   static size_t occ_key = 0;
@@ -172,18 +211,18 @@ static int launch_k(int D, const Dims &d, int threads, const int32_t *inv_l, con
 int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
                          const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
                          cudaStream_t st) {
-  // one CTA per SM with up to 512 threads and D >= 2 stages filling <= 190 KB of shared memory
-  // (sweep: profiles/r01_sweeps.md): bytes in flight per SM = D * K * threads * 16
-  const size_t budget = 190 * 1024;
-  int threads = g_tune.combine_threads > 0 ? g_tune.combine_threads : 512;
-  if (g_tune.combine_threads <= 0)
-    while (threads > 64 && (size_t)2 * d.K * threads * 16 > budget) threads >>= 1;
-  int D = g_tune.combine_depth;
+  // One CTA per SM, D = 3 stages, about 120 KB of rows in flight: threads = the multiple of 64 with
+  // 3 * K * threads * 16 <= 120 KB (K = 8: 320 threads, K = 10: 256).  With the lean instruction
+  // stream the kernel is latency-bound, and three shallow stages beat two wide ones on every shape
+  // (sweep: profiles/r01_sweeps.md, second addendum).
+  int threads = g_tune.combine_threads, D = g_tune.combine_depth;
+  if (threads <= 0) {
+    threads = (int)(120 * 1024 / ((size_t)(D > 0 ? D : 3) * d.K * 16)) / 64 * 64;
+    threads = threads < 64 ? 64 : threads > 512 ? 512 : threads;
+  }
   if (D <= 0) {
-    const int cand[] = {8, 6, 4, 3, 2};
-    D = 2;
-    for (int c : cand)
-      if ((size_t)c * d.K * threads * 16 <= (threads >= 512 ? 128 * 1024 : budget)) { D = c; break; }
+    D = 3;
+    if ((size_t)D * d.K * threads * 16 > 200 * 1024) D = 2;      // K = 32 with 64 threads: 96 KB, fits
   }
   if (d.act_dtype == FOREMOE_ACT_BF16)
     return launch_k<true>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);

@@ -45,20 +45,8 @@ DISPATCH_VARIANTS = [{}] + [{"dispatch_u": u, "dispatch_cta_per_sm": c} for u in
     {"dispatch_cta_per_sm": 4}, {"dispatch_cta_per_sm": 8},
     {"dispatch_impl": 1}, {"dispatch_impl": 1, "dispatch_warps": 4, "dispatch_stages": 3, "dispatch_cta_per_sm": 14},
 ]
-COMBINE_VARIANTS = [
-    {}, {"combine_impl": 0}, {"combine_impl": 0, "combine_u": 2},
-    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256},
-    {"combine_impl": 1, "combine_depth": 4, "combine_threads": 128},
-    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256},
-    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 2},
-    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 4},
-    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 512, "combine_cta_per_sm": 8},
-    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256, "combine_cta_per_sm": 4},
-    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256, "combine_cta_per_sm": 8},
-    {"combine_impl": 1, "combine_depth": 3, "combine_threads": 256, "combine_cta_per_sm": 16},
-    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256, "combine_cta_per_sm": 8},
-    {"combine_impl": 1, "combine_depth": 2, "combine_threads": 256, "combine_cta_per_sm": 16},
-]
+COMBINE_VARIANTS = [{}] + [
+    {"combine_impl": 1, "combine_depth": d, "combine_threads": t} for t in (192, 256, 320, 384, 448) for d in (3, 4, 6)]
 
 
 BWD_VARIANTS = [{}] + [{"bwd_depth": d, "bwd_cta_per_sm": c} for d in (2, 3) for c in (4, 8, 16, 32)]

@@ -247,6 +247,8 @@ static int launch_k(int D, const Dims &d, int threads, const int32_t *inv_l, con
                     void *d_eo, float *dw_l, cudaStream_t st) {
   switch (d.K) {
     case 2: return launch_depth<kBf16, 2, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
+    case 4: return launch_depth<kBf16, 4, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
+    case 6: return launch_depth<kBf16, 6, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
     case 8: return launch_depth<kBf16, 8, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
     case 10: return launch_depth<kBf16, 10, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
   }

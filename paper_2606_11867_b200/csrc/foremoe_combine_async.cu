@@ -202,6 +202,8 @@ static int launch_k(int D, const Dims &d, int threads, const int32_t *inv_l, con
                     cudaStream_t st) {
   switch (d.K) {
     case 2: return launch_depth<kBf16, 2>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+    case 4: return launch_depth<kBf16, 4>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+    case 6: return launch_depth<kBf16, 6>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
     case 8: return launch_depth<kBf16, 8>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
     case 10: return launch_depth<kBf16, 10>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
   }

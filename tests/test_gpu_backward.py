@@ -104,7 +104,7 @@ def test_scaled_configs_backward(cuda_device, cfg_id, kw):
 
 
 @pytest.mark.parametrize("K,H,bf16", [(1, 8, False), (3, 40, True), (5, 264, True), (32, 72, False),
-                                      (7, 1000, True)])
+                                      (7, 1000, True), (4, 520, True), (6, 136, False)])
 def test_generic_k_and_ragged_rows(cuda_device, K, H, bf16):
     """K outside the specialised set (generic kernel), rows that are not a multiple of 512 bytes,
     empty micro-steps."""

@@ -125,13 +125,13 @@ def _random_case(rng, L, E, K, P, Nr, mb_sizes, dup_tokens=False, empty_slots=Tr
     return ids, w, mb_off, se, Nb, Ns
 
 
-@pytest.mark.parametrize("seed", range(6))
+@pytest.mark.parametrize("seed", range(8))
 def test_random_small_plans(cuda_device, seed):
     """Random placements with empty slots, same-rank duplicates, empty micro-steps, duplicate ids
-    inside a token, K in {1,2,3,8,10,32}: every integer output equals the oracle."""
+    inside a token, K in {1,2,3,8,10,32,4,6}: every integer output equals the oracle."""
     rng = np.random.default_rng(1000 + seed)
-    K = [1, 2, 3, 8, 10, 32][seed]
-    E, P, Nr = [8, 16, 12, 64, 40, 64][seed], [2, 4, 3, 8, 5, 4][seed], [1, 2, 3, 2, 4, 0][seed]
+    K = [1, 2, 3, 8, 10, 32, 4, 6][seed]
+    E, P, Nr = [8, 16, 12, 64, 40, 64, 32, 24][seed], [2, 4, 3, 8, 5, 4, 8, 6][seed], [1, 2, 3, 2, 4, 0, 1, 2][seed]
     mb_sizes = [int(v) for v in rng.integers(0, 900, size=7)]
     mb_sizes[2] = 0
     mb_sizes[5] = 1

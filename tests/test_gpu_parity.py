@@ -367,3 +367,44 @@ def test_step_host_matches_device_path(cuda_device):
         buf_ref = orc.gather(ref["perm"][l, a * s.K:b * s.K], xb[a:b], s.K, pair_base=a * s.K)
         y_ref = orc.combine(ref["inv"][l, a:b], w[l, a:b], buf_ref, s.act_dtype, row_base=a * s.K)
         assert (y_h[a:b].numpy().view(np.uint32) == y_ref.view(np.uint32)).all()
+
+
+def test_two_streams_reentrant(cuda_device):
+    """The library is re-entrant per stream: independent instances issued on two non-default streams
+    (each with its own buffers) give the results of the sequential default-stream calls, bit for bit."""
+    cfg = synth.config(2).scaled(L=2, n_samples=12, sample_len=500, H=512, mb_samples=3)
+    ids, w, mb_off, se = G.make_case(cfg)
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    s = sp.shape
+    x = G.activations(cfg, mb_off, range(cfg.n_mb))
+    inst = [(l, i) for l in range(cfg.L) for i in range(cfg.n_mb)]
+    n_max = max(int(mb_off[i + 1] - mb_off[i]) for i in range(cfg.n_mb))
+
+    def bufs():
+        return (torch.zeros((n_max * s.K,), dtype=torch.int32, device=G.DEV),
+                torch.zeros((n_max * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV),
+                torch.zeros((n_max, s.H), dtype=torch.float32, device=G.DEV))
+
+    ref_out = {}
+    perm, buf, y = bufs()
+    for (l, i) in inst:
+        sp.dispatch(l, i, i + 1, x[i], perm, buf)
+        sp.combine(l, i, i + 1, buf, y)
+        torch.cuda.synchronize()
+        ref_out[(l, i)] = (perm.clone(), buf.clone(), y.clone())
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    got = {}
+    torch.cuda.synchronize()
+    for j, st in enumerate(streams):
+        with torch.cuda.stream(st):
+            for (l, i) in inst[j::2]:
+                p_, b_, y_ = bufs()
+                sp.dispatch(l, i, i + 1, x[i], p_, b_)
+                sp.combine(l, i, i + 1, b_, y_)
+                got[(l, i)] = (p_, b_, y_)
+    torch.cuda.synchronize()
+    for key in inst:
+        n = int(mb_off[key[1] + 1] - mb_off[key[1]])
+        for a, b in zip(ref_out[key], got[key]):
+            rows = n * s.K if a.shape[0] == n_max * s.K else n
+            assert torch.equal(a[:rows].view(torch.uint8), b[:rows].view(torch.uint8)), key

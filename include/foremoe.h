@@ -31,6 +31,9 @@
  *    All entry points except foremoe_workspace_bytes / foremoe_version / foremoe_step_host
  *    enqueue work on `stream` (a cudaStream_t passed as void*) and return without synchronising.
  *  - Return value: FOREMOE_OK, or a negative host-detectable error (nothing was enqueued).
+ *  - CUDA graphs: the data-path calls (dispatch, combine, *_bwd) are stream-capturable once each
+ *    kernel variant has been launched eagerly (the first launch queries occupancy and opts into
+ *    large shared memory, which capture does not allow).
  *  - Data-dependent faults cannot be seen without a sync; they are OR-ed into *dev_status
  *    (device int32, may be NULL, never cleared by the library): FOREMOE_FAULT_* bits.  On a
  *    device fault the affected instance's outputs are unspecified, all writes stay in bounds.

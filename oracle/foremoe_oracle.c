@@ -341,7 +341,9 @@ static float bf16_to_float(uint16_t b) {
  * accumulated as acc = fmaf(w, v, acc) from acc = 0.0f with k ascending, fp32 output
  * ("the weighted sum of the selected experts' outputs, where the weights are the
  * corresponding router probabilities"; order / fma / output type = reading 16).
- * act_dtype 0 = bf16 rows, 1 = fp32 rows.
+ * act_dtype 0 = bf16 rows, 1 = fp32 rows.  A pair with inv < 0 (faulted in the plan: its expert id
+ * was out of range or had no host) has no dispatched row: it is skipped, like in O9 / O10
+ * (include/foremoe.h: "pairs with inv < 0 contribute nothing"; reading 38).
  * ------------------------------------------------------------------------------------------ */
 int oracle_combine(int64_t n_tok, int K, int H, int act_dtype, int32_t row_base,
                    const int32_t *inv, const float *w, const void *eo, float *y) {
@@ -349,6 +351,7 @@ int oracle_combine(int64_t n_tok, int K, int H, int act_dtype, int32_t row_base,
     for (int h = 0; h < H; h++) {
       float acc = 0.0f;
       for (int k = 0; k < K; k++) {
+        if (inv[t * K + k] < 0) continue;      /* faulted pair: contributes nothing (as O9 / O10) */
         int64_t row = (int64_t)inv[t * K + k] - row_base;
         float v = act_dtype == 0 ? bf16_to_float(((const uint16_t *)eo)[row * H + h])
                                  : ((const float *)eo)[row * H + h];

@@ -17,25 +17,22 @@ __global__ void __launch_bounds__(256)
 k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb_off, int mb_begin,
                 int mb_end, int K, int row_vec, int n_slices, const int4 *__restrict__ x,
                 int32_t *__restrict__ perm, int4 *__restrict__ buf) {
-  // Before the grid-dependency wait only the plan's own arrays are read (mb_off, inv: written by
-  // foremoe_assign, whose kernels never trigger an early programmatic launch): the index chain of
-  // the first item overlaps the drain of the previous kernel.  x / buf / perm are touched after it.
+  // Nothing in global memory is read before the grid-dependency wait: CUDA guarantees the
+  // predecessor's writes (inv from foremoe_assign, x from the caller's kernel) only after it.
   pdl_launch_dependents();
+  pdl_wait();
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const int lane = threadIdx.x & 31;
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
   const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
   const long long item0 = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  int d_first = -1;
-  if (item0 < n_items && lane < K) d_first = __ldg(inv_l + (rg.t_begin + (int)(item0 / n_slices)) * K + lane);
-  pdl_wait();
   for (long long item = item0; item < n_items; item += warps) {
     const int tl = (int)(item / n_slices);
     const int sl = (int)(item - (long long)tl * n_slices);
     const int p0 = (rg.t_begin + tl) * K;
     int d = -1;
     if (lane < K) {
-      d = item == item0 ? d_first : __ldg(inv_l + p0 + lane);
+      d = __ldg(inv_l + p0 + lane);
       if (d >= 0) d -= rg.row0;
       if (perm && sl == 0 && d >= 0) perm[d] = p0 + lane;
     }

@@ -84,7 +84,44 @@ def check_data_path(sp: runner.StepPlan, ref: dict, x_by_mb, layers, mbs, what: 
             worst = max(worst, float(rel.max()))
             assert rel.max() <= 1e-6, (what, "y", l, i, float(rel.max()))
             assert (y_g.view(np.uint32) == y_ref.view(np.uint32)).all(), (what, "y bits", l, i)
+            # the combine is defined on the experts' OUTPUTS, which differ per k:
+            # with expert_out = buf the K rows of a token are identical and a w_k <-> row mix-up
+            # would go unseen, so every instance is also combined on independent random rows
+            check_combine_random(sp, ref["inv"][l, a:b], w_h[l, a:b], l, i, a, n,
+                                 seed=1000 * l + i, what=what)
     return worst
+
+
+def random_expert_out(n_rows: int, H: int, dtype, seed: int) -> torch.Tensor:
+    """Independent random rows in slot order (a stand-in for the experts' outputs): N(0,1) with a
+    few large / tiny / negative-zero values so that a wrong row, weight or order shows in the bits."""
+    g = torch.Generator(device=DEV).manual_seed(seed)
+    eo = torch.randn((max(n_rows, 1), H), generator=g, device=DEV)
+    u = torch.rand((max(n_rows, 1), H), generator=g, device=DEV)
+    eo = torch.where(u < 0.01, eo * 1e4, eo)
+    eo = torch.where(u > 0.99, eo * 1e-4, eo)
+    eo = torch.where((u > 0.5) & (u < 0.505), torch.full_like(eo, -0.0), eo)
+    return eo.to(dtype).contiguous()
+
+
+def check_combine_random(sp: runner.StepPlan, inv_ref, w_ref, l: int, i: int, a: int, n: int,
+                         seed: int, what: str = "", mb_end=None, eo=None):
+    """foremoe_combine of micro-steps [i, mb_end) of layer l on random expert outputs against O6,
+    bit for bit.  inv_ref / w_ref: the oracle's inv and the weights of tokens [a, a+n)."""
+    s = sp.shape
+    if n == 0:
+        return
+    if eo is None:
+        eo = random_expert_out(n * s.K, s.H, s.act_torch_dtype, seed)
+    y = torch.full((n, s.H), float("nan"), dtype=torch.float32, device=DEV)
+    sp.combine(l, i, i + 1 if mb_end is None else mb_end, eo, y)
+    torch.cuda.synchronize()
+    y_ref = orc.combine(np.asarray(inv_ref).reshape(n, s.K), np.asarray(w_ref).reshape(n, s.K),
+                        to_bits(eo)[:n * s.K], s.act_dtype, row_base=a * s.K)
+    y_g = y.cpu().numpy()
+    bad = np.argwhere(y_g.view(np.uint32) != y_ref.view(np.uint32))
+    assert bad.size == 0, f"{what} combine(random expert_out) l={l} mb={i}: {len(bad)} words differ, " \
+                          f"first at {bad[0]}: gpu {y_g[tuple(bad[0])]} oracle {y_ref[tuple(bad[0])]}"
 
 
 def make_case(cfg: synth.TraceConfig, device: str = "cpu"):
@@ -99,3 +136,37 @@ def make_case(cfg: synth.TraceConfig, device: str = "cpu"):
 def activations(cfg: synth.TraceConfig, mb_off, mbs):
     return {i: synth.gen_activations(cfg, max(int(mb_off[i + 1] - mb_off[i]), 1), i, DEV)
             for i in mbs}
+
+
+def random_case(rng, L, E, K, P, Nr, mb_sizes, dup_tokens=False, empty_slots=True,
+                 same_rank_dup=True, skew=1.0):
+    Nb = E // P
+    Ns = Nb + Nr
+    S = P * Ns
+    T = int(sum(mb_sizes))
+    mb_off = np.concatenate([[0], np.cumsum(mb_sizes)]).astype(np.int32)
+    p = (np.arange(E) + 1.0) ** (-skew)
+    p /= p.sum()
+    ids = np.empty((L, T, K), dtype=np.int32)
+    for l in range(L):
+        perm = rng.permutation(E)
+        if dup_tokens:
+            ids[l] = perm[rng.choice(E, size=(T, K), p=p)]
+        else:
+            g = rng.gumbel(size=(T, E)) + np.log(p)[None, :]
+            ids[l] = perm[np.argsort(-g, axis=1)[:, :K]]
+    w = rng.random((L, T, K), dtype=np.float32)
+    se = np.full((L, S), -1, dtype=np.int32)
+    for l in range(L):
+        base = rng.permutation(E)
+        for r in range(P):
+            se[l, r * Ns:r * Ns + Nb] = base[r * Nb:(r + 1) * Nb]
+            for a in range(Nr):
+                u = rng.random()
+                if empty_slots and u < 0.2:
+                    continue
+                if same_rank_dup and u < 0.35:
+                    se[l, r * Ns + Nb + a] = se[l, r * Ns + rng.integers(Nb)]   # inactive duplicate
+                else:
+                    se[l, r * Ns + Nb + a] = rng.integers(E)
+    return ids, w, mb_off, se, Nb, Ns

@@ -123,6 +123,9 @@ def _oracle_checks(wl, layers, data_mbs):
             rel = np.abs(y_g - y_ref) / np.maximum(np.abs(y_ref), 1e-30)
             assert rel.max() <= 1e-6, ("y", l, i, float(rel.max()))
             assert (y_g.view(np.uint32) == y_ref.view(np.uint32)).all(), ("y bits", l, i)
+            # non-identity expert: independent random rows per k, same launch configuration
+            G.check_combine_random(sp, inv.reshape(n, s.K), w_h[1][a:b], l, i, a, n,
+                                   seed=7000 + 100 * l + i, what=f"cfg{cfg.cfg_id}")
 
 
 def _library_data_checks(wl, instances):

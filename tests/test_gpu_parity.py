@@ -91,38 +91,7 @@ def test_combine_identity_pins_on_gpu(cuda_device):
 
 
 # ------------------------------------------------------------------ edge cases
-def _random_case(rng, L, E, K, P, Nr, mb_sizes, dup_tokens=False, empty_slots=True,
-                 same_rank_dup=True, skew=1.0):
-    Nb = E // P
-    Ns = Nb + Nr
-    S = P * Ns
-    T = int(sum(mb_sizes))
-    mb_off = np.concatenate([[0], np.cumsum(mb_sizes)]).astype(np.int32)
-    p = (np.arange(E) + 1.0) ** (-skew)
-    p /= p.sum()
-    ids = np.empty((L, T, K), dtype=np.int32)
-    for l in range(L):
-        perm = rng.permutation(E)
-        if dup_tokens:
-            ids[l] = perm[rng.choice(E, size=(T, K), p=p)]
-        else:
-            g = rng.gumbel(size=(T, E)) + np.log(p)[None, :]
-            ids[l] = perm[np.argsort(-g, axis=1)[:, :K]]
-    w = rng.random((L, T, K), dtype=np.float32)
-    se = np.full((L, S), -1, dtype=np.int32)
-    for l in range(L):
-        base = rng.permutation(E)
-        for r in range(P):
-            se[l, r * Ns:r * Ns + Nb] = base[r * Nb:(r + 1) * Nb]
-            for a in range(Nr):
-                u = rng.random()
-                if empty_slots and u < 0.2:
-                    continue
-                if same_rank_dup and u < 0.35:
-                    se[l, r * Ns + Nb + a] = se[l, r * Ns + rng.integers(Nb)]   # inactive duplicate
-                else:
-                    se[l, r * Ns + Nb + a] = rng.integers(E)
-    return ids, w, mb_off, se, Nb, Ns
+_random_case = G.random_case
 
 
 @pytest.mark.parametrize("seed", range(8))

@@ -206,6 +206,34 @@ def test_combine_fixed_order_small():
     assert y[0, 0] == np.float32(exact) and exact != 0.0
 
 
+def test_combine_skips_faulted_pairs():
+    """A pair with inv < 0 has no dispatched row (foremoe.h; reading 38): it contributes nothing --
+    the result equals the combine of the remaining pairs alone (same order), whatever the rows hold,
+    and a token without any valid pair gives exactly 0."""
+    rng = np.random.default_rng(8)
+    n, K, H = 50, 4, 24
+    eo = rng.standard_normal((n * K, H)).astype(np.float32)
+    eo[7] = np.nan                                       # no pair maps here
+    inv = rng.permutation(n * K).astype(np.int32).reshape(n, K)
+    w = rng.random((n, K), dtype=np.float32)
+    hit = np.argwhere(inv == 7)[0]
+    inv[hit[0], hit[1]] = -1
+    inv[3, :] = -1
+    inv[5, 0] = -1
+    inv[6, K - 1] = -1
+    y = orc.combine(inv, w, eo, 1)
+    assert np.isfinite(y).all() and (y[3] == 0).all()
+    for t in range(n):
+        keep = [k for k in range(K) if inv[t, k] >= 0]
+        if not keep:
+            continue
+        y_t = orc.combine(inv[t:t + 1, keep], w[t:t + 1, keep], eo, 1)
+        assert (y_t[0].view(np.uint32) == y[t].view(np.uint32)).all()
+    # with a row base: layer-global rows, the -1 marker is not shifted
+    y2 = orc.combine(np.where(inv >= 0, inv + 400, -1).astype(np.int32), w, eo, 1, row_base=400)
+    assert (y2.view(np.uint32) == y.view(np.uint32)).all()
+
+
 # ------------------------------------------------------------------ workload sanity (context)
 def test_balance_improves_on_natural_placement(qwen_small):
     """Not parity: the synthetic trace is skewed, and the planned assignment is near-balanced

@@ -25,15 +25,22 @@
  * General rules
  *  - Every data pointer is a DEVICE pointer owned by the caller unless the argument is marked
  *    "host".  The foremoe_shape_t pointer is a host pointer, read during the call only.
- *  - The library allocates no device memory and is re-entrant per stream.  Its only process state
- *    is a set of memoised launch facts (SM count, occupancy, shared-memory opt-in), keyed by the
- *    current device and refilled when it changes, and the sweep-only tuning at the end of this file.
- *    All entry points except foremoe_workspace_bytes / foremoe_version / foremoe_step_host
- *    enqueue work on `stream` (a cudaStream_t passed as void*) and return without synchronising.
+ *  - The library allocates no device memory, keeps no tunable global state and is re-entrant: any
+ *    number of host threads may drive any number of streams and devices concurrently.  Its only
+ *    process state is a lock-free memo of launch facts (SM count, occupancy, shared-memory opt-in)
+ *    per device and kernel variant, filled on first use or by foremoe_warmup.
+ *    All entry points except foremoe_workspace_bytes / foremoe_version / foremoe_warmup /
+ *    foremoe_step_host enqueue work on `stream` (a cudaStream_t passed as void*) and return without
+ *    synchronising.
  *  - Return value: FOREMOE_OK, or a negative host-detectable error (nothing was enqueued).
- *  - CUDA graphs: the data-path calls (dispatch, combine, *_bwd) are stream-capturable once each
- *    kernel variant has been launched eagerly (the first launch queries occupancy and opts into
- *    large shared memory, which capture does not allow).
+ *  - Stream order is the only ordering the data-path calls need: their kernels are launched with
+ *    programmatic stream serialisation and read nothing from global memory before the grid
+ *    dependency is resolved, so inputs written by the preceding kernel of the stream (inv by
+ *    foremoe_assign, x / expert_out / w by the caller's kernels) are always seen complete.
+ *  - CUDA graphs: the data-path calls (dispatch, combine, *_bwd) are stream-capturable.  The first
+ *    launch of a kernel variant on a device queries occupancy and opts into large shared memory,
+ *    which capture does not allow: call foremoe_warmup(shape) once per shape and device before
+ *    capturing (or run the calls once eagerly).
  *  - Data-dependent faults cannot be seen without a sync; they are OR-ed into *dev_status
  *    (device int32, may be NULL, never cleared by the library): FOREMOE_FAULT_* bits.  On a
  *    device fault the affected instance's outputs are unspecified, all writes stay in bounds.
@@ -83,6 +90,16 @@ int foremoe_version(void);
 
 /* Bytes of device scratch foremoe_assign needs for this shape.  Host only, no CUDA call. */
 int foremoe_workspace_bytes(const foremoe_shape_t *shape, size_t *bytes /* host, out */);
+
+/*
+ * Prepares every data-path kernel variant this shape selects (dispatch, combine, combine_bwd with and
+ * without dw, dispatch_bwd) on the calling thread's current device: opts them into large shared
+ * memory and memoises their occupancy.  Launches nothing and does not synchronise; `stream` is
+ * accepted for symmetry and ignored.  After it, the data-path calls for this shape issue no CUDA
+ * call other than the kernel launch, so the very first one may already be stream-captured.
+ * Optional otherwise: every call prepares its own variant on first use.
+ */
+int foremoe_warmup(const foremoe_shape_t *shape, void *stream);
 
 /*
  * (a1) Load histogram -- w_{s,e} with the single source rank and its step
@@ -339,20 +356,6 @@ int foremoe_step_host(const foremoe_shape_t *shape, const int32_t *ids_h, const 
                       const int32_t *mb_off_h, const int32_t *slot_expert_h, const void *x_h,
                       int32_t *quota_h, int32_t *rank_load_h, int32_t *slot_off_h, float *y_h,
                       void *arena, size_t arena_bytes, int32_t *status_h, void *stream);
-
-/*
- * Sweeps only (paper_2606_11867_b200/tune.py; profiles/r01_sweeps.md, r01_hist.md, r01_backward.md):
- * process-wide launch parameters of the data-path kernels and the histogram variant.  They select
- * among kernels that compute bit-identical results; not part of the product contract, not
- * thread-safe, defaults are restored by passing the default values again.
- *   foremoe_debug_set_tuning: key = index into {dispatch_impl, dispatch_u, dispatch_cta_per_sm,
- *     dispatch_stages, dispatch_warps, combine_impl, combine_u, combine_cta_per_sm, combine_depth,
- *     combine_threads, pdl, bwd_depth, bwd_cta_per_sm}; unknown keys are ignored.
- *   foremoe_debug_set_hist_variant: 0 = 4-byte loads, 1 = warp-aggregated (match.any), 2 = 16-byte
- *     loads (default).
- */
-void foremoe_debug_set_tuning(int key, int value);
-void foremoe_debug_set_hist_variant(int variant);
 
 #ifdef __cplusplus
 }

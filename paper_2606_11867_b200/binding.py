@@ -35,7 +35,7 @@ FAULT_SOURCE = 32
 ACT_BF16 = 0
 ACT_FP32 = 1
 
-EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_load_hist", "foremoe_assign",
+EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_warmup", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
            "foremoe_swap_relocation", "foremoe_replication",
@@ -114,6 +114,7 @@ def lib() -> C.CDLL:
         l.foremoe_version.restype = C.c_int
         l.foremoe_version.argtypes = []
         l.foremoe_workspace_bytes.argtypes = [sp, C.POINTER(sz)]
+        l.foremoe_warmup.argtypes = [sp, vp]
         l.foremoe_load_hist.argtypes = [sp, vp, vp, vp, vp, vp, vp]
         l.foremoe_assign.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
         l.foremoe_dispatch.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
@@ -182,6 +183,12 @@ def workspace_bytes(shape: Shape) -> int:
     out = C.c_size_t(0)
     _check("foremoe_workspace_bytes", lib().foremoe_workspace_bytes(C.byref(shape.c()), C.byref(out)))
     return out.value
+
+
+def warmup(shape: Shape) -> None:
+    """Prepare every data-path kernel variant of this shape on the current device (no launch): after
+    it the data-path calls can be captured into a CUDA graph from the first call on."""
+    _check("foremoe_warmup", lib().foremoe_warmup(C.byref(shape.c()), _stream()))
 
 
 def load_hist(shape: Shape, ids, mb_off, hist, step_hist=None, dev_status=None) -> None:

@@ -1,7 +1,7 @@
 """Build paper_2606_11867_b200/libforemoe.so (the C-ABI library of include/foremoe.h) with nvcc for
 sm_100a.  In-tree on purpose: the built .so travels to the GPU box with the repo snapshot.
 
-    python -m paper_2606_11867_b200.build [--force]
+    python -m paper_2606_11867_b200.build [--force] [-v] [--tuning]
 """
 from __future__ import annotations
 
@@ -32,16 +32,29 @@ def _stale() -> bool:
     return any(os.path.getmtime(p) > t for p in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every .cu under csrc/ into libforemoe.so; returns its path."""
+LIB_TUNING = os.path.join(HERE, "libforemoe_tuning.so")
+
+
+def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> str:
+    """Compile every .cu under csrc/ into libforemoe.so; returns its path.
+
+    tuning=True builds libforemoe_tuning.so instead, with -DFOREMOE_TUNING: the same kernels with
+    mutable launch parameters and the extra export foremoe_tuning_set (sweeps only; the binding
+    never loads it)."""
+    if tuning:
+        return _build(LIB_TUNING, "build_tuning", ["-DFOREMOE_TUNING"], verbose)
     if not force and not _stale():
         return LIB
+    return _build(LIB, "build", [], verbose)
+
+
+def _build(LIB: str, objdir: str, extra, verbose: bool) -> str:
     objs = []
     procs = []
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    os.makedirs(os.path.join(HERE, objdir), exist_ok=True)
     for src in sources():
-        obj = os.path.join(HERE, "build", os.path.basename(src)[:-3] + ".o")
-        cmd = [NVCC] + [f for f in FLAGS if f != "-shared"] + ["-c", src, "-o", obj]
+        obj = os.path.join(HERE, objdir, os.path.basename(src)[:-3] + ".o")
+        cmd = [NVCC] + [f for f in FLAGS if f != "-shared"] + list(extra) + ["-c", src, "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((cmd, subprocess.Popen(cmd)))
@@ -57,4 +70,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, tuning="--tuning" in sys.argv))

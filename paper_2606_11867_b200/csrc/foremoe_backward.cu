@@ -196,21 +196,15 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
 template <bool kBf16, int K_T, int D, bool kDw>
 static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const float *w_l, const int32_t *mb_off,
                       int mb_begin, int mb_end, const float *dy, const void *eo, void *d_eo,
-                      float *dw_l, cudaStream_t st) {
+                      float *dw_l, cudaStream_t st, bool prepare) {
   const int NV = (kBf16 ? 2 : 1) + (kDw ? d.K : 0);
   const size_t smem = (size_t)D * NV * threads * 16 + (size_t)(threads / 32) * D * 32 * 8;
   if (smem > 220 * 1024) return FOREMOE_ERR_INVALID_ARG;
   auto kern = k_combine_bwd<kBf16, K_T, D, kDw>;
-  static int occ = 0, cached_dev = -1;
-  static size_t occ_key = 0;
-  if (cache_stale(&cached_dev)) {
-    occ = 0;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) {
-      cached_dev = -1;
-      return FOREMOE_ERR_CUDA;
-    }
-  }
-  if (!occ || occ_key != smem * 1024 + threads) { occ = occupancy_ctas(kern, threads, smem); occ_key = smem * 1024 + threads; }
+  static DeviceMemo memo;
+  const int occ = launch_facts(kern, memo, threads, smem);
+  if (!occ) return FOREMOE_ERR_CUDA;
+  if (prepare) return FOREMOE_OK;
   // oversubscribed grid: 8-16 CTAs per SM (32 without the eo reads) although only `occ` are resident --
   // fresh CTAs streaming in balance the tail and run 5-9 % faster than a strictly persistent grid
   // (sweep: profiles/r01_backward.md), the same effect as on the dispatch store path
@@ -228,15 +222,16 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
+#define FOREMOE_ARGS d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st, prepare
+
 template <bool kBf16, int K_T, bool kDw>
 static int launch_depth(int D, const Dims &d, int threads, const int32_t *inv_l, const float *w_l,
                         const int32_t *mb_off, int mb_begin, int mb_end, const float *dy,
-                        const void *eo, void *d_eo, float *dw_l, cudaStream_t st) {
+                        const void *eo, void *d_eo, float *dw_l, cudaStream_t st, bool prepare) {
   switch (D) {
-    case 2: return launch_one<kBf16, K_T, 2, kDw>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 3: return launch_one<kBf16, K_T, 3, kDw>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 4: return launch_one<kBf16, K_T, 4, kDw>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 8: return launch_one<kBf16, K_T, 8, kDw>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
+    case 2: return launch_one<kBf16, K_T, 2, kDw>(FOREMOE_ARGS);
+    case 3: return launch_one<kBf16, K_T, 3, kDw>(FOREMOE_ARGS);
+    case 4: return launch_one<kBf16, K_T, 4, kDw>(FOREMOE_ARGS);
   }
   return FOREMOE_ERR_INVALID_ARG;
 }
@@ -244,16 +239,35 @@ static int launch_depth(int D, const Dims &d, int threads, const int32_t *inv_l,
 template <bool kBf16, bool kDw>
 static int launch_k(int D, const Dims &d, int threads, const int32_t *inv_l, const float *w_l,
                     const int32_t *mb_off, int mb_begin, int mb_end, const float *dy, const void *eo,
-                    void *d_eo, float *dw_l, cudaStream_t st) {
+                    void *d_eo, float *dw_l, cudaStream_t st, bool prepare) {
   switch (d.K) {
-    case 2: return launch_depth<kBf16, 2, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 4: return launch_depth<kBf16, 4, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 6: return launch_depth<kBf16, 6, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 8: return launch_depth<kBf16, 8, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
-    case 10: return launch_depth<kBf16, 10, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
+    case 2: return launch_depth<kBf16, 2, kDw>(D, FOREMOE_ARGS);
+    case 4: return launch_depth<kBf16, 4, kDw>(D, FOREMOE_ARGS);
+    case 6: return launch_depth<kBf16, 6, kDw>(D, FOREMOE_ARGS);
+    case 8: return launch_depth<kBf16, 8, kDw>(D, FOREMOE_ARGS);
+    case 10: return launch_depth<kBf16, 10, kDw>(D, FOREMOE_ARGS);
   }
-  return launch_depth<kBf16, 0, kDw>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, dy, eo, d_eo, dw_l, st);
+  return launch_depth<kBf16, 0, kDw>(D, FOREMOE_ARGS);
 }
+
+int combine_bwd_rows(const Dims &d, const int32_t *inv_l, const float *w_l, const int32_t *mb_off,
+                     int mb_begin, int mb_end, const float *dy, const void *eo, void *d_eo, float *dw_l,
+                     cudaStream_t st, bool want_dw, bool prepare) {
+  const int NV = (d.act_dtype == FOREMOE_ACT_BF16 ? 2 : 1) + (want_dw ? d.K : 0);
+  // same sizing as k_combine_async: D = 3 stages, about 120 KB in flight per CTA (K = 8: 256 threads,
+  // K = 10: 192); without the eo reads only the dy slices are staged and 2 stages of 256 threads do
+  int D = g_tune.bwd_depth > 0 ? g_tune.bwd_depth : (want_dw ? 3 : 2);
+  int threads = want_dw ? (int)(120 * 1024 / ((size_t)D * NV * 16)) / 32 * 32 : 256;
+  threads = threads < 32 ? 32 : threads > 256 ? 256 : threads;
+  if (threads > 64) threads = threads / 64 * 64;
+  while (D > 2 && (size_t)D * NV * threads * 16 > 200 * 1024) D--;
+  const bool bf = d.act_dtype == FOREMOE_ACT_BF16;
+  if (bf && want_dw) return launch_k<true, true>(D, FOREMOE_ARGS);
+  if (bf) return launch_k<true, false>(D, FOREMOE_ARGS);
+  if (want_dw) return launch_k<false, true>(D, FOREMOE_ARGS);
+  return launch_k<false, false>(D, FOREMOE_ARGS);
+}
+#undef FOREMOE_ARGS
 
 }  // namespace foremoe
 
@@ -275,20 +289,6 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine_bwd(
   if (dw && !expert_out) return FOREMOE_ERR_INVALID_ARG;       // dw needs the forward expert outputs
   if (mb_begin == mb_end) return FOREMOE_OK;
   const size_t lo = (size_t)layer * d.T * d.K;
-  const bool want_dw = dw != nullptr;
-  float *dw_l = want_dw ? dw + lo : nullptr;
-  cudaStream_t st = (cudaStream_t)stream;
-  const int NV = (d.act_dtype == FOREMOE_ACT_BF16 ? 2 : 1) + (want_dw ? d.K : 0);
-  // same sizing as k_combine_async: D = 3 stages, about 120 KB in flight per CTA (K = 8: 256 threads,
-  // K = 10: 192); without the eo reads only the dy slices are staged and 2 stages of 256 threads do
-  int D = g_tune.bwd_depth > 0 ? g_tune.bwd_depth : (want_dw ? 3 : 2);
-  int threads = want_dw ? (int)(120 * 1024 / ((size_t)D * NV * 16)) / 32 * 32 : 256;
-  threads = threads < 32 ? 32 : threads > 256 ? 256 : threads;
-  if (threads > 64) threads = threads / 64 * 64;
-  while (D > 2 && (size_t)D * NV * threads * 16 > 200 * 1024) D--;
-  const bool bf = d.act_dtype == FOREMOE_ACT_BF16;
-  if (bf && want_dw) return launch_k<true, true>(D, d, threads, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out, dw_l, st);
-  if (bf) return launch_k<true, false>(D, d, threads, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out, dw_l, st);
-  if (want_dw) return launch_k<false, true>(D, d, threads, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out, dw_l, st);
-  return launch_k<false, false>(D, d, threads, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out, dw_l, st);
+  return combine_bwd_rows(d, inv + lo, w + lo, mb_off, mb_begin, mb_end, dy, expert_out, d_expert_out,
+                          dw ? dw + lo : nullptr, (cudaStream_t)stream, dw != nullptr, false);
 }

@@ -160,20 +160,14 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
 template <bool kBf16, int K_T, int D>
 static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const float *w_l,
                       const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
-                      cudaStream_t st) {
+                      cudaStream_t st, bool prepare) {
   const size_t smem = (size_t)D * d.K * threads * 16 + (size_t)(threads / 32) * D * 32 * 4;
   if (smem > 220 * 1024) return FOREMOE_ERR_INVALID_ARG;
-  static int occ = 0, cached_dev = -1;
-  static size_t occ_key = 0;
   auto kern = k_combine_async<kBf16, K_T, D>;
-  if (cache_stale(&cached_dev)) {
-    occ = 0;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) {
-      cached_dev = -1;
-      return FOREMOE_ERR_CUDA;
-    }
-  }
-  if (!occ || occ_key != smem * 1024 + threads) { occ = occupancy_ctas(kern, threads, smem); occ_key = smem * 1024 + threads; }
+  static DeviceMemo memo;
+  const int occ = launch_facts(kern, memo, threads, smem);
+  if (!occ) return FOREMOE_ERR_CUDA;
+  if (prepare) return FOREMOE_OK;
   const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 31) / 32;
   const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, threads, smem, st, inv_l, w_l, mb_off,
@@ -182,16 +176,16 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
+#define FOREMOE_ARGS d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare
+
 template <bool kBf16, int K_T>
 static int launch_depth(int D, const Dims &d, int threads, const int32_t *inv_l, const float *w_l,
                         const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
-                        cudaStream_t st) {
+                        cudaStream_t st, bool prepare) {
   switch (D) {
-    case 2: return launch_one<kBf16, K_T, 2>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 3: return launch_one<kBf16, K_T, 3>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 4: return launch_one<kBf16, K_T, 4>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 6: return launch_one<kBf16, K_T, 6>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 8: return launch_one<kBf16, K_T, 8>(d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+    case 2: return launch_one<kBf16, K_T, 2>(FOREMOE_ARGS);
+    case 3: return launch_one<kBf16, K_T, 3>(FOREMOE_ARGS);
+    case 4: return launch_one<kBf16, K_T, 4>(FOREMOE_ARGS);
   }
   return FOREMOE_ERR_INVALID_ARG;
 }
@@ -199,20 +193,20 @@ static int launch_depth(int D, const Dims &d, int threads, const int32_t *inv_l,
 template <bool kBf16>
 static int launch_k(int D, const Dims &d, int threads, const int32_t *inv_l, const float *w_l,
                     const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
-                    cudaStream_t st) {
+                    cudaStream_t st, bool prepare) {
   switch (d.K) {
-    case 2: return launch_depth<kBf16, 2>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 4: return launch_depth<kBf16, 4>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 6: return launch_depth<kBf16, 6>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 8: return launch_depth<kBf16, 8>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-    case 10: return launch_depth<kBf16, 10>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+    case 2: return launch_depth<kBf16, 2>(D, FOREMOE_ARGS);
+    case 4: return launch_depth<kBf16, 4>(D, FOREMOE_ARGS);
+    case 6: return launch_depth<kBf16, 6>(D, FOREMOE_ARGS);
+    case 8: return launch_depth<kBf16, 8>(D, FOREMOE_ARGS);
+    case 10: return launch_depth<kBf16, 10>(D, FOREMOE_ARGS);
   }
-  return launch_depth<kBf16, 0>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+  return launch_depth<kBf16, 0>(D, FOREMOE_ARGS);
 }
 
 int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
                          const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
-                         cudaStream_t st) {
+                         cudaStream_t st, bool prepare) {
   // One CTA per SM, D = 3 stages, about 120 KB of rows in flight: threads = the multiple of 64 with
   // 3 * K * threads * 16 <= 120 KB (K = 8: 320 threads, K = 10: 256).  With the lean instruction
   // stream the kernel is latency-bound, and three shallow stages beat two wide ones on every shape
@@ -226,9 +220,9 @@ int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
     D = 3;
     if ((size_t)D * d.K * threads * 16 > 200 * 1024) D = 2;      // K = 32 with 64 threads: 96 KB, fits
   }
-  if (d.act_dtype == FOREMOE_ACT_BF16)
-    return launch_k<true>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-  return launch_k<false>(D, d, threads, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+  if (d.act_dtype == FOREMOE_ACT_BF16) return launch_k<true>(D, FOREMOE_ARGS);
+  return launch_k<false>(D, FOREMOE_ARGS);
 }
+#undef FOREMOE_ARGS
 
 }  // namespace foremoe

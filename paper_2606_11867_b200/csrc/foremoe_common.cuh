@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+
 #include "../../include/foremoe.h"
 
 namespace foremoe {
@@ -102,16 +104,32 @@ __device__ __forceinline__ int find_range(const int32_t *__restrict__ off, int n
 
 int num_sms();
 
-// The launchers memoise per-kernel launch facts (occupancy, the opt-in shared-memory attribute).
-// Both are per DEVICE: a cache remembers the device it was filled on and is refilled when the
-// calling thread's current device differs (one process per GPU is the normal case; this keeps a
-// process that drives several devices correct).  Returns true when the cache must be refilled.
-inline bool cache_stale(int *cached_dev) {
+// The launchers memoise per-kernel launch facts (SM count, occupancy, the opt-in shared-memory
+// attribute).  They are per DEVICE and must be safe when several host threads drive several
+// streams or devices at once, so a memo is a small table of atomics indexed by the calling
+// thread's current device: a slot holds 0 (unknown) or (key << 16 | value).  Two threads that miss
+// at the same time compute the same fact twice and store the same word: no lock is needed.
+constexpr int kMaxDevices = 64;
+constexpr int kMemoWays = 4;
+
+inline int current_device() {
   int dev = -1;
-  if (cudaGetDevice(&dev) != cudaSuccess) return true;
-  if (*cached_dev == dev) return false;
-  *cached_dev = dev;
-  return true;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return -1;
+  return dev;
 }
+
+struct DeviceMemo {
+  std::atomic<uint64_t> slot[kMaxDevices][kMemoWays];
+  // value in [1, 65535] or 0 when (dev, key) is not cached; key < 2^47
+  int get(int dev, uint64_t key) const {
+    if (dev < 0) return 0;
+    const uint64_t v = slot[dev][key % kMemoWays].load(std::memory_order_acquire);
+    return (v >> 16) == key + 1 ? (int)(v & 0xffff) : 0;
+  }
+  void put(int dev, uint64_t key, int value) {
+    if (dev >= 0 && value > 0 && value <= 0xffff)
+      slot[dev][key % kMemoWays].store(((key + 1) << 16) | (uint64_t)value, std::memory_order_release);
+  }
+};
 
 }  // namespace foremoe

@@ -150,13 +150,18 @@ k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
 }
 
 // ---- launch configuration -------------------------------------------------------------------------
+#ifdef FOREMOE_TUNING
 DataTuning g_tune;
+#endif
 
 template <int U>
 static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
-                           int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
-  static int occ = 0, cached_dev = -1;
-  if (cache_stale(&cached_dev) || !occ) occ = occupancy_ctas(k_dispatch_rows<U>, 256);
+                           int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st,
+                           bool prepare) {
+  static DeviceMemo memo;
+  const int occ = launch_facts(k_dispatch_rows<U>, memo, 256, 0);
+  if (!occ) return FOREMOE_ERR_CUDA;
+  if (prepare) return FOREMOE_OK;
   // Oversubscribed grid, about one (token, slice) item per warp although only `occ` CTAs are
   // resident per SM: the store path runs ~10 % faster with fresh CTAs streaming in than with a
   // strictly persistent grid (profiles/r01_sweeps.md).  The item count of a launch is estimated
@@ -179,9 +184,11 @@ static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *m
 template <bool kBf16, int KB, int U>
 static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
                           const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
-                          cudaStream_t st) {
-  static int occ = 0, cached_dev = -1;
-  if (cache_stale(&cached_dev) || !occ) occ = occupancy_ctas(k_combine_rows<kBf16, KB, U>, 256);
+                          cudaStream_t st, bool prepare) {
+  static DeviceMemo memo;
+  const int occ = launch_facts(k_combine_rows<kBf16, KB, U>, memo, 256, 0);
+  if (!occ) return FOREMOE_ERR_CUDA;
+  if (prepare) return FOREMOE_OK;
   const int per_sm = g_tune.combine_cta_per_sm > 0 ? g_tune.combine_cta_per_sm : occ;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   const cudaError_t e = launch_pdl(k_combine_rows<kBf16, KB, U>, num_sms() * per_sm, 256, 0, st, inv_l,
@@ -193,17 +200,17 @@ static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
 template <bool kBf16, int KB>
 static int launch_combine_u(int U, const Dims &d, const int32_t *inv_l, const float *w_l,
                             const int32_t *mb_off, int mb_begin, int mb_end, const void *eo,
-                            float *y, cudaStream_t st) {
-  if (U >= 2) return launch_combine<kBf16, KB, 2>(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
-  return launch_combine<kBf16, KB, 1>(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+                            float *y, cudaStream_t st, bool prepare) {
+  if (U >= 2) return launch_combine<kBf16, KB, 2>(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+  return launch_combine<kBf16, KB, 1>(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
 }
 
 template <bool kBf16>
 static int launch_combine_kb(int KB, int U, const Dims &d, const int32_t *inv_l, const float *w_l,
                              const int32_t *mb_off, int mb_begin, int mb_end, const void *eo,
-                             float *y, cudaStream_t st) {
+                             float *y, cudaStream_t st, bool prepare) {
 #define FOREMOE_KB_CASE(n) \
-  case n: return launch_combine_u<kBf16, n>(U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st);
+  case n: return launch_combine_u<kBf16, n>(U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
   switch (KB) {
     FOREMOE_KB_CASE(1) FOREMOE_KB_CASE(2) FOREMOE_KB_CASE(3) FOREMOE_KB_CASE(4)
     FOREMOE_KB_CASE(5) FOREMOE_KB_CASE(6) FOREMOE_KB_CASE(7) FOREMOE_KB_CASE(8)
@@ -218,18 +225,59 @@ static int check_range(const Dims &d, int layer, int mb_begin, int mb_end) {
   return FOREMOE_OK;
 }
 
+// a4 + a5: selects the kernel variant of the shape and launches it (prepare: memoises its launch
+// facts instead)
+int dispatch_rows(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
+                  int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st, bool prepare) {
+  if (g_tune.dispatch_impl == 1) {   // default (-1, 0): register-staged rows
+    const int rc = launch_dispatch_tma(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
+    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
+  }
+  int U = g_tune.dispatch_u;
+  if (U <= 0) U = d.row_vec >= 64 ? 2 : 1;      // 1 KB slices: best or within 1 % of best on every config (sweep)
+  if (U >= 8) return launch_dispatch<8>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
+  if (U >= 4) return launch_dispatch<4>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
+  if (U >= 2) return launch_dispatch<2>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
+  return launch_dispatch<1>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
+}
+
+// a6 and its unit-weight form (w_l == nullptr sums the K rows: fma(1, v, acc) = acc + v exactly)
+int combine_rows(const Dims &d, const int32_t *inv_l, const float *w_l, const int32_t *mb_off,
+                 int mb_begin, int mb_end, const void *eo, float *y, cudaStream_t st, bool prepare) {
+  int rc;
+  if (g_tune.combine_impl < 0 || g_tune.combine_impl == 2) {   // default: bulk-copy ring
+    rc = launch_combine_bulk(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;
+  }
+  if (g_tune.combine_impl != 0) {    // cp.async ring
+    rc = launch_combine_async(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;
+  }
+  const int groups = (d.K + 7) / 8;
+  const int KB = (d.K + groups - 1) / groups;
+  int U = g_tune.combine_u;
+  if (U <= 0) U = (d.row_vec >= 64 && KB <= 4) ? 2 : 1;
+  if (d.act_dtype == FOREMOE_ACT_BF16)
+    return launch_combine_kb<true>(KB, U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+  return launch_combine_kb<false>(KB, U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+}
+
 }  // namespace foremoe
 
 using namespace foremoe;
 
-// sweeps only: key = field index of DataTuning in declaration order
-extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_tuning(int key, int value) {
+#ifdef FOREMOE_TUNING
+// sweep builds only (not declared in include/foremoe.h): key = field index of DataTuning in
+// declaration order
+extern "C" __attribute__((visibility("default"))) void foremoe_tuning_set(int key, int value) {
   int *f[] = {&g_tune.dispatch_impl, &g_tune.dispatch_u, &g_tune.dispatch_cta_per_sm,
               &g_tune.dispatch_stages, &g_tune.dispatch_warps, &g_tune.combine_impl,
               &g_tune.combine_u, &g_tune.combine_cta_per_sm, &g_tune.combine_depth,
-              &g_tune.combine_threads, &g_tune.pdl, &g_tune.bwd_depth, &g_tune.bwd_cta_per_sm};
+              &g_tune.combine_threads, &g_tune.pdl, &g_tune.bwd_depth, &g_tune.bwd_cta_per_sm,
+              &g_tune.bwd_impl, &g_tune.hist_variant};
   if (key >= 0 && key < (int)(sizeof(f) / sizeof(f[0]))) *f[key] = value;
 }
+#endif
 
 extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
                                 int32_t mb_end, const int32_t *mb_off, const int32_t *inv,
@@ -243,21 +291,10 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const for
   if (!mb_off || !inv || !x || !buf || !aligned(x, 16) || !aligned(buf, 16))
     return FOREMOE_ERR_INVALID_ARG;
   if (mb_begin == mb_end) return FOREMOE_OK;
-  const int32_t *inv_l = inv + (size_t)layer * d.T * d.K;
-  cudaStream_t st = (cudaStream_t)stream;
-  if (g_tune.dispatch_impl == 1) {   // default (-1, 0): register-staged rows
-    rc = launch_dispatch_tma(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
-    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
-  }
-  int U = g_tune.dispatch_u;
-  if (U <= 0) U = d.row_vec >= 64 ? 2 : 1;      // 1 KB slices: best or within 1 % of best on every config (sweep)
-  if (U >= 8) return launch_dispatch<8>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
-  if (U >= 4) return launch_dispatch<4>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
-  if (U >= 2) return launch_dispatch<2>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
-  return launch_dispatch<1>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st);
+  return dispatch_rows(d, inv + (size_t)layer * d.T * d.K, mb_off, mb_begin, mb_end, x, perm, buf,
+                       (cudaStream_t)stream, false);
 }
 
-// a6 and its unit-weight form: w == nullptr sums the K rows (fma(1, v, acc) = acc + v exactly)
 static int combine_entry(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
                          int32_t mb_end, const int32_t *mb_off, const int32_t *inv, const float *w,
                          const void *expert_out, float *y, void *stream) {
@@ -269,19 +306,8 @@ static int combine_entry(const foremoe_shape_t *shape, int32_t layer, int32_t mb
     return FOREMOE_ERR_INVALID_ARG;
   if (mb_begin == mb_end) return FOREMOE_OK;
   const size_t lo = (size_t)layer * d.T * d.K;
-  const float *w_l = w ? w + lo : nullptr;
-  cudaStream_t st = (cudaStream_t)stream;
-  if (g_tune.combine_impl != 0) {    // default: cp.async shared-memory ring
-    rc = launch_combine_async(d, inv + lo, w_l, mb_off, mb_begin, mb_end, expert_out, y, st);
-    if (rc != FOREMOE_ERR_INVALID_ARG) return rc;
-  }
-  const int groups = (d.K + 7) / 8;
-  const int KB = (d.K + groups - 1) / groups;
-  int U = g_tune.combine_u;
-  if (U <= 0) U = (d.row_vec >= 64 && KB <= 4) ? 2 : 1;
-  if (d.act_dtype == FOREMOE_ACT_BF16)
-    return launch_combine_kb<true>(KB, U, d, inv + lo, w_l, mb_off, mb_begin, mb_end, expert_out, y, st);
-  return launch_combine_kb<false>(KB, U, d, inv + lo, w_l, mb_off, mb_begin, mb_end, expert_out, y, st);
+  return combine_rows(d, inv + lo, w ? w + lo : nullptr, mb_off, mb_begin, mb_end, expert_out, y,
+                      (cudaStream_t)stream, false);
 }
 
 extern "C" __attribute__((visibility("default"))) int foremoe_combine(const foremoe_shape_t *shape, int32_t layer, int32_t mb_begin,
@@ -298,4 +324,20 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch_bwd(const
                                     const void *d_buf, float *dx, int32_t *dev_status, void *stream) {
   (void)dev_status;
   return combine_entry(shape, layer, mb_begin, mb_end, mb_off, inv, nullptr, d_buf, dx, stream);
+}
+
+// Memoises the launch facts (occupancy, shared-memory opt-in) of every data-path kernel variant this
+// shape selects, on the calling thread's current device: after it the data-path calls make no CUDA
+// call other than the launch, so they can be stream-captured from the first call on.
+extern "C" __attribute__((visibility("default"))) int foremoe_warmup(const foremoe_shape_t *shape, void *stream) {
+  (void)stream;
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if ((rc = dispatch_rows(d, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, nullptr, true))) return rc;
+  if ((rc = combine_rows(d, nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, true))) return rc;
+  if ((rc = combine_bwd_rows(d, nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, true, true))) return rc;
+  if ((rc = combine_bwd_rows(d, nullptr, nullptr, nullptr, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr, false, true))) return rc;
+  num_sms();
+  return FOREMOE_OK;
 }

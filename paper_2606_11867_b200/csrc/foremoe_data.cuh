@@ -5,24 +5,32 @@
 
 namespace foremoe {
 
-// Tunables of the data path (defaults chosen from the ncu evidence under profiles/; the debug
-// setter exists for sweeps only).
+// Launch parameters of the data path.  In the product build they are compile-time defaults (chosen
+// from the ncu evidence under profiles/) and nothing can change them; a sweep build
+// (python -m paper_2606_11867_b200.build --tuning: -DFOREMOE_TUNING, a separate libforemoe_tuning.so)
+// makes them mutable through foremoe_tuning_set, which is not part of include/foremoe.h.
 struct DataTuning {
   int dispatch_impl = -1;        // -1 auto, 0 = register-staged LSU rows, 1 = TMA bulk-copy ring
   int dispatch_u = 0;            // impl 0: 16-byte vectors per lane per item (0 = auto)
-  int dispatch_cta_per_sm = 0;   // 0 = occupancy
+  int dispatch_cta_per_sm = 0;   // 0 = auto
   int dispatch_stages = 0;       // impl 1: ring stages per warp (0 = auto)
   int dispatch_warps = 0;        // impl 1: warps per CTA (0 = auto)
-  int combine_impl = -1;         // -1 auto, 0 = register-staged LSU rows, 1 = cp.async smem ring
-  int combine_u = 0;             // impl 0
+  int combine_impl = -1;         // -1 auto, 0 = register-staged LSU rows, 1 = cp.async ring, 2 = bulk-copy ring
+  int combine_u = 0;             // impl 0 / 2: 16-byte vectors per lane per row slice (0 = auto)
   int combine_cta_per_sm = 0;
-  int combine_depth = 0;         // impl 1: stages in flight per thread (0 = auto)
-  int combine_threads = 0;       // impl 1: threads per CTA (0 = auto)
+  int combine_depth = 0;         // impl 1 / 2: stages in flight (0 = auto)
+  int combine_threads = 0;       // impl 1 / 2: threads per CTA (0 = auto)
   int pdl = 1;                   // programmatic dependent launch on the data-path kernels
   int bwd_depth = 0;             // k_combine_bwd: stages in flight per thread (0 = auto)
-  int bwd_cta_per_sm = 0;        // 0 = occupancy
+  int bwd_cta_per_sm = 0;        // 0 = auto
+  int bwd_impl = -1;             // -1 auto, 1 = cp.async ring, 2 = bulk-copy ring
+  int hist_variant = 2;          // k_load_hist: 0 = 4-byte loads, 1 = warp-aggregated, 2 = 16-byte loads
 };
+#ifdef FOREMOE_TUNING
 extern DataTuning g_tune;
+#else
+constexpr DataTuning g_tune{};
+#endif
 
 struct RangeInfo { int t_begin, t_end, row0; };
 
@@ -90,12 +98,78 @@ static int occupancy_ctas(Kern kern, int threads, size_t smem = 0) {
   return n;
 }
 
-// launchers of the asynchronous variants; return FOREMOE_ERR_INVALID_ARG when the shape does not
-// fit the variant (the caller then uses the register-staged kernel)
+constexpr int kSmemOptIn = 227 * 1024;   // largest dynamic shared memory a CTA can opt into on sm_100a
+
+// Resident CTAs per SM (>= 1) of `kern` at (threads, smem) on the calling thread's current device,
+// memoised per device in `memo` (one DeviceMemo per kernel instantiation).  On a miss the kernel is
+// opted into the full shared-memory carve-out (always the same value, so shapes with different
+// footprints cannot undo each other) and the occupancy is queried: neither is allowed during stream
+// capture, which is what foremoe_warmup is for.  Returns 0 on a CUDA error.
+template <typename Kern>
+static int launch_facts(Kern kern, DeviceMemo &memo, int threads, size_t smem) {
+  const int dev = current_device();
+  const uint64_t key = (uint64_t)smem * 2048 + (uint64_t)threads;
+  int occ = memo.get(dev, key);
+  if (occ) return occ;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemOptIn) != cudaSuccess)
+    return 0;
+  occ = occupancy_ctas(kern, threads, smem);
+  memo.put(dev, key, occ);
+  return occ;
+}
+
+// Every launcher takes `prepare`: true = memoise the launch facts of the variant this shape selects
+// and return without launching (foremoe_warmup).
+// launchers of the ring variants; return FOREMOE_ERR_INVALID_ARG when the shape does not fit the
+// variant (the caller then uses the next one)
 int launch_dispatch_tma(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
-                        int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st);
+                        int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st,
+                        bool prepare);
 int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
                          const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
-                         cudaStream_t st);
+                         cudaStream_t st, bool prepare);
+int launch_combine_bulk(const Dims &d, const int32_t *inv_l, const float *w_l,
+                        const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
+                        cudaStream_t st, bool prepare);
+
+// backward of a6 (foremoe_backward.cu): want_dw selects the variant that also reads expert_out
+int combine_bwd_rows(const Dims &d, const int32_t *inv_l, const float *w_l, const int32_t *mb_off,
+                     int mb_begin, int mb_end, const float *dy, const void *eo, void *d_eo, float *dw_l,
+                     cudaStream_t st, bool want_dw, bool prepare);
+
+// mbarrier + bulk-copy (TMA, 1-D) primitives shared by the bulk rings
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}"
+      :: "r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+               :: "l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+// orders generic-proxy accesses to shared memory before later async-proxy (bulk-copy) accesses
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 }  // namespace foremoe

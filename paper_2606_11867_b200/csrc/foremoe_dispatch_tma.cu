@@ -7,37 +7,6 @@
 
 namespace foremoe {
 
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_%=:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra DONE_%=;\n\t"
-      "bra WAIT_%=;\n\t"
-      "DONE_%=:\n\t}"
-      :: "r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void bulk_s2g(void *dst, uint32_t src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-               :: "l"(dst), "r"(src), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() {
-  asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(N) : "memory");
-}
-__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
-
 // smem layout: [warps][NS][row_bytes] rows (16-byte aligned), then [warps][NS] mbarriers (8 B),
 // then [warps][NS][32] destination rows.
 __global__ void __launch_bounds__(512)
@@ -45,8 +14,8 @@ k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb
                int mb_end, int K, int row_bytes, int NS, const char *__restrict__ x,
                int32_t *__restrict__ perm, char *__restrict__ buf) {
   extern __shared__ __align__(128) unsigned char smem[];
-  pdl_wait();
   pdl_launch_dependents();
+  pdl_wait();
   const int n_warps = blockDim.x >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   unsigned char *rows = smem + (size_t)warp * NS * row_bytes;
@@ -99,7 +68,8 @@ k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb
 }
 
 int launch_dispatch_tma(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
-                        int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st) {
+                        int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st,
+                        bool prepare) {
   const size_t budget = 200 * 1024;
   int warps = g_tune.dispatch_warps > 0 ? g_tune.dispatch_warps : (d.row_bytes <= 4096 ? 8 : 4);
   if (warps > 16) warps = 16;
@@ -109,12 +79,9 @@ int launch_dispatch_tma(const Dims &d, const int32_t *inv_l, const int32_t *mb_o
   while (NS >= 3 && per_stage * warps * NS > budget) NS--;
   if (NS < 3) return FOREMOE_ERR_INVALID_ARG;       // rows too large for a ring: caller falls back
   const size_t smem = per_stage * warps * NS;
-  static int cached_dev = -1;
-  if (cache_stale(&cached_dev) &&
-      cudaFuncSetAttribute(k_dispatch_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)budget) != cudaSuccess) {
-    cached_dev = -1;
-    return FOREMOE_ERR_CUDA;
-  }
+  static DeviceMemo memo;
+  if (!launch_facts(k_dispatch_tma, memo, warps * 32, smem)) return FOREMOE_ERR_CUDA;
+  if (prepare) return FOREMOE_OK;
   const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : 1;
   k_dispatch_tma<<<num_sms() * per_sm, warps * 32, smem, st>>>(
       inv_l, mb_off, mb_begin, mb_end, d.K, d.row_bytes, NS, (const char *)x, perm, (char *)buf);

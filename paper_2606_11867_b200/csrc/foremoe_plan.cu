@@ -3,7 +3,7 @@
 // Contract: include/foremoe.h.  Rule and readings: DESIGN.md sec. 3.
 #include <limits.h>
 
-#include "foremoe_common.cuh"
+#include "foremoe_data.cuh"
 
 namespace foremoe {
 
@@ -712,20 +712,18 @@ using namespace foremoe;
 
 namespace foremoe {
 int num_sms() {
-  static int n = 0, cached_dev = -1;
-  if (cache_stale(&cached_dev) || n == 0) {
-    if (cached_dev < 0 ||
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, cached_dev) != cudaSuccess || n <= 0) {
-      n = 0;
-      cached_dev = -1;
-      return 148;
-    }
-  }
+  static DeviceMemo memo;
+  const int dev = current_device();
+  int n = memo.get(dev, 0);
+  if (n) return n;
+  if (dev < 0 || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+    return 148;
+  memo.put(dev, 0, n);
   return n;
 }
 }  // namespace foremoe
 
-extern "C" __attribute__((visibility("default"))) int foremoe_version(void) { return 100; }
+extern "C" __attribute__((visibility("default"))) int foremoe_version(void) { return 200; }
 
 extern "C" __attribute__((visibility("default"))) int foremoe_workspace_bytes(const foremoe_shape_t *shape, size_t *bytes) {
   Dims d;
@@ -735,9 +733,6 @@ extern "C" __attribute__((visibility("default"))) int foremoe_workspace_bytes(co
   *bytes = make_workspace(d).total;
   return FOREMOE_OK;
 }
-
-static int g_hist_variant = 2;   // kMode of k_load_hist (sweeps only)
-extern "C" __attribute__((visibility("default"))) void foremoe_debug_set_hist_variant(int v) { g_hist_variant = v; }
 
 extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const foremoe_shape_t *shape, const int32_t *ids,
                                  const int32_t *mb_off, int32_t *hist, int64_t *step_hist,
@@ -756,10 +751,10 @@ extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const fo
     const long long n_tiles = (long long)tiles_per_layer * d.L;
     const int grid = (int)(n_tiles < (long long)num_sms() * 8 ? n_tiles : (long long)num_sms() * 8);
     const size_t smem = sizeof(int32_t) * d.E;
-    if (g_hist_variant == 1)
+    if (g_tune.hist_variant == 1)
       k_load_hist<1><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
                                               tiles_per_layer, hist, dev_status);
-    else if (g_hist_variant == 0)
+    else if (g_tune.hist_variant == 0)
       k_load_hist<0><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
                                               tiles_per_layer, hist, dev_status);
     else

@@ -38,6 +38,9 @@ def test_exported_symbols_are_exactly_the_declared_ones(libpath):
     out = subprocess.run(["nm", "-D", "--defined-only", libpath], capture_output=True, text=True, check=True).stdout
     exported = {ln.split()[-1] for ln in out.splitlines() if " T " in ln and ln.split()[-1].startswith("foremoe_")}
     assert exported == declared, (exported ^ declared)
+    # the boundary keeps no tunable global state: sweep knobs exist only in the
+    # separate -DFOREMOE_TUNING build, never in the product library or its header
+    assert not [n for n in exported if "debug" in n or "tuning" in n]
 
 
 @pytest.mark.parametrize("lang,std", [("c", "c99"), ("c", "c11"), ("c++", "c++14")])

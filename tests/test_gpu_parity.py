@@ -379,6 +379,121 @@ def test_two_streams_reentrant(cuda_device):
             assert torch.equal(a[:rows].view(torch.uint8), b[:rows].view(torch.uint8)), key
 
 
+def test_two_host_threads_two_streams(cuda_device):
+    """Two HOST threads, each driving its own stream with its own shape (so each needs different
+    kernel variants and launch facts), started together on variants no earlier call has prepared:
+    results equal the sequential ones bit for bit (the launch-fact memo is lock-free and per device)."""
+    import threading
+    cases = []
+    for (H, K, E, P, Nr, seed) in [(1544, 8, 64, 8, 2, 1), (776, 6, 24, 6, 2, 2)]:
+        rng = np.random.default_rng(900 + seed)
+        mb_sizes = [400, 33, 800]
+        ids, w, mb_off, se, Nb, Ns = G.random_case(rng, 2, E, K, P, Nr, mb_sizes)
+        shape = fm.Shape(L=2, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=3, H=H,
+                         act_dtype=fm.ACT_BF16)
+        sp = G.gpu_plan(shape, ids, w, mb_off, se)
+        x = {i: torch.randn((mb_sizes[i], H), device=G.DEV).bfloat16() for i in range(3)}
+        cases.append((sp, mb_sizes, x))
+
+    def run_all(sp, mb_sizes, x, out):
+        s = sp.shape
+        for rep in range(4):
+            for l in range(2):
+                for i in range(3):
+                    n = mb_sizes[i]
+                    perm = torch.empty((n * s.K,), dtype=torch.int32, device=G.DEV)
+                    buf = torch.empty((n * s.K, s.H), dtype=torch.bfloat16, device=G.DEV)
+                    y = torch.empty((n, s.H), dtype=torch.float32, device=G.DEV)
+                    dx = torch.empty((n, s.H), dtype=torch.float32, device=G.DEV)
+                    sp.dispatch(l, i, i + 1, x[i], perm, buf)
+                    sp.combine(l, i, i + 1, buf, y)
+                    sp.dispatch_bwd(l, i, i + 1, buf, dx)
+                    out[(rep, l, i)] = (perm, buf, y, dx)
+
+    errors = []
+
+    def worker(case, out):
+        try:
+            torch.cuda.set_device(0)
+            with torch.cuda.stream(torch.cuda.Stream()):
+                run_all(*case, out)
+                torch.cuda.current_stream().synchronize()
+        except Exception as e:      # surfaced below
+            errors.append(e)
+
+    outs = [dict(), dict()]
+    threads = [threading.Thread(target=worker, args=(c, o)) for c, o in zip(cases, outs)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    torch.cuda.synchronize()
+    for case, got in zip(cases, outs):
+        ref = {}
+        run_all(*case, ref)
+        torch.cuda.synchronize()
+        for key in ref:
+            for a, b in zip(ref[key], got[key]):
+                assert torch.equal(a.view(torch.uint8), b.view(torch.uint8)), key
+        assert case[0].faults() == 0
+
+
+_CAPTURE_FIRST_CALL = r"""
+import sys, numpy as np, torch
+sys.path.insert(0, sys.argv[1])
+from paper_2606_11867_b200 import binding as fm, synth
+from tests import gpu_common as G
+cfg = synth.config(2).scaled(L=1, n_samples=6, sample_len=400, H=512, mb_samples=3)
+ids, w, mb_off, se = G.make_case(cfg)
+sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)      # plan kernels only
+s = sp.shape
+n = int(mb_off[1] - mb_off[0])
+x = synth.gen_activations(cfg, n, 0, G.DEV)
+dy = torch.randn((n, s.H), device=G.DEV)
+mk = lambda: (torch.zeros((n * s.K,), dtype=torch.int32, device=G.DEV),
+              torch.zeros((n * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV),
+              torch.zeros((n, s.H), dtype=torch.float32, device=G.DEV),
+              torch.zeros((n * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV),
+              torch.zeros((n, s.H), dtype=torch.float32, device=G.DEV),
+              torch.zeros((s.L, s.T, s.K), dtype=torch.float32, device=G.DEV),
+              torch.zeros((n * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV))
+def run(b):
+    perm, buf, y, d_buf, dx, dw, d_buf2 = b
+    sp.dispatch(0, 0, 1, x, perm, buf)
+    sp.combine(0, 0, 1, buf, y)
+    sp.combine_bwd(0, 0, 1, dy, buf, d_buf, dw)
+    sp.combine_bwd(0, 0, 1, dy, None, d_buf2, None)
+    sp.dispatch_bwd(0, 0, 1, d_buf, dx)
+fm.warmup(s)                        # no data-path call has run in this process
+graphed = mk()
+torch.cuda.synchronize()
+g = torch.cuda.CUDAGraph()
+with torch.cuda.graph(g):
+    run(graphed)                    # the FIRST data-path calls of the process, under capture
+g.replay()
+torch.cuda.synchronize()
+eager = mk()
+run(eager)
+torch.cuda.synchronize()
+for a, b in zip(eager, graphed):
+    assert torch.equal(a.view(torch.uint8), b.view(torch.uint8))
+assert sp.faults() == 0
+print("capture-first-call ok")
+"""
+
+
+def test_graph_capture_of_first_call_after_warmup(cuda_device):
+    """foremoe_warmup makes the data-path calls capturable from the very first call: a fresh process
+    warms up, captures dispatch + combine + both backward calls without ever running them eagerly,
+    replays, and the results equal the eager calls made afterwards."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _CAPTURE_FIRST_CALL, root], capture_output=True, text=True,
+                       cwd=root, timeout=600)
+    assert r.returncode == 0 and "capture-first-call ok" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])
+
+
 def test_cuda_graph_replay(cuda_device):
     """The data-path calls are capturable into a CUDA graph once each kernel variant has run eagerly
     (the first launch of a variant queries occupancy / opts into large shared memory); the replay

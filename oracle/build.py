@@ -14,7 +14,25 @@ SRC = os.path.join(HERE, "foremoe_oracle.c")
 LIB = os.path.join(HERE, "liboracle_foremoe.so")
 
 
+LIB_SAN = os.path.join(HERE, "liboracle_foremoe_san.so")
+
+
+def build_sanitized() -> str:
+    """The same source with -fsanitize=address,undefined -fno-sanitize-recover:
+    tests/test_oracle_sanitizers.py runs the oracle pins on it in a child process."""
+    cmd = ["gcc", "-O1", "-g", "-std=gnu11", "-fPIC", "-shared", "-ffp-contract=off", "-Wall", "-Wextra",
+           "-fsanitize=address,undefined", "-fno-sanitize-recover=all", "-fno-omit-frame-pointer",
+           "-o", LIB_SAN + ".tmp", SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(LIB_SAN + ".tmp", LIB_SAN)
+    return LIB_SAN
+
+
 def build(force: bool = False) -> str:
+    # FOREMOE_ORACLE_LIB: load this build of the oracle instead (the sanitizer run sets it)
+    override = os.environ.get("FOREMOE_ORACLE_LIB")
+    if override:
+        return override
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB

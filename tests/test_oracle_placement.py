@@ -46,6 +46,72 @@ def test_golden_vector():
         assert f == 0 and out.reshape(g["P"], -1).tolist() == g[key]
 
 
+def test_golden_vector_machines_matter():
+    """Second hand-worked vector: micro-step loads that differ from the step totals, so that M = 2
+    (relocation / replication confined to each machine) gives another placement than M = 1."""
+    g = json.load(open(os.path.join(HERE, "golden", "placement_vectors.json")))
+    v = g["second_vector"]
+    base, f = orc.base_placement(np.array(v["tot"]), g["P"], g["Nb"], g["Nr"])
+    assert f == 0 and base.reshape(g["P"], -1).tolist() == g["base"]
+    c = np.array(v["c_mb"], dtype=np.int32)
+    outs = {}
+    for M in (1, 2):
+        out, f = orc.microstep_placement(c, base, g["P"], g["Nb"], g["Nr"], M)
+        assert f == 0 and out.reshape(g["P"], -1).tolist() == v[f"microstep_M{M}"], M
+        outs[M] = out
+        _replay_stage3(c, out, g["P"], g["Nb"], g["Nr"], M)
+    assert (outs[1] != outs[2]).any()
+
+
+def _replay_stage3(c, out, P, Nb, Nr, M):
+    """Re-derive every replication round of Alg. 3 Stage 3 (readings 22-25)
+    from the OUTPUT alone, independently of the oracle's bookkeeping: the base slots of `out` are the
+    Stage-2 result; round by round the expected (expert, rank) is recomputed from scratch -- the locally
+    heaviest expert PER COPY (exact fractions, ties lower id) among those that still have an eligible
+    rank, on the least-loaded local rank with a free redundant slot that does not host it (ties lowest
+    rank), rank loads = sum over experts of the exact integer even split (first c mod n hosts in
+    ascending slot index carry one more) -- and must be what `out` holds in that rank's next redundant
+    slot.  Slots no round fills must be -1."""
+    from fractions import Fraction
+    Ns, R, E = Nb + Nr, P // M, len(c)
+    se = np.asarray(out).reshape(P, Ns)
+    hosts = {e: [] for e in range(E)}                   # global slot indices, base slots first
+    for r in range(P):
+        for b in range(Nb):
+            if se[r, b] >= 0:
+                hosts[int(se[r, b])].append(r * Ns + b)
+    assert all(len(h) == 1 for h in hosts.values())
+    mach = {e: (hosts[e][0] // Ns) // R for e in range(E)}
+    filled = [0] * P
+
+    def rank_loads():
+        RL = [0] * P
+        for e in range(E):
+            hs = sorted(hosts[e])
+            n = len(hs)
+            for idx, j in enumerate(hs):
+                RL[j // Ns] += int(c[e]) // n + (1 if idx < int(c[e]) % n else 0)
+        return RL
+
+    for m in range(M):
+        ranks = range(m * R, (m + 1) * R)
+        for _ in range(R * Nr):
+            def eligible(e):
+                on = {j // Ns for j in hosts[e]}
+                return [r for r in ranks if filled[r] < Nr and r not in on]
+            cands = [e for e in range(E) if mach[e] == m and c[e] > 0 and eligible(e)]
+            if not cands:
+                break
+            estar = min(cands, key=lambda e: (-Fraction(int(c[e]), len(hosts[e])), e))
+            RL = rank_loads()
+            rstar = min(eligible(estar), key=lambda r: (RL[r], r))
+            assert se[rstar, Nb + filled[rstar]] == estar, (m, estar, rstar, se.tolist())
+            hosts[estar].append(rstar * Ns + Nb + filled[rstar])
+            filled[rstar] += 1
+        for r in ranks:
+            assert (se[r, Nb + filled[r]:] == -1).all(), (r, se.tolist())
+
+
 def test_equal_loads_round_robin():
     E, P, Nb, Nr = 12, 4, 3, 2
     se, f = orc.base_placement(np.full(E, 5), P, Nb, Nr)
@@ -98,6 +164,7 @@ def test_random_instances_invariants(seed):
         out, f = orc.microstep_placement(c, base, P, Nb, Nr, M)
         assert f == 0
         _structure_ok(out, E, P, Nb, Nr, c=c)
+        _replay_stage3(c, out, P, Nb, Nr, M)              # every replication round, from the output
         RL = _check_lpt_invariant(c, out, P, Nb, Ns, lambda r: range((r // R) * R, (r // R + 1) * R))
         # experts stay on the machine of their base rank; replicas too
         mach = {int(base[j]): (j // Ns) // R for j in range(len(base)) if base[j] >= 0}
@@ -179,6 +246,30 @@ def test_replication_only_composes_with_stage2(seed):
         assert f == 0 and f1 == 0 and f2 == 0 and f3 == 0
         assert (rep == full).all()
         _structure_ok(rep, E, P, Nb, Nr, c=c)
+        _replay_stage3(c, rep, P, Nb, Nr, M)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_replication_only_replay_on_arbitrary_base(seed):
+    """O13's own pin (independent of O8): on a RANDOM base placement (any expert on any rank -- what
+    Alg. 2's swaps may produce, not an LPT result) every replication round is re-derived from the
+    output; base slots come through unchanged and the input's redundant slots are ignored."""
+    rng = np.random.default_rng(4400 + seed)
+    P = int(rng.choice([2, 3, 4, 6, 8]))
+    Nb, Nr = int(rng.integers(1, 5)), int(rng.integers(1, 4))
+    E, Ns = P * Nb, Nb + Nr
+    c = (rng.integers(0, 50, size=E) * (rng.random(E) < 0.8)).astype(np.int32)
+    if seed % 3 == 0:
+        c[:] = c[0]                                          # all ties: lower id / lowest rank decide
+    placed = np.full((P, Ns), -1, dtype=np.int32)
+    placed[:, :Nb] = rng.permutation(E).reshape(P, Nb)
+    placed[:, Nb:] = rng.integers(-1, E, size=(P, Nr))       # garbage: must be ignored
+    for M in [m for m in (1, 2, P) if P % m == 0]:
+        rep, f = orc.replication(c, placed.ravel(), P, Nb, Nr, M)
+        assert f == 0
+        assert (rep.reshape(P, Ns)[:, :Nb] == placed[:, :Nb]).all()
+        _structure_ok(rep, E, P, Nb, Nr, c=c)
+        _replay_stage3(c, rep, P, Nb, Nr, M)
 
 
 def test_replication_only_on_swapped_placement_and_faults():

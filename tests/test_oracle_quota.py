@@ -44,6 +44,28 @@ def test_golden_vectors():
             assert rl2.tolist() == v["phase_b_loads"]
 
 
+def test_phase_c_order_vectors():
+    """Three hand-worked vectors in which two augmenting choices compete (tests/golden/
+    phase_c_vectors.json): each fixes one of Phase C's order rules -- ascending expert id, ascending
+    host slot / first discovered target, lowest-indexed most loaded rank.  A flip of any of them in
+    the oracle produces the stored 'other_order_quota' (same optimum) and fails here."""
+    vec = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "phase_c_vectors.json")))["vectors"]
+    assert len(vec) == 3
+    for v in vec:
+        c, se = np.array(v["c"], np.int32), np.array(v["slot_expert"], np.int32)
+        q2, rl2, _, _, f = orc.quota(c, se, v["P"], v["Ns"], stop_after=2)
+        assert f == 0 and rl2.tolist() == v["phase_b_loads"], v["name"]
+        q, rl, so, (passes, moved), f = orc.quota(c, se, v["P"], v["Ns"])
+        assert f == 0 and q.tolist() == v["quota"], v["name"]
+        assert rl.tolist() == v["loads"] and moved == v["moved"], v["name"]
+        assert q.tolist() != v["other_order_quota"]
+        # the alternative is an equally optimal, feasible split (so optimality / LP / brute-force pins
+        # cannot tell the two apart: only these vectors do)
+        alt = np.array(v["other_order_quota"], np.int32)
+        assert orc.check_quota(c, se, alt) == 0
+        assert alt.reshape(v["P"], v["Ns"]).sum(1).max() == rl.max()
+
+
 def _check_invariants(c, se, P, Ns, q, rl, so):
     S = P * Ns
     assert (q >= 0).all()

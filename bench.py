@@ -164,6 +164,46 @@ class OracleSample:
         return time.perf_counter() - t0
 
 
+_POOL_BARRIER = None
+
+
+def _pool_init(barrier) -> None:
+    global _POOL_BARRIER
+    _POOL_BARRIER = barrier
+
+
+def _pool_worker(job):
+    """One host core: its own sample of the workload (different samples of the same recipe), generated
+    untimed, then one timed pass of the oracle over it, started together with the other workers."""
+    cfg_id, mb_samples, seed, n_mb = job
+    cfg = synth.config(cfg_id, mb_samples=mb_samples)
+    cfg.seed = seed
+    samp = OracleSample(cfg, 1, n_mb)
+    _POOL_BARRIER.wait()
+    t0 = time.time()
+    samp.step()
+    return samp.routed_tokens, t0, time.time()
+
+
+def oracle_all_cores(cfg, n_mb_each: int) -> dict:
+    """The oracle as it stands (single-threaded C) on every host core at once: one process per core,
+    each over its own instances (instances are independent).  Aggregate routed tokens/s
+    over the window from the common start to the last finish."""
+    import multiprocessing as mp
+    n = max(1, len(os.sched_getaffinity(0)))
+    ctx = mp.get_context("spawn")              # the parent holds a CUDA context: no fork
+    barrier = ctx.Barrier(n)
+    jobs = [(cfg.cfg_id, cfg.mb_samples, cfg.seed + 1000 + k, n_mb_each) for k in range(n)]
+    with ctx.Pool(n, initializer=_pool_init, initargs=(barrier,)) as pool:
+        res = pool.map(_pool_worker, jobs, chunksize=1)
+    tokens = sum(r[0] for r in res)
+    secs = max(r[2] for r in res) - min(r[1] for r in res)
+    return {"value": tokens / secs, "unit": UNIT, "cores": n, "kind": "oracle",
+            "sample": f"{n} processes x (1 layer x {n_mb_each} micro-step(s)) = {tokens} routed tokens, "
+                      "one single-threaded oracle process per host core, started together",
+            "seconds": secs}
+
+
 def run_reference(args, cfg) -> None:
     """--impl reference: the oracle on host cores, same metric / unit / config."""
     rank, _, world = multi.env_rank()
@@ -331,6 +371,38 @@ class Workload:
         torch.cuda.empty_cache()
 
 
+def capture_instance(wl: "Workload", inst) -> tuple:
+    """After the timed region: run one instance of the timed configuration once more (same buffers,
+    same calls) and bring its inputs and outputs to the host for verify_against_oracle."""
+    l, i = inst
+    s = wl.shape
+    a, b = int(wl.mb_off_h[i]), int(wl.mb_off_h[i + 1])
+    n = b - a
+    wl.instance(l, i)
+    torch.cuda.synchronize()
+    bits = lambda t: (t.view(torch.int16).cpu().numpy().view(np.uint16) if t.dtype == torch.bfloat16
+                      else t.cpu().numpy())
+    return (dict(l=l, i=i, a=a, K=s.K, act_dtype=s.act_dtype), wl.plan.inv[l, a:b].cpu().numpy(),
+            wl.plan.w[l, a:b].cpu().numpy(), bits(wl.x[i][:n]), wl.perm[:n * s.K].cpu().numpy(),
+            bits(wl.buf[:n * s.K]), wl.y[:n].cpu().numpy())
+
+
+def verify_against_oracle(meta, inv, w, x, perm, buf, y) -> dict:
+    """cpu_baseline leg only: the captured instance's perm / buf / y against O5 / O6, bit for bit (the
+    plan itself, inv, is compared with the oracle by the tests; here it is checked to be a bijection
+    consistent with perm)."""
+    from oracle import foremoe_oracle as orc      # test infrastructure: allowed in this leg only
+    K, base = meta["K"], meta["a"] * meta["K"]
+    ok_perm = bool((perm[inv.reshape(-1) - base] == np.arange(base, base + inv.size)).all())
+    buf_ref = orc.gather(perm, x, K, pair_base=base)
+    ok_buf = bool((buf_ref == buf).all())
+    y_ref = orc.combine(inv, w, buf_ref, meta["act_dtype"], row_base=base)
+    ok_y = bool((y_ref.view(np.uint32) == y.view(np.uint32)).all())
+    assert ok_perm and ok_buf and ok_y, ("timed configuration disagrees with the oracle", ok_perm, ok_buf, ok_y)
+    return {"instance": [meta["l"], meta["i"]], "perm": ok_perm, "buf_bit_exact": ok_buf, "y_bit_exact": ok_y,
+            "against": "oracle O5/O6 after the timed region"}
+
+
 def probe_stats(probes, bpt) -> dict:
     out = {}
     for name, lst in probes.items():
@@ -437,16 +509,20 @@ def run_ours(args, cfg) -> None:
     dom = "combine" if bpt["combine"] >= bpt["dispatch"] else "dispatch"
     if upd:
         dom = "combine_bwd"
-    traffic = None
+    traffic, traffic_src = None, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")      # written from the committed ncu capture
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get(f"config{cfg.cfg_id}", {}).get(dom)
+            tj = json.load(open(tp))
+            traffic = tj.get(f"config{cfg.cfg_id}", {}).get(dom)
+            if traffic is not None:
+                traffic_src = "stored constant, NOT measured in this run: " + tj.get("_source", "profiles/traffic.json")
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": f"foremoe_{dom}",
                 "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src,
                 "bytes_per_launch": bpt[dom] * max(wl.tok), "avg_launch_ms": kern[dom]["avg_ms"],
                 "whole_path_gbs": value / world * total_bpt / 1e9,
                 "whole_path_frac": value / world * total_bpt / 1e9 / peak,
@@ -484,11 +560,15 @@ def run_ours(args, cfg) -> None:
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
                    "stage": args.stage, "machines": args.machines, "planner": args.planner, "bytes_per_routed_token": total_bpt,
+                   **({"sweep_tuning": args.tune} if args.tune else {}),
                    "launch": ("cuda graph replay of the instance loop" if args.graph else
                               f"{args.streams} streams, independent instances interleaved" if args.streams > 1
                               else "stream launches")},
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
+    verify = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not upd and not args.machines and args.planner != "full":
+        verify = capture_instance(wl, wl.instances[len(wl.instances) // 2])
     if not args.no_e2e and not upd and not args.machines and args.planner != "full":
         line["e2e"] = run_e2e(args, cfg, wl, dev)
     else:
@@ -502,10 +582,31 @@ def run_ours(args, cfg) -> None:
         secs = samp.step()
         line["cpu_baseline"] = {"value": samp.routed_tokens / secs, "unit": UNIT, "cores": 1,
                                 "kind": "oracle", "sample": samp.desc, "seconds": secs}
+        del samp
+        if not args.no_cpu_all_cores:
+            line["cpu_baseline"]["all_cores"] = oracle_all_cores(cfg, max(1, n_samp // 4))
+        if verify is not None:
+            line["verified"] = verify_against_oracle(*verify)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         torch.distributed.destroy_process_group()
+
+
+TUNING_KEYS = ["dispatch_impl", "dispatch_u", "dispatch_cta_per_sm", "dispatch_stages", "dispatch_warps",
+               "combine_impl", "combine_u", "combine_cta_per_sm", "combine_depth", "combine_threads", "pdl",
+               "bwd_depth", "bwd_cta_per_sm", "bwd_impl", "hist_variant"]      # DataTuning, declaration order
+
+
+def apply_tuning(spec: str) -> None:
+    """Sweep runs: switch the binding to libforemoe_tuning.so and set the named launch parameters."""
+    from paper_2606_11867_b200 import binding as fm
+    fm.LIB_PATH = os.path.join(fm.HERE, "libforemoe_tuning.so")
+    lib = fm.lib()
+    lib.foremoe_tuning_set.restype = None
+    for kv in spec.split(","):
+        k, v = kv.split("=")
+        lib.foremoe_tuning_set(TUNING_KEYS.index(k.strip()), int(v))
 
 
 def main() -> None:
@@ -540,7 +641,15 @@ def main() -> None:
                     help="> 1: interleave the independent instances over that many CUDA streams")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-all-cores", action="store_true",
+                    help="skip the all-cores leg of cpu_baseline (one oracle process per host core)")
+    ap.add_argument("--tune", default="",
+                    help="sweeps only: comma-separated key=value launch parameters (csrc/foremoe_data.cuh "
+                         "DataTuning); loads the -DFOREMOE_TUNING build (python -m paper_2606_11867_b200.build "
+                         "--tuning) instead of the product library and marks the line as a sweep")
     args = ap.parse_args()
+    if args.tune:
+        apply_tuning(args.tune)
     cfg = synth.config(args.config, mb_samples=args.mb_samples)
     if args.layers:
         cfg = cfg.scaled(L=args.layers)

@@ -284,12 +284,18 @@ class Workload:
 
     def instance(self, l: int, i: int, ev=None):
         """The data path of one instance; ev (optional) collects CUDA events between the calls."""
-        p = self.plan
+        p = self.plan.data_path()          # binding.DataPath: the plan's arguments marshalled once
+        if ev is None:
+            p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
+            p.combine(l, i, i + 1, self.buf, self.y)
+            if self.stage == "update":
+                p.combine_bwd(l, i, i + 1, self.dy, self.buf, self.d_buf, self.dw)
+                p.dispatch_bwd(l, i, i + 1, self.d_buf, self.dx)
+            return
 
         def mark():
-            if ev is not None:
-                ev.append(torch.cuda.Event(enable_timing=True))
-                ev[-1].record()
+            ev.append(torch.cuda.Event(enable_timing=True))
+            ev[-1].record()
 
         mark()
         p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)

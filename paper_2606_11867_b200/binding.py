@@ -247,6 +247,68 @@ def dispatch_bwd(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, i
         _dev(dev_status, torch.int32), _stream()))
 
 
+class DataPath:
+    """The data-path calls of ONE plan with the plan's own arguments marshalled once.
+
+    The per-instance calls of small micro-steps are host-bound (about 7 us of argument checking and
+    ctypes conversion per call through the functions above, against 10-20 us of kernel time for a
+    one-sample micro-step): this object validates shape, mb_off, inv, w and dev_status when it is
+    built and keeps their C forms, so that a call converts only the activations it is given.  Same
+    C entry points, same semantics; the tensors must stay alive and unmoved while it is used."""
+
+    def __init__(self, shape: Shape, mb_off, inv, w, dev_status=None):
+        self.shape = shape
+        self._keep = (mb_off, inv, w, dev_status)
+        self._sp = C.byref(shape.c())
+        self._mb = C.c_void_p(_dev(mb_off, torch.int32))
+        self._inv = C.c_void_p(_dev(inv, torch.int32))
+        self._w = C.c_void_p(_dev(w, torch.float32))
+        self._st = C.c_void_p(_dev(dev_status, torch.int32))
+        self._act = shape.act_torch_dtype
+        l = lib()
+        self._dispatch, self._combine = l.foremoe_dispatch, l.foremoe_combine
+        self._combine_bwd, self._dispatch_bwd = l.foremoe_combine_bwd, l.foremoe_dispatch_bwd
+        self._dev_index = inv.device.index
+
+    def _act_ptr(self, t) -> int:
+        if t.dtype != self._act or not t.is_cuda or not t.is_contiguous():
+            raise ValueError(f"expected a contiguous CUDA tensor of dtype {self._act}")
+        return t.data_ptr()
+
+    @staticmethod
+    def _f32_ptr(t) -> int:
+        if t.dtype != torch.float32 or not t.is_cuda or not t.is_contiguous():
+            raise ValueError("expected a contiguous CUDA float32 tensor")
+        return t.data_ptr()
+
+    def dispatch(self, layer: int, mb_begin: int, mb_end: int, x, perm, buf) -> None:
+        rc = self._dispatch(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._act_ptr(x),
+                            None if perm is None else _dev(perm, torch.int32), self._act_ptr(buf), self._st,
+                            _raw_stream(self._dev_index))
+        if rc:
+            raise ForeMoEError("foremoe_dispatch", rc)
+
+    def combine(self, layer: int, mb_begin: int, mb_end: int, expert_out, y) -> None:
+        rc = self._combine(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._w,
+                           self._act_ptr(expert_out), self._f32_ptr(y), self._st, _raw_stream(self._dev_index))
+        if rc:
+            raise ForeMoEError("foremoe_combine", rc)
+
+    def combine_bwd(self, layer: int, mb_begin: int, mb_end: int, dy, expert_out, d_expert_out, dw=None) -> None:
+        rc = self._combine_bwd(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._w,
+                               self._f32_ptr(dy), None if expert_out is None else self._act_ptr(expert_out),
+                               self._act_ptr(d_expert_out), None if dw is None else self._f32_ptr(dw),
+                               self._st, _raw_stream(self._dev_index))
+        if rc:
+            raise ForeMoEError("foremoe_combine_bwd", rc)
+
+    def dispatch_bwd(self, layer: int, mb_begin: int, mb_end: int, d_buf, dx) -> None:
+        rc = self._dispatch_bwd(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._act_ptr(d_buf),
+                                self._f32_ptr(dx), self._st, _raw_stream(self._dev_index))
+        if rc:
+            raise ForeMoEError("foremoe_dispatch_bwd", rc)
+
+
 def base_placement(shape: Shape, step_hist, slot_expert, dev_status=None) -> None:
     """(f.4) Stage-1 rank-level LPT: step_hist int64 [L,E] -> slot_expert int32 [L,S]."""
     _check("foremoe_base_placement", lib().foremoe_base_placement(

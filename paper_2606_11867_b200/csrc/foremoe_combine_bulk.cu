@@ -205,9 +205,9 @@ static int launch_one(const Dims &d, int warps, int D, const int32_t *inv_l, con
   if (prepare) return FOREMOE_OK;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   int per_sm = g_tune.combine_cta_per_sm;
-  if (per_sm <= 0) {      // 32 CTAs per SM, fewer when the mean micro-step has under 4 items per warp
+  if (per_sm <= 0) {      // 32 CTAs per SM, fewer when the mean micro-step has under 2 items per warp
     const long long items = (long long)(d.T / d.n_mb + 1) * n_slices;
-    const long long want = (items + 4LL * warps * num_sms() - 1) / (4LL * warps * num_sms());
+    const long long want = (items + 2LL * warps * num_sms() - 1) / (2LL * warps * num_sms());
     per_sm = want < 1 ? 1 : want > 32 ? 32 : (int)want;
   }
   (void)occ;

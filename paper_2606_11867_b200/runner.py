@@ -35,6 +35,13 @@ class StepPlan:
         self.inv = torch.empty((s.L, s.T, s.K), **i32)
         self.workspace = torch.empty(fm.workspace_bytes(s) + 16, dtype=torch.uint8, device=dev)
         self.status = torch.zeros(1, **i32)
+        self._dp = None
+
+    def data_path(self) -> fm.DataPath:
+        """The data-path calls with this plan's arguments marshalled once (binding.DataPath)."""
+        if self._dp is None:
+            self._dp = fm.DataPath(self.shape, self.mb_off, self.inv, self.w, self.status)
+        return self._dp
 
     def load_hist(self) -> None:
         fm.load_hist(self.shape, self.ids, self.mb_off, self.hist, self.step_hist, self.status)
@@ -49,21 +56,17 @@ class StepPlan:
         self.assign(quota_in)
 
     def dispatch(self, layer: int, mb_begin: int, mb_end: int, x, perm, buf) -> None:
-        fm.dispatch(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, x, perm, buf,
-                    self.status)
+        self.data_path().dispatch(layer, mb_begin, mb_end, x, perm, buf)
 
     def combine(self, layer: int, mb_begin: int, mb_end: int, expert_out, y) -> None:
-        fm.combine(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, self.w, expert_out,
-                   y, self.status)
+        self.data_path().combine(layer, mb_begin, mb_end, expert_out, y)
 
     def combine_bwd(self, layer: int, mb_begin: int, mb_end: int, dy, expert_out, d_expert_out,
                     dw=None) -> None:
-        fm.combine_bwd(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, self.w, dy,
-                       expert_out, d_expert_out, dw, self.status)
+        self.data_path().combine_bwd(layer, mb_begin, mb_end, dy, expert_out, d_expert_out, dw)
 
     def dispatch_bwd(self, layer: int, mb_begin: int, mb_end: int, d_buf, dx) -> None:
-        fm.dispatch_bwd(self.shape, layer, mb_begin, mb_end, self.mb_off, self.inv, d_buf, dx,
-                        self.status)
+        self.data_path().dispatch_bwd(layer, mb_begin, mb_end, d_buf, dx)
 
     def faults(self) -> int:
         """Device fault bits raised so far (synchronises)."""

@@ -751,6 +751,123 @@ done:
 }
 
 /* ==========================================================================================
+ * O15 oracle_quota_tradeoff: per-source Stage 4 under the objective of Eq.(10),
+ *     F = a * L* + b * C*,   L* = max_r L_r (Eq.(4)),  C* = max_{i != j} C_{i,j} (Eq.(5)),
+ * with caller-supplied non-negative integers a ~ n1*K1, b ~ n2*K2 (the paper
+ * never prints the coefficients: DESIGN.md reading 33).  The paper solves this LP with HiGHS; its
+ * only algorithmic description of a locality / load trade-off is the heuristic of PAPER.md:337
+ * ("tokens prefer same-machine replicas ..., any leftover tokens are routed to minimize per-rank
+ * load").  Reading 39 turns that sentence into a FAMILY of exact sub-problems indexed by a
+ * threshold theta and lets the objective choose among them:
+ *   member theta: commodity (e, m) whose machine m holds n_loc >= 1 copies of e (ranks) keeps to
+ *     those local copies unless serving it locally would by itself put more than theta times the
+ *     mean rank load on each of them,
+ *         c[e][m] / n_loc  >  theta * total / P      (exact:  c * den * P > num * n_loc * total),
+ *     in which case it may use every copy of e ("leftover tokens"); a commodity without a local
+ *     copy uses every copy (as in O11).  theta = infinity (den = 0) is O11's hard locality;
+ *     theta = 0 lets every non-empty commodity use every copy (the unrestricted min L_max).
+ *   Within a member, L_max is minimised exactly by O2 on the virtual instance (as O11).
+ *   Result: the member with the smallest F; ties to the earliest member of the ladder.
+ * Ladder given by the caller as (num_k, den_k), k = 0 .. n_theta-1.
+ * Outputs: member index, F of every member, and q_src / rank_load / traffic / quota_v /
+ * slot_off_v / se_v of the chosen member (layouts of O11).
+ * Pins (tests/test_oracle_tradeoff.py): member infinity == O11, member 0 reaches O2's optimum on
+ * the summed counts; L_max non-increasing along a descending ladder; F_sel = min_k F_k recomputed
+ * from the members' outputs with numpy; F_sel >= LP* of Eq.(10) incl. the C rows (HiGHS) and >=
+ * the brute-force integer optimum on tiny instances (== when b = 0); a hand-worked vector in
+ * which an intermediate theta wins (tests/golden/tradeoff_vectors.json).
+ * ========================================================================================== */
+int oracle_local_placement_theta(int E, int P, int Ns, int M, int64_t num, int64_t den,
+                                 const int32_t *c_v /* [E*M] */, const int32_t *slot_expert,
+                                 int32_t *slot_expert_v /* [P*Ns*M] */) {
+  const int S = P * Ns;
+  if (M <= 0 || P % M != 0 || num < 0 || den < 0) return ORACLE_BAD_ARG;
+  const int R = P / M;
+  int fault = 0;
+  int64_t total = 0;
+  for (int v = 0; v < E * M; v++) total += c_v[v];
+  for (int j = 0; j < S; j++) {
+    const int32_t e = slot_expert[j];
+    if (e < -1 || e >= E) fault |= FAULT_SLOT_EXPERT;
+    for (int m = 0; m < M; m++) {
+      int32_t v = -1;
+      if (e >= 0 && e < E) {
+        const int mj = (j / Ns) / R;               /* machine of slot j */
+        int n_loc = 0;                             /* ranks of machine m that hold e */
+        for (int r = m * R; r < (m + 1) * R; r++) {
+          int holds = 0;
+          for (int j2 = r * Ns; j2 < (r + 1) * Ns; j2++) holds |= (slot_expert[j2] == e);
+          n_loc += holds;
+        }
+        int spill = 0;
+        if (n_loc > 0 && den > 0)
+          spill = (int64_t)c_v[e * M + m] * den * P > num * n_loc * total;
+        if (mj == m || n_loc == 0 || spill) v = e * M + m;
+      }
+      slot_expert_v[(size_t)j * M + m] = v;
+    }
+  }
+  return fault;
+}
+
+int oracle_quota_tradeoff(int E, int P, int Ns, int M, int64_t a, int64_t b, int n_theta,
+                          const int64_t *theta_num, const int64_t *theta_den,
+                          const int32_t *w_se /* [P][E] per-source counts */, const int32_t *slot_expert,
+                          int32_t *member /* [1] */, int64_t *F /* [n_theta] */,
+                          int32_t *q_src /* [M][S] */, int32_t *rank_load /* [P] */,
+                          int32_t *traffic /* [M][M] */, int32_t *quota_v /* [S*M] */,
+                          int32_t *slot_off_v /* [S*M+1] */, int32_t *se_v_sel /* [S*M] */) {
+  const int S = P * Ns;
+  if (M <= 0 || P % M != 0 || n_theta <= 0 || a < 0 || b < 0) return ORACLE_BAD_ARG;
+  const int R = P / M;
+  int32_t *c_v = (int32_t *)calloc((size_t)E * M, sizeof(int32_t));
+  int32_t *se_v = (int32_t *)calloc((size_t)S * M, sizeof(int32_t));
+  int32_t *q_v = (int32_t *)calloc((size_t)S * M, sizeof(int32_t));
+  int32_t *so_v = (int32_t *)calloc((size_t)S * M + 1, sizeof(int32_t));
+  int32_t *rl = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int fault = 0, best = -1;
+  if (!c_v || !se_v || !q_v || !so_v || !rl) { fault = ORACLE_NO_MEM; goto done; }
+  for (int s = 0; s < P; s++)
+    for (int e = 0; e < E; e++) c_v[e * M + s / R] += w_se[(size_t)s * E + e];
+  for (int k = 0; k < n_theta; k++) {
+    int f = oracle_local_placement_theta(E, P, Ns, M, theta_num[k], theta_den[k], c_v, slot_expert, se_v);
+    if (f < 0) { fault = f; goto done; }
+    f |= oracle_quota(E * M, P, Ns * M, c_v, se_v, q_v, rl, so_v, 3, NULL);
+    if (f < 0) { fault = f; goto done; }
+    fault |= f;
+    int64_t lmax = 0, cmax = 0;
+    for (int r = 0; r < P; r++) if (rl[r] > lmax) lmax = rl[r];
+    for (int i = 0; i < M; i++)
+      for (int mj = 0; mj < M; mj++) {
+        if (i == mj) continue;
+        int64_t t = 0;
+        for (int j = mj * R * Ns; j < (mj + 1) * R * Ns; j++) t += q_v[(size_t)j * M + i];
+        if (t > cmax) cmax = t;
+      }
+    F[k] = a * lmax + b * cmax;
+    if (best < 0 || F[k] < F[best]) {              /* strict: ties stay with the earlier member */
+      best = k;
+      for (int m = 0; m < M; m++)
+        for (int j = 0; j < S; j++) q_src[(size_t)m * S + j] = q_v[(size_t)j * M + m];
+      for (int i = 0; i < M; i++)
+        for (int mj = 0; mj < M; mj++) {
+          int64_t t = 0;
+          for (int j = mj * R * Ns; j < (mj + 1) * R * Ns; j++) t += q_v[(size_t)j * M + i];
+          traffic[i * M + mj] = (int32_t)t;
+        }
+      memcpy(rank_load, rl, sizeof(int32_t) * (size_t)P);
+      memcpy(quota_v, q_v, sizeof(int32_t) * (size_t)S * M);
+      memcpy(slot_off_v, so_v, sizeof(int32_t) * ((size_t)S * M + 1));
+      memcpy(se_v_sel, se_v, sizeof(int32_t) * (size_t)S * M);
+    }
+  }
+  *member = best;
+done:
+  free(c_v); free(se_v); free(q_v); free(so_v); free(rl);
+  return fault;
+}
+
+/* ==========================================================================================
  * NEXT row (second half): Alg. 2 Stage 2, expert relocation by swaps
  * (sec. 8.2 prose; listing lines 4-12).
  *

@@ -211,6 +211,41 @@ def quota_local(w_se: np.ndarray, slot_expert: np.ndarray, P: int, Ns: int, M: i
     return out
 
 
+DEFAULT_LADDER = ((0, 0), (2, 1), (1, 1), (1, 2), (1, 4), (0, 1))   # theta = inf, 2, 1, 1/2, 1/4, 0 as (num, den)
+
+
+def local_placement_theta(c_v: np.ndarray, slot_expert: np.ndarray, E: int, P: int, Ns: int, M: int,
+                          num: int, den: int):
+    """O15 member: commodity counts int32 [E*M], real placement [S] -> virtual placement [S*M], fault."""
+    c_v, se = _i32(c_v), _i32(slot_expert)
+    out = np.full(P * Ns * M, -1, dtype=np.int32)
+    f = lib().oracle_local_placement_theta
+    f.argtypes = [C.c_int] * 4 + [C.c_int64, C.c_int64] + [C.c_void_p] * 3
+    fault = f(E, P, Ns, M, num, den, _p(c_v), _p(se), _p(out))
+    return out, fault
+
+
+def quota_tradeoff(w_se: np.ndarray, slot_expert: np.ndarray, P: int, Ns: int, M: int, a: int, b: int,
+                   ladder=DEFAULT_LADDER):
+    """O15 for one instance: per-source counts int32 [P,E], placement [S], objective a*L_max + b*C_max ->
+    dict(member, F [n_theta], q_src [M,S], rank_load [P], traffic [M,M], quota_v, slot_off_v, se_v, fault)."""
+    w_se, se = _i32(w_se), _i32(slot_expert)
+    E, S = w_se.shape[1], P * Ns
+    num = np.array([t[0] for t in ladder], dtype=np.int64)
+    den = np.array([t[1] for t in ladder], dtype=np.int64)
+    out = dict(member=np.zeros(1, np.int32), F=np.zeros(len(ladder), np.int64),
+               q_src=np.zeros((M, S), np.int32), rank_load=np.zeros(P, np.int32),
+               traffic=np.zeros((M, M), np.int32), quota_v=np.zeros(S * M, np.int32),
+               slot_off_v=np.zeros(S * M + 1, np.int32), se_v=np.zeros(S * M, np.int32))
+    f = lib().oracle_quota_tradeoff
+    f.argtypes = [C.c_int] * 4 + [C.c_int64, C.c_int64, C.c_int] + [C.c_void_p] * 12
+    out["fault"] = f(E, P, Ns, M, a, b, len(ladder), _p(num), _p(den), _p(w_se), _p(se), _p(out["member"]),
+                     _p(out["F"]), _p(out["q_src"]), _p(out["rank_load"]), _p(out["traffic"]),
+                     _p(out["quota_v"]), _p(out["slot_off_v"]), _p(out["se_v"]))
+    out["member"] = int(out["member"][0])
+    return out
+
+
 def swap_relocation(c_me: np.ndarray, base_se: np.ndarray, P: int, Nb: int, Nr: int, M: int = 1,
                     win: int = 2, max_rounds: int = 16, a: int = 1, b: int = 0):
     """O12 for one instance: per-source-machine loads int32 [M,E] (or [E] with M = 1), base

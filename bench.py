@@ -237,7 +237,8 @@ class Workload:
     """Device-resident inputs and outputs of one rank's step (inputs are seeded and synthetic:
     recipe in DESIGN.md sec. 4).  Nothing here is timed."""
 
-    def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0, planner: str = "stage4"):
+    def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0, planner: str = "stage4",
+                 objective=None):
         from paper_2606_11867_b200 import binding as fm
         from paper_2606_11867_b200 import runner
         self.fm, self.cfg, self.dev = fm, cfg, dev
@@ -260,8 +261,11 @@ class Workload:
             self.tok_src_h = synth.gen_tok_src(cfg)
             se_dev = self.plan.slot_expert
             self.plan = None
-            self.plan = runner.LocalStepPlan(s, machines, ids, w, mb_off, se_dev,
-                                             torch.from_numpy(self.tok_src_h).to(dev))
+            src = torch.from_numpy(self.tok_src_h).to(dev)
+            if objective:     # Eq.(10): F = a L_max + b C_max over the threshold ladder (reading 39)
+                self.plan = runner.TradeoffStepPlan(s, machines, objective[0], objective[1], ids, w, mb_off, se_dev, src)
+            else:             # hard locality (reading 30)
+                self.plan = runner.LocalStepPlan(s, machines, ids, w, mb_off, se_dev, src)
             self.real_shape, self.shape = s, self.plan.shape      # same K, H, T, n_mb; E, Nb, Nr x M
         tok = [int(self.mb_off_h[i + 1] - self.mb_off_h[i]) for i in range(s.n_mb)]
         self.tok = tok
@@ -273,7 +277,9 @@ class Workload:
         self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
         self.routed_tokens = sum(tok) * s.L
         self.stage = stage
+        n_lad = len(runner.DEFAULT_LADDER) if (objective and machines and planner != "full") else 0
         self.launches_per_step = (2 + 5 + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
+                                  + n_lad * 5 + (1 if n_lad else 0)
                                   + (4 if stage == "update" else 2) * len(self.instances))
         if stage == "update":          # forward + backward of every instance
             self.dy = torch.randn((mx, s.H), dtype=torch.float32, device=dev,
@@ -473,7 +479,8 @@ def run_ours(args, cfg) -> None:
     torch.cuda.set_device(dev)
     multi.init("nccl", dev)
     cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
-    wl = Workload(cfg, dev, args.stage, args.machines, args.planner)
+    objective = tuple(int(v) for v in args.objective.split(",")) if args.objective else None
+    wl = Workload(cfg, dev, args.stage, args.machines, args.planner, objective)
     bpt = bytes_per_token(cfg)
     upd = args.stage == "update"
     total_bpt = bpt["total_update"] if upd else bpt["total"]
@@ -555,6 +562,11 @@ def run_ours(args, cfg) -> None:
         off = tr.clone()
         off.diagonal(dim1=-2, dim2=-1).zero_()
         balance["machines"] = args.machines
+        if objective:
+            balance["objective"] = {"a": objective[0], "b": objective[1],
+                                    "members_chosen": torch.bincount(wl.plan.member[live].flatten().long(),
+                                                                     minlength=len(wl.plan.ladder)).tolist(),
+                                    "ladder": [list(t) for t in wl.plan.ladder]}
         balance["cross_machine_fraction"] = {"mean": float(cross[live].mean()), "max": float(cross[live].max())}
         balance["c_max_tokens"] = {"median": float(off.amax((-1, -2))[live].median()), "max": float(off.max())}
     line = {
@@ -565,7 +577,8 @@ def run_ours(args, cfg) -> None:
         "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
-                   "stage": args.stage, "machines": args.machines, "planner": args.planner, "bytes_per_routed_token": total_bpt,
+                   "stage": args.stage, "machines": args.machines, "planner": args.planner,
+                   **({"objective": args.objective} if args.objective else {}), "bytes_per_routed_token": total_bpt,
                    **({"sweep_tuning": args.tune} if args.tune else {}),
                    "launch": ("cuda graph replay of the instance loop" if args.graph else
                               f"{args.streams} streams, independent instances interleaved" if args.streams > 1
@@ -639,6 +652,9 @@ def main() -> None:
     ap.add_argument("--machines", type=int, default=0,
                     help="M > 0: per-source, locality-aware Stage 4 over M machines of P/M ranks "
                          "(commodity plan, SURVEY.md sec. 8(f).1); the data path is unchanged")
+    ap.add_argument("--objective", default="",
+                    help="with --machines: 'a,b' = Stage 4 under F = a*L_max + b*C_max (Eq.(10)) over the "
+                         "locality-threshold ladder instead of the hard locality rule")
     ap.add_argument("--planner", default="stage4", choices=["stage4", "full"],
                     help="stage4 = the headline path (step-level placement is an input, Stage 4 on the GPU); "
                          "full = Stage 1 + Alg. 3 Stages 2-3 + Stage 4 all on the GPU inside the timed step "

@@ -132,6 +132,9 @@ int foremoe_load_hist(const foremoe_shape_t *shape, const int32_t *ids, const in
  *   inv         [L][T][K]      out: layer-global destination row of every pair
  *               = mb_off[i]*K + slot_off[j] + (stable rank of the pair inside slot j).  -1 on fault.
  *   workspace   device scratch of at least foremoe_workspace_bytes() bytes, 16-byte aligned.
+ * pair_slot and inv may BOTH be NULL: only the quotas (a2) are computed -- quota, rank_load,
+ * slot_off -- and the ids are not read (used to evaluate candidate placements, see
+ * foremoe_tradeoff_select).
  * Faults: ID_RANGE, NO_HOST, SLOT_EXPERT, MB_OFF, QUOTA_IN.
  */
 int foremoe_assign(const foremoe_shape_t *shape, const int32_t *ids, const int32_t *mb_off,
@@ -292,6 +295,42 @@ int foremoe_local_placement(const foremoe_shape_t *shape, int32_t M, const int32
 
 int foremoe_traffic(const foremoe_shape_t *shape, int32_t M, const int32_t *quota_v,
                     int32_t *traffic, void *stream);
+
+/*
+ * (NEXT, the C* term) Per-source Stage 4 under the objective of Eq.(10),
+ *     F = a * L* + b * C*,  L* = max_r L_r,  C* = max_{i != j} C_{i,j},
+ * with caller-supplied integers a ~ n1*K1, b ~ n2*K2 in [0, 2^20] (reading 33).  The paper
+ * solves this LP on the CPU; here the locality heuristic of PAPER.md:337 becomes a LADDER of exact
+ * sub-problems (reading 39): member theta = num / den restricts commodity (e, m) to the
+ * copies of e on machine m unless its count per local copy exceeds theta times the mean rank load,
+ *     hist_v[e*M+m] * den * P  >  num * n_loc(e, m) * sum(hist_v),
+ * in which case (or when machine m holds no copy) it may use every copy.  den = 0 means theta =
+ * infinity: foremoe_local_placement's hard locality; num = 0, den = 1: no restriction.
+ * Composition (paper_2606_11867_b200/runner.py TradeoffStepPlan), per member k of the ladder:
+ *   foremoe_local_placement_theta -> slot_expert_v_k [n_mb][L][S*M]  (one placement per instance)
+ *   foremoe_assign(shape_v with placement_mb_stride = L*S*M, pair_slot = inv = NULL) -> quota_k,
+ *       rank_load_k  (exact min L_max within the member);  foremoe_traffic -> traffic_k;
+ * then foremoe_tradeoff_select picks, per instance, the member with the smallest F (ties: the
+ * earliest) and copies out its quotas and placement, and one more foremoe_assign with
+ * quota_in = quota_sel on slot_expert_v_sel assigns the pairs.
+ *
+ * foremoe_local_placement_theta: hist_v [n_mb][L][E*M] (foremoe_load_hist on the commodity ids);
+ *   slot_expert [L][S] or [n_mb][L][S] per placement_mb_stride; slot_expert_v_mb [n_mb][L][S*M] out.
+ *   theta_num, theta_den in [0, 2^20].  Fault SLOT_EXPERT for values outside [-1, E).
+ * foremoe_tradeoff_select: arrays with a leading member axis [n_members][n_mb][L][...]:
+ *   rank_load_k [..][P], traffic_k [..][M][M], quota_k [..][S*M], slot_expert_v_k [..][S*M];
+ *   member [n_mb][L] out; F [n_members][n_mb][L] int64 out or NULL; quota_sel, slot_expert_v_sel
+ *   [n_mb][L][S*M] out.  n_members <= 64, M <= 128.
+ * `shape` in both calls is the REAL shape; M must divide P.
+ */
+int foremoe_local_placement_theta(const foremoe_shape_t *shape, int32_t M, int64_t theta_num,
+                                  int64_t theta_den, const int32_t *hist_v, const int32_t *slot_expert,
+                                  int32_t *slot_expert_v_mb, int32_t *dev_status, void *stream);
+
+int foremoe_tradeoff_select(const foremoe_shape_t *shape, int32_t M, int32_t n_members, int64_t a,
+                            int64_t b, const int32_t *rank_load_k, const int32_t *traffic_k,
+                            const int32_t *quota_k, const int32_t *slot_expert_v_k, int32_t *member,
+                            int64_t *F, int32_t *quota_sel, int32_t *slot_expert_v_sel, void *stream);
 
 /*
  * (NEXT, second half) Alg. 2 Stage 2: expert relocation by swaps

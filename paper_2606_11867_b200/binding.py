@@ -38,6 +38,7 @@ ACT_FP32 = 1
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_warmup", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
+           "foremoe_local_placement_theta", "foremoe_tradeoff_select",
            "foremoe_swap_relocation", "foremoe_replication",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
@@ -126,6 +127,8 @@ def lib() -> C.CDLL:
         l.foremoe_source_ids.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_local_placement.argtypes = [sp, i32, vp, vp, vp, vp]
         l.foremoe_traffic.argtypes = [sp, i32, vp, vp, vp]
+        l.foremoe_local_placement_theta.argtypes = [sp, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp]
+        l.foremoe_tradeoff_select.argtypes = [sp, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_replication.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_swap_relocation.argtypes = [sp, i32, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp]
         l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
@@ -350,6 +353,24 @@ def traffic(shape: Shape, M: int, quota_v, traffic_out) -> None:
     """(f.1) quota_v [n_mb,L,S*M] -> traffic [n_mb,L,M,M] (Eq.(5) off the diagonal)."""
     _check("foremoe_traffic", lib().foremoe_traffic(
         C.byref(shape.c()), M, _dev(quota_v, torch.int32), _dev(traffic_out, torch.int32), _stream()))
+
+
+def local_placement_theta(shape: Shape, M: int, num: int, den: int, hist_v, slot_expert, slot_expert_v_mb,
+                          dev_status=None) -> None:
+    """(f.1, C* term) one ladder member: hist_v [n_mb,L,E*M] + slot_expert -> slot_expert_v_mb [n_mb,L,S*M]."""
+    _check("foremoe_local_placement_theta", lib().foremoe_local_placement_theta(
+        C.byref(shape.c()), M, num, den, _dev(hist_v, torch.int32), _dev(slot_expert, torch.int32),
+        _dev(slot_expert_v_mb, torch.int32), _dev(dev_status, torch.int32), _stream()))
+
+
+def tradeoff_select(shape: Shape, M: int, a: int, b: int, rank_load_k, traffic_k, quota_k, slot_expert_v_k,
+                    member, F, quota_sel, slot_expert_v_sel) -> None:
+    """(f.1, C* term) per instance the member with the smallest a*L_max + b*C_max; [n_members, ...] inputs."""
+    _check("foremoe_tradeoff_select", lib().foremoe_tradeoff_select(
+        C.byref(shape.c()), M, int(rank_load_k.shape[0]), a, b, _dev(rank_load_k, torch.int32),
+        _dev(traffic_k, torch.int32), _dev(quota_k, torch.int32), _dev(slot_expert_v_k, torch.int32),
+        _dev(member, torch.int32), _dev(F, torch.int64), _dev(quota_sel, torch.int32),
+        _dev(slot_expert_v_sel, torch.int32), _stream()))
 
 
 def swap_relocation(shape: Shape, M: int, win: int, max_rounds: int, a: int, b: int, hist_v,

@@ -777,9 +777,10 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
   Dims d;
   int rc = make_dims(shape, &d);
   if (rc) return rc;
-  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !pair_slot ||
-      !inv || !workspace)
+  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
     return FOREMOE_ERR_INVALID_ARG;
+  if ((pair_slot == nullptr) != (inv == nullptr)) return FOREMOE_ERR_INVALID_ARG;
+  const bool want_pairs = pair_slot != nullptr;      // both NULL: quotas only (a2), no pass over the ids
   if (!aligned(workspace, 16)) return FOREMOE_ERR_INVALID_ARG;
   const Workspace w = make_workspace(d);
   if (workspace_bytes < w.total) return FOREMOE_ERR_WORKSPACE;
@@ -814,14 +815,14 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
                                                    pl_host_slot, pl_active, pl_rslot, pl_fault,
                                                    dev_status);
   const dim3 cgrid(d.max_chunks, d.L);
-  if (d.T > 0)
+  if (d.T > 0 && want_pairs)
     k_chunk_hist<<<cgrid, kChunkThreads, sizeof(int32_t) * d.E, st>>>(
         ids, mb_off, chunk_off, d.L, d.T, d.K, d.E, d.n_mb, d.tpc, d.max_chunks, chunk_cnt);
   k_quota<<<d.n_inst, kQuotaThreads, smem_quota, st>>>(
       hist, quota_in, mb_ok, chunk_off, pl_host_ptr, pl_host_slot, pl_active, pl_rslot, pl_fault,
       slot_expert, d.L, d.E, d.P, d.Ns, d.pl_per_mb, d.max_chunks, quota, rank_load, slot_off,
       inst_cum_end, inst_slot_adj, inst_ok, chunk_cnt, dev_status);
-  if (d.T > 0)
+  if (d.T > 0 && want_pairs)
     k_assign_pairs<<<cgrid, kChunkThreads, smem_pairs, st>>>(
         ids, mb_off, chunk_off, pl_host_ptr, pl_host_slot, inst_cum_end, inst_slot_adj, inst_ok,
         chunk_cnt, d.L, d.T, d.K, d.E, d.S, d.n_mb, d.tpc, d.max_chunks, d.pl_per_mb, pair_slot,

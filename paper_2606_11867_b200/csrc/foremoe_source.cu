@@ -87,6 +87,92 @@ k_traffic(const int32_t *__restrict__ quota_v, int S, int Ns, int P, int M,
   for (int i = threadIdx.x; i < M * M; i += blockDim.x) traffic[(size_t)blockIdx.x * M * M + i] = acc[i];
 }
 
+// ---------------------------------------------------------------------------------------------
+// Stage 4 under F = a * L_max + b * C_max (Eq.(10)) as a ladder of locality
+// thresholds (reading 39).  k_local_placement_theta builds ONE member's virtual placement
+// per (micro-step, layer) instance: commodity (e, m) keeps to machine m's copies of e unless
+// c[e][m] / n_loc > theta * total / P, i.e. c * den * P > num * n_loc * total (den = 0: never).
+// one CTA per instance; smem: nloc[E*M] (ranks of machine m holding e), red[32] (int64 reduction)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_local_placement_theta(const int32_t *__restrict__ se, const int32_t *__restrict__ hist_v, int L, int E,
+                        int S, int Ns, int P, int M, int pl_per_mb, long long num, long long den,
+                        int32_t *__restrict__ se_v, int32_t *dev_status) {
+  extern __shared__ long long red64[];                 // [32] then int32 nloc[E*M]
+  int32_t *nloc = (int32_t *)(red64 + 32);
+  const int R = P / M, inst = blockIdx.x, l = inst % L;
+  const int32_t *src = se + (size_t)(pl_per_mb ? inst : l) * S;
+  const int32_t *c = hist_v + (size_t)inst * E * M;
+  int32_t *dst = se_v + (size_t)inst * S * M;
+  for (int i = threadIdx.x; i < E * M; i += blockDim.x) nloc[i] = 0;
+  long long part = 0;
+  for (int i = threadIdx.x; i < E * M; i += blockDim.x) part += c[i];
+#pragma unroll
+  for (int o = 16; o; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+  if ((threadIdx.x & 31) == 0) red64[threadIdx.x >> 5] = part;
+  __syncthreads();
+  long long total = 0;
+  for (int w = 0; w < (int)(blockDim.x >> 5); w++) total += red64[w];
+  int fault = 0;
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {   // each rank counts an expert once
+    const int e = src[j];
+    if (e < -1 || e >= E) { fault |= FOREMOE_FAULT_SLOT_EXPERT; continue; }
+    if (e < 0) continue;
+    bool first = true;
+    for (int j2 = (j / Ns) * Ns; j2 < j; j2++) first &= (src[j2] != e);
+    if (first) atomicAdd(nloc + e * M + (j / Ns) / R, 1);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < S * M; i += blockDim.x) {
+    const int j = i / M, m = i - j * M;
+    const int e = src[j];
+    int v = -1;
+    if (e >= 0 && e < E) {
+      const int n = nloc[e * M + m];
+      const bool spill = n > 0 && den > 0 && (long long)c[e * M + m] * den * P > num * n * total;
+      if ((j / Ns) / R == m || n == 0 || spill) v = e * M + m;
+    }
+    dst[i] = v;
+  }
+  raise_fault(dev_status, fault);
+}
+
+// The member with the smallest F = a * max_r rank_load + b * max_{i != j} traffic wins (ties: the
+// earliest member); its quotas and virtual placement are copied out.  One CTA per instance.
+__global__ void __launch_bounds__(256)
+k_tradeoff_select(int n_members, size_t n_inst, int P, int M, int SM, long long a, long long b,
+                  const int32_t *__restrict__ rank_load_k, const int32_t *__restrict__ traffic_k,
+                  const int32_t *__restrict__ quota_k, const int32_t *__restrict__ se_v_k,
+                  int32_t *__restrict__ member, long long *__restrict__ F,
+                  int32_t *__restrict__ quota_sel, int32_t *__restrict__ se_v_sel) {
+  __shared__ int best_k;
+  const size_t inst = blockIdx.x;
+  if (threadIdx.x == 0) {
+    long long best = 0;
+    int bk = -1;
+    for (int k = 0; k < n_members; k++) {
+      const int32_t *rl = rank_load_k + ((size_t)k * n_inst + inst) * P;
+      const int32_t *tr = traffic_k + ((size_t)k * n_inst + inst) * M * M;
+      long long lmax = 0, cmax = 0;
+      for (int r = 0; r < P; r++) lmax = rl[r] > lmax ? rl[r] : lmax;
+      for (int i = 0; i < M; i++)
+        for (int j = 0; j < M; j++)
+          if (i != j && tr[i * M + j] > cmax) cmax = tr[i * M + j];
+      const long long f = a * lmax + b * cmax;
+      if (F) F[(size_t)k * n_inst + inst] = f;
+      if (bk < 0 || f < best) { best = f; bk = k; }
+    }
+    best_k = bk;
+    member[inst] = bk;
+  }
+  __syncthreads();
+  const size_t from = ((size_t)best_k * n_inst + inst) * SM, to = inst * SM;
+  for (int i = threadIdx.x; i < SM; i += blockDim.x) {
+    quota_sel[to + i] = quota_k[from + i];
+    se_v_sel[to + i] = se_v_k[from + i];
+  }
+}
+
 static int check_machines(const Dims &d, int M) {
   if (M <= 0 || d.P % M != 0) return FOREMOE_ERR_INVALID_ARG;
   if ((int64_t)d.E * M >= ((int64_t)1 << 30) || (int64_t)d.S * M >= ((int64_t)1 << 24))
@@ -143,5 +229,45 @@ extern "C" __attribute__((visibility("default"))) int foremoe_traffic(
   if (!quota_v || !traffic || M > 128) return FOREMOE_ERR_INVALID_ARG;
   k_traffic<<<d.n_inst, 256, sizeof(int32_t) * (size_t)M * M, (cudaStream_t)stream>>>(
       quota_v, d.S, d.Ns, d.P, M, traffic);
+  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_local_placement_theta(
+    const foremoe_shape_t *shape, int32_t M, int64_t theta_num, int64_t theta_den, const int32_t *hist_v,
+    const int32_t *slot_expert, int32_t *slot_expert_v_mb, int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if ((rc = check_machines(d, M))) return rc;
+  if (!hist_v || !slot_expert || !slot_expert_v_mb || theta_num < 0 || theta_den < 0 ||
+      theta_num > (1 << 20) || theta_den > (1 << 20))
+    return FOREMOE_ERR_INVALID_ARG;
+  const size_t smem = 32 * sizeof(long long) + sizeof(int32_t) * (size_t)d.E * M;
+  if (smem > 200 * 1024) return FOREMOE_ERR_INVALID_ARG;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(k_local_placement_theta, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return FOREMOE_ERR_CUDA;
+  k_local_placement_theta<<<d.n_inst, 256, smem, (cudaStream_t)stream>>>(
+      slot_expert, hist_v, d.L, d.E, d.S, d.Ns, d.P, M, d.pl_per_mb, theta_num, theta_den,
+      slot_expert_v_mb, dev_status);
+  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_tradeoff_select(
+    const foremoe_shape_t *shape, int32_t M, int32_t n_members, int64_t a, int64_t b,
+    const int32_t *rank_load_k, const int32_t *traffic_k, const int32_t *quota_k,
+    const int32_t *slot_expert_v_k, int32_t *member, int64_t *F, int32_t *quota_sel,
+    int32_t *slot_expert_v_sel, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if ((rc = check_machines(d, M))) return rc;
+  if (!rank_load_k || !traffic_k || !quota_k || !slot_expert_v_k || !member || !quota_sel ||
+      !slot_expert_v_sel || n_members <= 0 || n_members > 64 || a < 0 || b < 0 || a > (1 << 20) ||
+      b > (1 << 20) || M > 128)
+    return FOREMOE_ERR_INVALID_ARG;
+  k_tradeoff_select<<<d.n_inst, 256, 0, (cudaStream_t)stream>>>(
+      n_members, (size_t)d.n_inst, d.P, M, d.S * M, a, b, rank_load_k, traffic_k, quota_k,
+      slot_expert_v_k, member, (long long *)F, quota_sel, slot_expert_v_sel);
   return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }

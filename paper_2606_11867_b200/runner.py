@@ -97,6 +97,53 @@ class LocalStepPlan(StepPlan):
         fm.traffic(self.real_shape, self.M, self.quota, self.traffic)
 
 
+DEFAULT_LADDER = ((0, 0), (2, 1), (1, 1), (1, 2), (1, 4), (0, 1))    # theta = inf, 2, 1, 1/2, 1/4, 0 as (num, den)
+
+
+class TradeoffStepPlan(LocalStepPlan):
+    """Per-source Stage 4 under F = a * L_max + b * C_max (Eq.(10); DESIGN.md reading
+    39): every member of the threshold ladder is solved exactly for every instance (quotas only), the
+    objective picks one per instance, and the pairs are assigned on the chosen member.  Attributes as
+    LocalStepPlan, plus ``member`` [n_mb,L], ``F`` [n_members,n_mb,L]; ``slot_expert`` is the chosen
+    virtual placement [n_mb,L,S*M] and the plan's shape carries ``placement_mb_stride = L*S*M``."""
+
+    def __init__(self, shape: fm.Shape, M: int, a: int, b: int, ids, w, mb_off, slot_expert, tok_src,
+                 ladder=DEFAULT_LADDER):
+        import dataclasses
+        super().__init__(shape, M, ids, w, mb_off, slot_expert, tok_src)
+        dev, s, n = ids.device, shape, len(ladder)
+        self.a, self.b, self.ladder = a, b, tuple(ladder)
+        sv = self.shape
+        self.shape = dataclasses.replace(sv, placement_mb_stride=sv.L * sv.S)      # one placement per instance
+        self._dp = None
+        i32 = dict(dtype=torch.int32, device=dev)
+        self.se_v_k = torch.empty((n, s.n_mb, s.L, sv.S), **i32)
+        self.quota_k = torch.empty((n, s.n_mb, s.L, sv.S), **i32)
+        self.rank_load_k = torch.empty((n, s.n_mb, s.L, s.P), **i32)
+        self.slot_off_k = torch.empty((s.n_mb, s.L, sv.S + 1), **i32)              # scratch, not kept per member
+        self.traffic_k = torch.empty((n, s.n_mb, s.L, M, M), **i32)
+        self.member = torch.empty((s.n_mb, s.L), **i32)
+        self.F = torch.empty((n, s.n_mb, s.L), dtype=torch.int64, device=dev)
+        self.quota_sel = torch.empty((s.n_mb, s.L, sv.S), **i32)
+        self.slot_expert = torch.empty((s.n_mb, s.L, sv.S), **i32)
+        self.workspace = torch.empty(fm.workspace_bytes(self.shape) + 16, dtype=torch.uint8, device=dev)
+
+    def plan(self, quota_in: Optional[torch.Tensor] = None) -> None:
+        assert quota_in is None
+        rs, M = self.real_shape, self.M
+        fm.source_ids(rs, M, self.real_ids, self.tok_src, self.ids, self.status)
+        self.load_hist()
+        for k, (num, den) in enumerate(self.ladder):
+            fm.local_placement_theta(rs, M, num, den, self.hist, self.real_slot_expert, self.se_v_k[k], self.status)
+            fm.assign(self.shape, self.ids, self.mb_off, self.hist, self.se_v_k[k], None, self.quota_k[k],
+                      self.rank_load_k[k], self.slot_off_k, None, None, self.workspace, self.status)
+            fm.traffic(rs, M, self.quota_k[k], self.traffic_k[k])
+        fm.tradeoff_select(rs, M, self.a, self.b, self.rank_load_k, self.traffic_k, self.quota_k, self.se_v_k,
+                           self.member, self.F, self.quota_sel, self.slot_expert)
+        self.assign(self.quota_sel)
+        fm.traffic(rs, M, self.quota, self.traffic)
+
+
 class PlannerStepPlan(StepPlan):
     """All four planner stages on the device: Stage 1 (rank-level LPT from the step totals), Alg. 3
     Stages 2-3 per (micro-step, layer) over ``M`` machines, Stage 4 on the per-micro-step placements

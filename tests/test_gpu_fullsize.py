@@ -301,3 +301,44 @@ def test_full_config_local(cuda_device, cfg_id, M):
         assert (lp.pair_slot[0, a:b].cpu().numpy().ravel() == ps).all(), ("pair_slot_v", i)
         assert (lp.inv[0, a:b].cpu().numpy().ravel() == inv).all(), ("inv", i)
     _library_data_checks(wl, [wl.instances[0], wl.instances[-1]])
+
+
+def test_full_config2_tradeoff(cuda_device):
+    """Per-source Stage 4 under F = L_max + C_max at full size (bench.Workload with machines = 2,
+    objective (1, 1)): invariants of the chosen commodity plan for every instance, F never above either
+    end of the ladder, O15 on the first and last micro-step of layer 0, the data path on one instance."""
+    cfg = synth.config(2)
+    M = 2
+    wl = bench.Workload(cfg, cuda_device, "recompute", M, "stage4", (1, 1))
+    tp = wl.plan
+    tp.plan()
+    torch.cuda.synchronize()
+    assert tp.faults() == 0
+    # the plan's placement differs per instance: evaluate the invariants against the chosen one
+    dev = tp.ids.device
+    s = wl.shape
+    quota, hist = tp.quota.long(), tp.hist.long()
+    se = tp.slot_expert.long()                                        # [n_mb, L, S_v]
+    per_e = torch.zeros((s.n_mb, s.L, s.E + 1), dtype=torch.int64, device=dev)
+    per_e.scatter_add_(2, torch.where(se >= 0, se, torch.full_like(se, s.E)), quota)
+    assert torch.equal(per_e[..., :s.E], hist) and (per_e[..., s.E] == 0).all()     # Eq.(8) / (9)
+    assert torch.equal(tp.rank_load.long(), quota.view(s.n_mb, s.L, s.P, s.Ns).sum(-1))
+    F = tp.F
+    Fsel = F.gather(0, tp.member.long()[None]).squeeze(0)
+    assert (Fsel == F.min(0).values).all() and (tp.member.long() == F.argmin(0)).all()
+    R = cfg.P // M
+    ids_h = tp.real_ids[0].cpu().numpy()
+    for i in (0, cfg.n_mb - 1):
+        a, b = int(wl.mb_off_h[i]), int(wl.mb_off_h[i + 1])
+        key = np.repeat(wl.tok_src_h[a:b].astype(np.int64), cfg.K) * cfg.E + ids_h[a:b].reshape(-1)
+        w_se = np.bincount(key, minlength=cfg.P * cfg.E).reshape(cfg.P, cfg.E).astype(np.int32)
+        ref = orc.quota_tradeoff(w_se, wl.se_h[0], cfg.P, cfg.Ns, M, 1, 1)
+        assert ref["fault"] == 0 and int(tp.member[i, 0]) == ref["member"]
+        assert tp.F[:, i, 0].cpu().numpy().tolist() == ref["F"].tolist()
+        assert (tp.quota[i, 0].cpu().numpy() == ref["quota_v"]).all()
+        assert (tp.traffic[i, 0].cpu().numpy() == ref["traffic"]).all()
+        ids_v = (ids_h[a:b].astype(np.int64) * M + (wl.tok_src_h[a:b] // R)[:, None]).astype(np.int32)
+        ps, inv, perm, f = orc.assign_instance(ids_v, ref["se_v"], ref["quota_v"], ref["slot_off_v"], cfg.E * M,
+                                               base=a * cfg.K)
+        assert f == 0 and (tp.inv[0, a:b].cpu().numpy().ravel() == inv).all()
+    _library_data_checks(wl, [wl.instances[0], wl.instances[-1]])

@@ -751,6 +751,186 @@ done:
 }
 
 /* ==========================================================================================
+ * O16 oracle_replica_search: Alg. 2 Stage 3, expert replication by a search over (expert, rank)
+ * candidates (sec. 8.2 prose; listing lines 14-19), ONE instance.
+ *   "With Stage 2's placement fixed, P * N_r redundant slots remain.  We allocate them one at a time.
+ *    At each step, for every (expert, rank) candidate, we estimate the objective reduction obtained by
+ *    adding that replica using a locality-aware token assignment heuristic: tokens prefer same-machine
+ *    replicas to avoid cross-machine traffic, and any leftover tokens are routed to minimize per-rank
+ *    load.  The candidate yielding the largest reduction is selected.  The loop terminates when all
+ *    redundant slots are filled or no candidate improves the objective."
+ * Reading 40 fixes what the paper leaves open:
+ *   state   every slot j holding expert e carries flows x[j][m] = tokens of e from the sources of
+ *           machine m that j serves; RL[r] = sum over the slots of r (Eq.(4)); LT[i][j] = tokens from
+ *           machine i served on machine j (Eq.(5) off the diagonal).  Initially every expert has its
+ *           base slot only (Stage 2's result): x[j][m] = c[m][e].
+ *   objective  F = a * max_r RL[r] + b * max_{i != j} LT[i][j]  (as O12, reading 33).
+ *   estimate of candidate (e, r) -- r has a free redundant slot, does not host e, e has tokens and
+ *           fewer than max_copies hosts: ONLY e's tokens are re-assigned (everything else stays), over
+ *           hosts(e) + r, by the locality-aware heuristic in ONE pass: commodities (e, m) in descending
+ *           count (ties ascending m); commodity (e, m) may use the hosts on machine m if there is one,
+ *           else all hosts; its tokens go one at a time to the allowed host whose rank is least loaded
+ *           (ties: lowest rank).  Delta = F(after) - F(now).
+ *   choice  the smallest Delta; ties: lowest expert id, then lowest rank.  "if Delta >= 0 then break".
+ *           The replica goes to r's next free redundant slot and the estimate becomes the state.
+ *   at most P * N_r rounds.
+ * placed_se: every expert exactly once in the base slots (O12's / O8-Stage-2's output); its redundant
+ * slots are not read.  out_se: base slots copied, redundant slots filled or -1.
+ * stats (may be NULL): [0] replicas placed, [1] F before, [2] F after.
+ * Pins (tests/test_oracle_replica_search.py): every round replayed from the output by an independent
+ * Python implementation with the CLOSED-FORM water-fill (another algorithmic form than the unit loop
+ * below); F strictly decreasing and equal to a numpy recomputation from the final flows; structure;
+ * M = 1 / b = 0 special cases; a hand-worked vector (tests/golden/replica_search_vectors.json).
+ * ========================================================================================== */
+static int64_t swap_objective(int P, int M, int64_t a, int64_t b, const int64_t *RL, const int64_t *LT);   /* O12, below */
+
+typedef struct {
+  int E, P, Ns, Nb, M, R;
+  int64_t a, b;
+  const int32_t *c_me;      /* [M][E] */
+  int32_t *se;              /* [S] current placement */
+  int64_t *x;               /* [S][M] flows */
+  int64_t *RL;              /* [P] */
+  int64_t *LT;              /* [M][M] */
+} rs_state_t;
+
+static int64_t rs_objective(const rs_state_t *st, const int64_t *RL, const int64_t *LT) {
+  return swap_objective(st->P, st->M, st->a, st->b, RL, LT);
+}
+
+/* the locality-aware re-assignment of expert e over its current hosts plus (optionally) rank r_new.
+ * Writes RL2 / LT2 (the state with e re-assigned) and xnew[rank][m]; returns F(after). */
+static int64_t rs_estimate(const rs_state_t *st, int e, int r_new, int64_t *RL2, int64_t *LT2,
+                           int64_t *xnew /* [P][M] */, int32_t *is_host /* [P] */) {
+  const int P = st->P, M = st->M, Ns = st->Ns, R = st->R, E = st->E;
+  memcpy(RL2, st->RL, sizeof(int64_t) * (size_t)P);
+  memcpy(LT2, st->LT, sizeof(int64_t) * (size_t)M * M);
+  for (int r = 0; r < P; r++) { is_host[r] = 0; for (int m = 0; m < M; m++) xnew[(size_t)r * M + m] = 0; }
+  for (int j = 0; j < P * Ns; j++) {            /* take e's tokens out */
+    if (st->se[j] != e) continue;
+    const int r = j / Ns;
+    is_host[r] = 1;
+    for (int m = 0; m < M; m++) {
+      RL2[r] -= st->x[(size_t)j * M + m];
+      LT2[m * M + r / R] -= st->x[(size_t)j * M + m];
+    }
+  }
+  if (r_new >= 0) is_host[r_new] = 1;
+  /* commodities (e, m): descending count, ties ascending m */
+  int32_t order[128];
+  int n = 0;
+  for (int m = 0; m < M; m++) if (st->c_me[(size_t)m * E + e] > 0) order[n++] = m;
+  for (int u = 1; u < n; u++) {
+    const int m = order[u];
+    int v = u;
+    while (v > 0 && st->c_me[(size_t)order[v - 1] * E + e] < st->c_me[(size_t)m * E + e]) { order[v] = order[v - 1]; v--; }
+    order[v] = m;
+  }
+  for (int u = 0; u < n; u++) {
+    const int m = order[u];
+    int local = 0;
+    for (int r = m * R; r < (m + 1) * R; r++) local |= is_host[r];
+    for (int32_t t = 0; t < st->c_me[(size_t)m * E + e]; t++) {      /* one token at a time */
+      int best = -1;
+      for (int r = 0; r < P; r++) {
+        if (!is_host[r] || (local && r / R != m)) continue;
+        if (best < 0 || RL2[r] < RL2[best]) best = r;
+      }
+      RL2[best] += 1;
+      LT2[m * M + best / R] += 1;
+      xnew[(size_t)best * M + m] += 1;
+    }
+  }
+  return rs_objective(st, RL2, LT2);
+}
+
+int oracle_replica_search(int E, int P, int Nb, int Nr, int M, int max_copies, int64_t a, int64_t b,
+                          const int32_t *c_me /* [M][E] */, const int32_t *placed_se, int32_t *out_se,
+                          int64_t *stats /* [3] or NULL */) {
+  const int Ns = Nb + Nr, S = P * Ns;
+  if (M <= 0 || M > 128 || P % M != 0 || max_copies < 1 || a < 0 || b < 0) return ORACLE_BAD_ARG;
+  int fault = 0;
+  rs_state_t st = {E, P, Ns, Nb, M, P / M, a, b, c_me, out_se, NULL, NULL, NULL};
+  int64_t *ctot = (int64_t *)calloc((size_t)E, sizeof(int64_t));
+  int32_t *seen = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *nhost = (int32_t *)calloc((size_t)E, sizeof(int32_t));
+  int32_t *nred = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int32_t *is_host = (int32_t *)calloc((size_t)P, sizeof(int32_t));
+  int64_t *RL2 = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  int64_t *LT2 = (int64_t *)calloc((size_t)M * M, sizeof(int64_t));
+  int64_t *xnew = (int64_t *)calloc((size_t)P * M, sizeof(int64_t));
+  st.x = (int64_t *)calloc((size_t)S * M, sizeof(int64_t));
+  st.RL = (int64_t *)calloc((size_t)P, sizeof(int64_t));
+  st.LT = (int64_t *)calloc((size_t)M * M, sizeof(int64_t));
+  for (int j = 0; j < S; j++) out_se[j] = -1;
+  if (!ctot || !seen || !nhost || !nred || !is_host || !RL2 || !LT2 || !xnew || !st.x || !st.RL || !st.LT) {
+    fault = ORACLE_NO_MEM; goto done;
+  }
+  for (int e = 0; e < E; e++)
+    for (int m = 0; m < M; m++) {
+      if (c_me[(size_t)m * E + e] < 0) fault |= FAULT_ID_RANGE;
+      ctot[e] += c_me[(size_t)m * E + e];
+    }
+  for (int j = 0; j < S; j++) {
+    if (j % Ns >= Nb) continue;                          /* the input's redundant slots are not read */
+    const int32_t e = placed_se[j];
+    if (e < -1 || e >= E) { fault |= FAULT_SLOT_EXPERT; continue; }
+    if (e < 0) continue;
+    if (seen[e]) fault |= FAULT_SLOT_EXPERT;
+    seen[e] = 1;
+  }
+  for (int e = 0; e < E; e++) if (!seen[e]) fault |= FAULT_SLOT_EXPERT;
+  if (fault) goto done;
+  for (int j = 0; j < S; j++) {
+    if (j % Ns >= Nb || placed_se[j] < 0) continue;
+    const int e = placed_se[j], r = j / Ns;
+    out_se[j] = e;
+    nhost[e] = 1;
+    for (int m = 0; m < M; m++) {
+      st.x[(size_t)j * M + m] = c_me[(size_t)m * E + e];
+      st.RL[r] += c_me[(size_t)m * E + e];
+      st.LT[m * M + r / st.R] += c_me[(size_t)m * E + e];
+    }
+  }
+  const int64_t F0 = rs_objective(&st, st.RL, st.LT);
+  int64_t F = F0;
+  int placed = 0;
+  for (int round = 0; round < P * Nr; round++) {
+    int64_t best_delta = 0;
+    int best_e = -1, best_r = -1;
+    for (int e = 0; e < E; e++) {
+      if (ctot[e] <= 0 || nhost[e] >= max_copies) continue;
+      for (int r = 0; r < P; r++) {
+        if (nred[r] >= Nr) continue;
+        int hosted = 0;
+        for (int j = r * Ns; j < (r + 1) * Ns; j++) hosted |= (out_se[j] == e);
+        if (hosted) continue;
+        const int64_t delta = rs_estimate(&st, e, r, RL2, LT2, xnew, is_host) - F;
+        if (delta < best_delta) { best_delta = delta; best_e = e; best_r = r; }   /* strict: first wins ties */
+      }
+    }
+    if (best_e < 0) break;                                /* "if Delta >= 0 then break" */
+    F = rs_estimate(&st, best_e, best_r, RL2, LT2, xnew, is_host);
+    out_se[best_r * Ns + Nb + nred[best_r]] = best_e;
+    nred[best_r] += 1;
+    nhost[best_e] += 1;
+    memcpy(st.RL, RL2, sizeof(int64_t) * (size_t)P);
+    memcpy(st.LT, LT2, sizeof(int64_t) * (size_t)M * M);
+    for (int j = 0; j < S; j++) {
+      if (out_se[j] != best_e) continue;
+      for (int m = 0; m < M; m++) st.x[(size_t)j * M + m] = xnew[(size_t)(j / Ns) * M + m];
+    }
+    placed++;
+  }
+  if (stats) { stats[0] = placed; stats[1] = F0; stats[2] = F; }
+done:
+  if (fault > 0) for (int j = 0; j < S; j++) out_se[j] = -1;
+  free(ctot); free(seen); free(nhost); free(nred); free(is_host); free(RL2); free(LT2); free(xnew);
+  free(st.x); free(st.RL); free(st.LT);
+  return fault;
+}
+
+/* ==========================================================================================
  * O15 oracle_quota_tradeoff: per-source Stage 4 under the objective of Eq.(10),
  *     F = a * L* + b * C*,   L* = max_r L_r (Eq.(4)),  C* = max_{i != j} C_{i,j} (Eq.(5)),
  * with caller-supplied non-negative integers a ~ n1*K1, b ~ n2*K2 (the paper

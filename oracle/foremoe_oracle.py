@@ -211,6 +211,21 @@ def quota_local(w_se: np.ndarray, slot_expert: np.ndarray, P: int, Ns: int, M: i
     return out
 
 
+def replica_search(c_me: np.ndarray, placed_se: np.ndarray, P: int, Nb: int, Nr: int, M: int = 1,
+                   a: int = 1, b: int = 0, max_copies: int = 8):
+    """O16 for one instance: per-source-machine loads int32 [M,E] (or [E] with M = 1), placement with final
+    base slots [S] -> placement with the redundant slots filled by Alg. 2 Stage 3, stats (replicas, F before,
+    F after), fault."""
+    c_me = _i32(c_me).reshape(M, -1)
+    placed_se = _i32(placed_se)
+    out = np.full(P * (Nb + Nr), -1, dtype=np.int32)
+    stats = np.zeros(3, dtype=np.int64)
+    f = lib().oracle_replica_search
+    f.argtypes = [C.c_int] * 6 + [C.c_int64, C.c_int64] + [C.c_void_p] * 4
+    fault = f(c_me.shape[1], P, Nb, Nr, M, max_copies, a, b, _p(c_me), _p(placed_se), _p(out), _p(stats))
+    return out, stats, fault
+
+
 DEFAULT_LADDER = ((0, 0), (2, 1), (1, 1), (1, 2), (1, 4), (0, 1))   # theta = inf, 2, 1, 1/2, 1/4, 0 as (num, den)
 
 

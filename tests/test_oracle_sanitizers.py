@@ -12,7 +12,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 PINS = ["tests/test_oracle_quota.py", "tests/test_oracle_path.py", "tests/test_oracle_placement.py",
-        "tests/test_oracle_swap.py", "tests/test_oracle_local.py", "tests/test_oracle_backward.py"]
+        "tests/test_oracle_swap.py", "tests/test_oracle_local.py", "tests/test_oracle_backward.py",
+        "tests/test_oracle_tradeoff.py", "tests/test_oracle_replica_search.py"]
 
 
 def _runtime(name):

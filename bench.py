@@ -253,7 +253,14 @@ class Workload:
         self.se_h = synth.gen_placement(cfg, step_hist)
         self.plan.slot_expert.copy_(torch.from_numpy(self.se_h))
         self.machines, self.planner = machines, planner
-        if planner == "full":   # Stages 1-4 on the device: the harness placement above is not used
+        if planner == "alg2":   # Alg. 1 + Alg. 2 Stages 2-4 on the device (the paper's recompute-stage planner)
+            self.plan = None
+            M = max(machines, 1)
+            self.tok_src_h = synth.gen_tok_src(cfg)
+            a, b = objective if objective else (1, 0)
+            self.plan = runner.Alg2StepPlan(s, M, a, b, ids, w, mb_off, torch.from_numpy(self.tok_src_h).to(dev))
+            self.real_shape, self.shape = s, self.plan.shape
+        elif planner == "full":   # Stages 1-4 on the device: the harness placement above is not used
             self.plan = None
             self.plan = runner.PlannerStepPlan(s, max(machines, 1), ids, w, mb_off)
             self.shape = self.plan.shape
@@ -277,9 +284,11 @@ class Workload:
         self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
         self.routed_tokens = sum(tok) * s.L
         self.stage = stage
-        n_lad = len(runner.DEFAULT_LADDER) if (objective and machines and planner != "full") else 0
+        n_lad = len(runner.DEFAULT_LADDER) if (objective and machines and planner not in ("full", "alg2")) else 0
+        if planner == "alg2":
+            n_lad = len(self.plan.ladder)
         self.launches_per_step = (2 + 5 + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
-                                  + n_lad * 5 + (1 if n_lad else 0)
+                                  + n_lad * 5 + (1 if n_lad else 0) + (4 if planner == "alg2" else 0)
                                   + (4 if stage == "update" else 2) * len(self.instances))
         if stage == "update":          # forward + backward of every instance
             self.dy = torch.randn((mx, s.H), dtype=torch.float32, device=dev,
@@ -547,7 +556,9 @@ def run_ours(args, cfg) -> None:
     rl = wl.plan.rank_load.float()
     live = rl.sum(-1) > 0
     ratio = (rl.max(-1).values / rl.mean(-1).clamp(min=1e-9))[live]
-    hist_real = wl.plan.hist if (not args.machines or args.planner == "full") else wl.plan.hist.view(cfg.n_mb, cfg.L, cfg.E, args.machines).sum(-1)
+    virt = args.planner == "alg2" or (args.machines and args.planner != "full")
+    Mv = max(args.machines, 1)
+    hist_real = wl.plan.hist.view(cfg.n_mb, cfg.L, cfg.E, Mv).sum(-1) if virt else wl.plan.hist
     nat = hist_real.float().view(cfg.n_mb, cfg.L, cfg.P, cfg.Nb).sum(-1)
     nratio = (nat.max(-1).values / nat.mean(-1).clamp(min=1e-9))[live]
     balance = {"lmax_over_lmean": {"max": float(ratio.max()), "mean": float(ratio.mean()),
@@ -555,15 +566,18 @@ def run_ours(args, cfg) -> None:
                "natural_placement": {"max": float(nratio.max()), "mean": float(nratio.mean()),
                                      "median": float(nratio.median())}}
 
-    if args.machines and args.planner != "full":
+    if virt:
         tr = wl.plan.traffic.double()
         tot = tr.sum((-1, -2)).clamp(min=1)
         cross = (tot - tr.diagonal(dim1=-2, dim2=-1).sum(-1)) / tot
         off = tr.clone()
         off.diagonal(dim1=-2, dim2=-1).zero_()
-        balance["machines"] = args.machines
-        if objective:
-            balance["objective"] = {"a": objective[0], "b": objective[1],
+        balance["machines"] = Mv
+        if args.planner == "alg2":
+            balance["alg2"] = {"swaps_mean": float(wl.plan.swaps[live].float().mean()),
+                               "replicas_mean": float(wl.plan.replicas[live].float().mean())}
+        if objective or args.planner == "alg2":
+            balance["objective"] = {"a": wl.plan.a, "b": wl.plan.b,
                                     "members_chosen": torch.bincount(wl.plan.member[live].flatten().long(),
                                                                      minlength=len(wl.plan.ladder)).tolist(),
                                     "ladder": [list(t) for t in wl.plan.ladder]}
@@ -586,9 +600,9 @@ def run_ours(args, cfg) -> None:
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
     verify = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline and not upd and not args.machines and args.planner != "full":
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not upd and not args.machines and args.planner == "stage4":
         verify = capture_instance(wl, wl.instances[len(wl.instances) // 2])
-    if not args.no_e2e and not upd and not args.machines and args.planner != "full":
+    if not args.no_e2e and not upd and not args.machines and args.planner == "stage4":
         line["e2e"] = run_e2e(args, cfg, wl, dev)
     else:
         wl.release()
@@ -655,10 +669,12 @@ def main() -> None:
     ap.add_argument("--objective", default="",
                     help="with --machines: 'a,b' = Stage 4 under F = a*L_max + b*C_max (Eq.(10)) over the "
                          "locality-threshold ladder instead of the hard locality rule")
-    ap.add_argument("--planner", default="stage4", choices=["stage4", "full"],
+    ap.add_argument("--planner", default="stage4", choices=["stage4", "full", "alg2"],
                     help="stage4 = the headline path (step-level placement is an input, Stage 4 on the GPU); "
                          "full = Stage 1 + Alg. 3 Stages 2-3 + Stage 4 all on the GPU inside the timed step "
-                         "(--machines M then restricts relocation / replication to machines of P/M ranks)")
+                         "(--machines M then restricts relocation / replication to machines of P/M ranks); "
+                         "alg2 = Alg. 1 + Alg. 2 Stages 2-4 (swaps, replica search, Stage 4 under --objective a,b "
+                         "over --machines M) on the GPU inside the timed step")
     ap.add_argument("--streams", type=int, default=1,
                     help="> 1: interleave the independent instances over that many CUDA streams")
     ap.add_argument("--no-e2e", action="store_true")

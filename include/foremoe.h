@@ -360,8 +360,8 @@ int foremoe_swap_relocation(const foremoe_shape_t *shape, int32_t M, int32_t win
  * (NEXT) Stage 3 alone: replication on per-micro-step placements whose base
  * slots are already final -- the output of foremoe_swap_relocation -- with Alg. 3's choice rule
  * (readings 22-25), so that Alg. 2's relocation by swaps, replication
- * and Stage 4 compose.  (Alg. 2's own replica score, an "estimated drop" under a locality-aware
- * assignment, is not defined precisely enough to restate: DESIGN.md reading 36.)
+ * and Stage 4 compose.  (Alg. 2's own replica score, the "estimated drop" under a locality-aware
+ * assignment of PAPER.md:337, is foremoe_replica_search below.)
  *   hist                  [n_mb][L][E] micro-step loads.
  *   placed_slot_expert_mb [n_mb][L][S]: every expert exactly once in the base slots; the
  *                         redundant slots of the input are not read.
@@ -372,6 +372,36 @@ int foremoe_swap_relocation(const foremoe_shape_t *shape, int32_t M, int32_t win
 int foremoe_replication(const foremoe_shape_t *shape, int32_t M, const int32_t *hist,
                         const int32_t *placed_slot_expert_mb, int32_t *slot_expert_mb,
                         int32_t *dev_status, void *stream);
+
+/*
+ * (NEXT) Alg. 2 Stage 3: expert replication by a search over (expert, rank) candidates (PAPER.md:337
+ * sec. 8.2; listing lines 14-19) for every (micro-step, layer) instance, on
+ * placements whose base slots are final (foremoe_swap_relocation's output).  State: every slot
+ * holding expert e carries the tokens of e it serves per source machine; RL[r] (Eq.(4)) and LT[i][j]
+ * (Eq.(5)) follow.  Each round, for every candidate (e, r) -- rank r has a free redundant slot, does
+ * not host e, e has tokens and fewer than max_copies hosts -- ONLY e's tokens are re-assigned over
+ * hosts(e) + r by the locality-aware heuristic ("tokens prefer same-machine replicas ..., any leftover
+ * tokens are routed to minimize per-rank load"): commodities (e, m) in descending count (ties
+ * ascending m), each over the hosts on machine m if there is one, else all hosts, token by token to
+ * the least-loaded allowed rank (ties: lowest rank).  Delta = change of F = a * max_r RL +
+ * b * max_{i != j} LT (a, b as in foremoe_swap_relocation).  The smallest Delta wins (ties: lowest
+ * expert id, then lowest rank); "if Delta >= 0 then break"; otherwise the replica takes r's next
+ * free redundant slot and the estimate becomes the state; at most P * N_r replicas (DESIGN.md
+ * reading 40).
+ *   hist_v                [n_mb][L][E*M] (as foremoe_swap_relocation).
+ *   placed_slot_expert_mb [n_mb][L][S]: every expert exactly once in the base slots; redundant slots
+ *                         are not read.
+ *   slot_expert_mb        [n_mb][L][S] out (may alias the input): base slots copied, redundant slots
+ *                         filled front to back or -1.
+ *   replicas              [n_mb][L] out or NULL: replicas placed.
+ *   F                     [n_mb][L][2] int64 out or NULL: objective before / after.
+ *   M <= 32, 1 <= max_copies <= 31.
+ * Faults: SLOT_EXPERT, ID_RANGE as in foremoe_replication (instance output all -1).
+ */
+int foremoe_replica_search(const foremoe_shape_t *shape, int32_t M, int32_t max_copies, int64_t a, int64_t b,
+                           const int32_t *hist_v, const int32_t *placed_slot_expert_mb,
+                           int32_t *slot_expert_mb, int32_t *replicas, int64_t *F, int32_t *dev_status,
+                           void *stream);
 
 /* Bytes of device arena foremoe_step_host needs for this shape (includes the assign workspace).
  * mb_off_h: host [n_mb+1] (the arena holds activations of the largest micro-step).  Host only. */

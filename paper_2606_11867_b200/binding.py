@@ -39,7 +39,7 @@ EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_warmup", "fore
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
            "foremoe_local_placement_theta", "foremoe_tradeoff_select",
-           "foremoe_swap_relocation", "foremoe_replication",
+           "foremoe_swap_relocation", "foremoe_replication", "foremoe_replica_search",
            "foremoe_microstep_placement", "foremoe_step_host_arena_bytes", "foremoe_step_host")
 
 
@@ -130,6 +130,7 @@ def lib() -> C.CDLL:
         l.foremoe_local_placement_theta.argtypes = [sp, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp]
         l.foremoe_tradeoff_select.argtypes = [sp, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_replication.argtypes = [sp, i32, vp, vp, vp, vp, vp]
+        l.foremoe_replica_search.argtypes = [sp, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_swap_relocation.argtypes = [sp, i32, i32, i32, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp]
         l.foremoe_microstep_placement.argtypes = [sp, i32, vp, vp, vp, vp, vp]
         l.foremoe_step_host_arena_bytes.argtypes = [sp, vp, C.POINTER(sz)]
@@ -387,6 +388,15 @@ def replication(shape: Shape, M: int, hist, placed_slot_expert_mb, slot_expert_m
     _check("foremoe_replication", lib().foremoe_replication(
         C.byref(shape.c()), M, _dev(hist, torch.int32), _dev(placed_slot_expert_mb, torch.int32),
         _dev(slot_expert_mb, torch.int32), _dev(dev_status, torch.int32), _stream()))
+
+
+def replica_search(shape: Shape, M: int, max_copies: int, a: int, b: int, hist_v, placed_slot_expert_mb,
+                   slot_expert_mb, replicas=None, F=None, dev_status=None) -> None:
+    """(NEXT) Alg. 2 Stage 3: hist_v [n_mb,L,E*M] + placements with final base slots -> slot_expert_mb."""
+    _check("foremoe_replica_search", lib().foremoe_replica_search(
+        C.byref(shape.c()), M, max_copies, a, b, _dev(hist_v, torch.int32),
+        _dev(placed_slot_expert_mb, torch.int32), _dev(slot_expert_mb, torch.int32),
+        _dev(replicas, torch.int32), _dev(F, torch.int64), _dev(dev_status, torch.int32), _stream()))
 
 
 def virtual_shape(shape: Shape, M: int) -> Shape:

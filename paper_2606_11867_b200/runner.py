@@ -130,9 +130,12 @@ class TradeoffStepPlan(LocalStepPlan):
 
     def plan(self, quota_in: Optional[torch.Tensor] = None) -> None:
         assert quota_in is None
-        rs, M = self.real_shape, self.M
-        fm.source_ids(rs, M, self.real_ids, self.tok_src, self.ids, self.status)
+        fm.source_ids(self.real_shape, self.M, self.real_ids, self.tok_src, self.ids, self.status)
         self.load_hist()
+        self._stage4()
+
+    def _stage4(self) -> None:
+        rs, M = self.real_shape, self.M
         for k, (num, den) in enumerate(self.ladder):
             fm.local_placement_theta(rs, M, num, den, self.hist, self.real_slot_expert, self.se_v_k[k], self.status)
             fm.assign(self.shape, self.ids, self.mb_off, self.hist, self.se_v_k[k], None, self.quota_k[k],
@@ -142,6 +145,46 @@ class TradeoffStepPlan(LocalStepPlan):
                            self.member, self.F, self.quota_sel, self.slot_expert)
         self.assign(self.quota_sel)
         fm.traffic(rs, M, self.quota, self.traffic)
+
+
+class Alg2StepPlan(TradeoffStepPlan):
+    """The paper's planner for the recompute stage, all on the device: Alg. 1 (Stage 1, machine + rank
+    level) from the step totals, then per (micro-step, layer) Alg. 2 Stage 2 (relocation by swaps), Stage
+    3 (replica search) and Stage 4 under the same objective F = a * L_max + b * C_max (PAPER.md:282-407;
+    DESIGN.md readings 33-35, 37, 39, 40).  ``slot_expert_mb`` [n_mb,L,S] is the per-instance placement
+    of Stages 1-3; the plan's own ``slot_expert`` / ``quota`` / ``inv`` refer to the commodity instance
+    as in TradeoffStepPlan."""
+
+    def __init__(self, shape: fm.Shape, M: int, a: int, b: int, ids, w, mb_off, tok_src, win: int = 4,
+                 max_rounds: int = 32, max_copies: int = 8, ladder=None):
+        import dataclasses
+        dev = ids.device
+        if ladder is None:
+            ladder = DEFAULT_LADDER if M > 1 else ((0, 1),)        # one machine: every member is the same
+        base = torch.empty((shape.L, shape.S), dtype=torch.int32, device=dev)
+        super().__init__(shape, M, a, b, ids, w, mb_off, base, tok_src, ladder)
+        self.base_slot_expert = base
+        self.win, self.max_rounds, self.max_copies = win, max_rounds, max_copies
+        self.slot_expert_mb = torch.empty((shape.n_mb, shape.L, shape.S), dtype=torch.int32, device=dev)
+        self.swaps = torch.empty((shape.n_mb, shape.L), dtype=torch.int32, device=dev)
+        self.replicas = torch.empty((shape.n_mb, shape.L), dtype=torch.int32, device=dev)
+        self.F_stage3 = torch.empty((shape.n_mb, shape.L, 2), dtype=torch.int64, device=dev)
+        self.base_shape = shape
+        # Stages 2-3 hand Stage 4 one placement per instance
+        self.real_shape = dataclasses.replace(shape, placement_mb_stride=shape.L * shape.S)
+        self.real_slot_expert = self.slot_expert_mb
+
+    def plan(self, quota_in: Optional[torch.Tensor] = None) -> None:
+        assert quota_in is None
+        bs, M = self.base_shape, self.M
+        fm.source_ids(bs, M, self.real_ids, self.tok_src, self.ids, self.status)
+        self.load_hist()                                           # hist_v and its step totals
+        fm.base_placement_machines(bs, M, self.a, self.b, self.step_hist, self.base_slot_expert, self.status)
+        fm.swap_relocation(bs, M, self.win, self.max_rounds, self.a, self.b, self.hist, self.base_slot_expert,
+                           self.slot_expert_mb, self.swaps, self.status)
+        fm.replica_search(bs, M, self.max_copies, self.a, self.b, self.hist, self.slot_expert_mb,
+                          self.slot_expert_mb, self.replicas, self.F_stage3, self.status)
+        self._stage4()
 
 
 class PlannerStepPlan(StepPlan):

@@ -279,3 +279,102 @@ def test_base_placement_machines(cuda_device, seed):
     assert int(st.item()) & fm.FAULT_ID_RANGE and (out[3] == -1).all() and (out[0].cpu().numpy() == got[0]).all()
     with pytest.raises(fm.ForeMoEError):
         fm.base_placement_machines(shape, M, -1, b, torch.as_tensor(neg).to(dev), out, st)
+
+
+# ------------------------------------------------------------------ Alg. 2 Stage 3: replica search (O16)
+@pytest.mark.parametrize("seed", range(8))
+def test_replica_search(cuda_device, seed):
+    """foremoe_replica_search against oracle O16 on random instances: placements bit for bit, number of
+    replicas and objective before / after; the golden four-round vector; faults."""
+    rng = np.random.default_rng(600 + seed)
+    P, M, Nb, Nr = [(4, 1, 2, 1), (4, 2, 1, 1), (8, 2, 4, 2), (8, 4, 2, 2), (6, 3, 3, 1), (16, 4, 4, 1),
+                    (8, 8, 2, 2), (32, 8, 2, 1)][seed]
+    a, b = [(1, 0), (1, 1), (2, 1), (1, 3), (1, 1), (3, 2), (1, 2), (1, 1)][seed]
+    maxc = [8, 8, 3, 2, 8, 4, 8, 8][seed]
+    E, L, n_mb, Ns = P * Nb, 2, 5, Nb + Nr
+    shape = fm.Shape(L=L, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=n_mb, H=8, act_dtype=fm.ACT_FP32)
+    hv = (rng.integers(0, 80, size=(n_mb, L, E, M)) * (rng.random((n_mb, L, E, M)) < 0.7)).astype(np.int32)
+    hot = rng.choice(E, size=max(1, E // 6), replace=False)
+    hv[:, :, hot] *= 7
+    hv[4] = 0                                                         # an empty micro-step: nothing to place
+    hv[3, 1] = 5                                                      # all equal: ties only
+    placed = np.full((n_mb, L, P, Ns), -1, dtype=np.int32)
+    for i in range(n_mb):
+        for l in range(L):
+            placed[i, l, :, :Nb] = rng.permutation(E).reshape(P, Nb)
+    placed[..., Nb:] = rng.integers(-1, E, size=(n_mb, L, P, Nr))     # garbage: not read
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    t = lambda x, dt=torch.int32: torch.as_tensor(np.ascontiguousarray(x), dtype=dt).to(dev)
+    out = torch.full((n_mb, L, P * Ns), -7, dtype=torch.int32, device=dev)
+    reps = torch.full((n_mb, L), -7, dtype=torch.int32, device=dev)
+    F = torch.full((n_mb, L, 2), -7, dtype=torch.int64, device=dev)
+    fm.replica_search(shape, M, maxc, a, b, t(hv.reshape(n_mb, L, E * M)), t(placed.reshape(n_mb, L, -1)), out, reps, F, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) == 0
+    got, nrep, Fg = out.cpu().numpy(), reps.cpu().numpy(), F.cpu().numpy()
+    total = 0
+    for i in range(n_mb):
+        for l in range(L):
+            ref, stats, f = orc.replica_search(hv[i, l].T.copy(), placed[i, l].ravel(), P, Nb, Nr, M, a, b, max_copies=maxc)
+            assert f == 0
+            assert (got[i, l] == ref).all(), ("replica_search", seed, i, l, got[i, l].tolist(), ref.tolist())
+            assert nrep[i, l] == stats[0] and Fg[i, l].tolist() == [int(stats[1]), int(stats[2])]
+            total += int(stats[0])
+    assert total > 0 and nrep[4].sum() == 0
+    # in place, and without the optional outputs
+    buf = t(placed.reshape(n_mb, L, -1))
+    fm.replica_search(shape, M, maxc, a, b, t(hv.reshape(n_mb, L, E * M)), buf, buf, None, None, st)
+    torch.cuda.synchronize()
+    assert torch.equal(buf, out)
+
+
+def test_replica_search_golden_faults_and_pipeline(cuda_device):
+    import json, os
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "replica_search_vectors.json")))["vectors"][0]
+    P, Nb, Nr, M = g["P"], g["Nb"], g["Nr"], g["M"]
+    E = P * Nb
+    shape = fm.Shape(L=1, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=1, H=8, act_dtype=fm.ACT_FP32)
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    t = lambda x, dt=torch.int32: torch.as_tensor(np.ascontiguousarray(x), dtype=dt).to(dev)
+    hv = np.array(g["c_me"], dtype=np.int32).T.reshape(1, 1, E * M)             # [e*M + m]
+    out = torch.empty((1, 1, P * (Nb + Nr)), dtype=torch.int32, device=dev)
+    reps = torch.empty((1, 1), dtype=torch.int32, device=dev)
+    F = torch.empty((1, 1, 2), dtype=torch.int64, device=dev)
+    fm.replica_search(shape, M, g["max_copies"], g["a"], g["b"], t(hv), t(np.array(g["placed"]).reshape(1, 1, -1)), out, reps, F, st)
+    torch.cuda.synchronize()
+    assert out.view(P, -1).tolist() == g["out"] and [int(reps.item())] + F.view(-1).tolist() == g["stats"]
+    # faults: an expert twice in the base slots; a negative load
+    bad = np.array(g["placed"]).reshape(1, 1, -1).copy(); bad[0, 0, 0] = bad[0, 0, 2]
+    fm.replica_search(shape, M, 8, 1, 1, t(hv), t(bad), out, reps, F, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) & fm.FAULT_SLOT_EXPERT and (out == -1).all()
+    with pytest.raises(fm.ForeMoEError):
+        fm.replica_search(shape, 3, 8, 1, 1, t(hv), t(bad), out, reps, F, st)          # 3 does not divide P
+    with pytest.raises(fm.ForeMoEError):
+        fm.replica_search(shape, M, 40, 1, 1, t(hv), t(bad), out, reps, F, st)         # max_copies > 31
+    # Alg. 2 end to end on a config-2-shaped trace: Stage 1 -> swaps -> replica search -> Stage 4
+    cfg = synth.config(2).scaled(L=2, n_samples=16, sample_len=512, H=64, mb_samples=4)
+    ids, w, mb_off, _ = G.make_case(cfg)
+    shape = fm.shape_of(cfg)
+    hist, step, _ = orc.load_hist(ids, mb_off, cfg.E)
+    base = np.stack([orc.base_placement(step[l], cfg.P, cfg.Nb, cfg.Nr)[0] for l in range(cfg.L)])
+    swapped, nr, fault = _swap_gpu(shape, 1, 4, 32, 1, 0, hist, base)
+    assert fault == 0
+    st.zero_()
+    full = torch.empty((cfg.n_mb, cfg.L, cfg.S), dtype=torch.int32, device=dev)
+    fm.replica_search(shape, 1, 8, 1, 0, t(hist), t(swapped), full, None, None, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) == 0
+    for i in range(cfg.n_mb):
+        for l in range(cfg.L):
+            ref, _, f = orc.replica_search(hist[i, l], swapped[i, l], cfg.P, cfg.Nb, cfg.Nr, 1, 1, 0)
+            assert f == 0 and (full[i, l].cpu().numpy() == ref).all()
+    shape_mb = dataclasses.replace(shape, placement_mb_stride=shape.L * shape.S)
+    sp_sw = G.gpu_plan(shape_mb, ids, w, mb_off, swapped)
+    sp_rs = G.gpu_plan(shape_mb, ids, w, mb_off, full.cpu().numpy())
+    assert sp_sw.faults() == 0 and sp_rs.faults() == 0
+    m_sw = sp_sw.rank_load.max(-1).values
+    m_rs = sp_rs.rank_load.max(-1).values
+    assert (m_rs <= m_sw).all() and (m_rs < m_sw).any()                # replicas + Stage 4 only help

@@ -192,3 +192,51 @@ def test_lp_solution_fed_through_quota_in(cuda_device):
     tp = tradeoff_plan(shape, M, a, b, ids, w, mb_off, se, tok_src)
     Fsel = tp.F.gather(0, tp.member.long()[None]).squeeze(0).cpu().numpy().astype(float)
     print("ladder F / LP*: mean %.4f max %.4f" % (float((Fsel / lp_val).mean()), float((Fsel / lp_val).max())))
+
+
+@pytest.mark.parametrize("cfg_id,kw,M,a,b", [
+    (2, dict(L=2, n_samples=12, sample_len=700, H=256, mb_samples=4), 2, 1, 1),
+    (2, dict(L=1, n_samples=8, sample_len=500, H=128, mb_samples=4), 1, 1, 0),
+    (3, dict(L=1, n_samples=4, sample_len=1100, H=256, mb_samples=2), 8, 1, 2),
+])
+def test_alg2_planner_chain_equals_oracle_chain(cuda_device, cfg_id, kw, M, a, b):
+    """runner.Alg2StepPlan (Alg. 1 -> swaps -> replica search -> Stage 4 under a*L_max + b*C_max, all on
+    the device) against the same chain of oracles O14 -> O12 -> O16 -> O15, stage by stage."""
+    cfg = synth.config(cfg_id).scaled(**kw)
+    ids, w, mb_off, _ = G.make_case(cfg)
+    tok_src = synth.gen_tok_src(cfg)
+    R = cfg.P // M
+    t = lambda x, dt: torch.as_tensor(np.ascontiguousarray(x), dtype=dt).to(G.DEV)
+    ap = runner.Alg2StepPlan(fm.shape_of(cfg), M, a, b, t(ids, torch.int32), t(w, torch.float32), t(mb_off, torch.int32),
+                             t(tok_src, torch.int32))
+    ap.plan()
+    torch.cuda.synchronize()
+    assert ap.faults() == 0
+    ladder = ap.ladder
+    for l in range(cfg.L):
+        # per-source-machine loads of every instance and of the step
+        c_me = np.zeros((cfg.n_mb, M, cfg.E), dtype=np.int64)
+        for i in range(cfg.n_mb):
+            a0, b0 = int(mb_off[i]), int(mb_off[i + 1])
+            w_se = per_source_counts(ids[l, a0:b0], tok_src[a0:b0], cfg.P, cfg.E)
+            c_me[i] = w_se.reshape(M, R, cfg.E).sum(1)
+        base, f = orc.base_placement_machines(c_me.sum(0), cfg.P, cfg.Nb, cfg.Nr, M, a, b)
+        assert f == 0 and (ap.base_slot_expert[l].cpu().numpy() == base).all(), ("stage 1", l)
+        for i in range(cfg.n_mb):
+            a0, b0 = int(mb_off[i]), int(mb_off[i + 1])
+            sw, st, f = orc.swap_relocation(c_me[i].astype(np.int32), base, cfg.P, cfg.Nb, cfg.Nr, M, ap.win,
+                                            ap.max_rounds, a, b)
+            assert f == 0 and int(ap.swaps[i, l]) == st[0]
+            rs, st3, f = orc.replica_search(c_me[i].astype(np.int32), sw, cfg.P, cfg.Nb, cfg.Nr, M, a, b,
+                                            max_copies=ap.max_copies)
+            assert f == 0 and (ap.slot_expert_mb[i, l].cpu().numpy() == rs).all(), ("stages 2-3", l, i)
+            assert int(ap.replicas[i, l]) == st3[0] and ap.F_stage3[i, l].tolist() == [int(st3[1]), int(st3[2])]
+            w_se = per_source_counts(ids[l, a0:b0], tok_src[a0:b0], cfg.P, cfg.E)
+            ref = orc.quota_tradeoff(w_se, rs, cfg.P, cfg.Ns, M, a, b, ladder=ladder)
+            assert ref["fault"] == 0 and int(ap.member[i, l]) == ref["member"]
+            assert (ap.quota[i, l].cpu().numpy() == ref["quota_v"]).all(), ("stage 4", l, i)
+            assert (ap.traffic[i, l].cpu().numpy() == ref["traffic"]).all()
+            ids_v = (ids[l, a0:b0].astype(np.int64) * M + (tok_src[a0:b0] // R)[:, None]).astype(np.int32)
+            ps, inv, perm, f = orc.assign_instance(ids_v, ref["se_v"], ref["quota_v"], ref["slot_off_v"], cfg.E * M,
+                                                   base=a0 * cfg.K)
+            assert f == 0 and (ap.inv[l, a0:b0].cpu().numpy().ravel() == inv).all()

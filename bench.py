@@ -238,11 +238,13 @@ class Workload:
     recipe in DESIGN.md sec. 4).  Nothing here is timed."""
 
     def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0, planner: str = "stage4",
-                 objective=None):
+                 objective=None, plan_stable: bool = True):
         from paper_2606_11867_b200 import binding as fm
         from paper_2606_11867_b200 import runner
         self.fm, self.cfg, self.dev = fm, cfg, dev
-        self.shape = s = fm.shape_of(cfg)
+        # FOREMOE_FLAG_PLAN_STABLE: ids / w / mb_off are uploaded once and inv is written by foremoe_assign
+        # only, so no kernel launched right before a data-path call writes the plan arrays
+        self.shape = s = fm.shape_of(cfg, flags=fm.FLAG_PLAN_STABLE if plan_stable else 0)
         ids, w, mb_off = synth.gen_trace(cfg, str(dev))
         self.mb_off_h = cfg.mb_off()
         # step-level placement from the step totals (harness-side stand-in for Stages 1-3)
@@ -489,7 +491,7 @@ def run_ours(args, cfg) -> None:
     multi.init("nccl", dev)
     cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
     objective = tuple(int(v) for v in args.objective.split(",")) if args.objective else None
-    wl = Workload(cfg, dev, args.stage, args.machines, args.planner, objective)
+    wl = Workload(cfg, dev, args.stage, args.machines, args.planner, objective, not args.strict_order)
     bpt = bytes_per_token(cfg)
     upd = args.stage == "update"
     total_bpt = bpt["total_update"] if upd else bpt["total"]
@@ -591,6 +593,7 @@ def run_ours(args, cfg) -> None:
         "config": {"workload": workload_name(cfg), "parallelism": f"{world} independent shard(s), no collective",
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
+                   "plan_stable_flag": not args.strict_order,
                    "stage": args.stage, "machines": args.machines, "planner": args.planner,
                    **({"objective": args.objective} if args.objective else {}), "bytes_per_routed_token": total_bpt,
                    **({"sweep_tuning": args.tune} if args.tune else {}),
@@ -677,6 +680,9 @@ def main() -> None:
                          "over --machines M) on the GPU inside the timed step")
     ap.add_argument("--streams", type=int, default=1,
                     help="> 1: interleave the independent instances over that many CUDA streams")
+    ap.add_argument("--strict-order", action="store_true",
+                    help="do not set FOREMOE_FLAG_PLAN_STABLE: the data-path kernels then read nothing, not even "
+                         "the plan arrays, before the preceding kernel of the stream has completed")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cpu-all-cores", action="store_true",

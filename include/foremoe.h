@@ -34,9 +34,15 @@
  *    synchronising.
  *  - Return value: FOREMOE_OK, or a negative host-detectable error (nothing was enqueued).
  *  - Stream order is the only ordering the data-path calls need: their kernels are launched with
- *    programmatic stream serialisation and read nothing from global memory before the grid
- *    dependency is resolved, so inputs written by the preceding kernel of the stream (inv by
+ *    programmatic stream serialisation and, by default, read nothing from global memory before the
+ *    grid dependency is resolved, so inputs written by the preceding kernel of the stream (inv by
  *    foremoe_assign, x / expert_out / w by the caller's kernels) are always seen complete.
+ *    shape.flags = FOREMOE_FLAG_PLAN_STABLE is the caller's promise that the PLAN arrays of the call
+ *    (mb_off, inv, w) are not written by the kernel launched immediately before it on the same
+ *    stream -- foremoe_assign excepted: it ends with a full serialisation point, so calling the data
+ *    path right after it is covered.  The data-path kernels then fetch their first plan entries
+ *    while the preceding kernel drains (activations are still only touched after the dependency);
+ *    worth 4 % at one-sample micro-steps, under 1 % at 16 K tokens (profiles/r02_sweeps.md).
  *  - CUDA graphs: the data-path calls (dispatch, combine, *_bwd) are stream-capturable.  The first
  *    launch of a kernel variant on a device queries occupancy and opts into large shared memory,
  *    which capture does not allow: call foremoe_warmup(shape) once per shape and device before
@@ -75,6 +81,8 @@ extern "C" {
 #define FOREMOE_ACT_BF16 0
 #define FOREMOE_ACT_FP32 1
 
+#define FOREMOE_FLAG_PLAN_STABLE 1  /* see "Stream order" above                                    */
+
 typedef struct {
   int32_t L, E, K;             /* MoE layers, experts, top-k                                   */
   int32_t P, Nb, Nr;           /* logical ranks, base / redundant slots per rank               */
@@ -83,6 +91,7 @@ typedef struct {
   int32_t placement_mb_stride; /* 0: slot_expert is [L][S] (step-level placement);
                                   L*S: slot_expert is [n_mb][L][S] (one placement per micro-step,
                                   PAPER.md:343 A^{(i)})                                         */
+  int32_t flags;               /* 0, or FOREMOE_FLAG_PLAN_STABLE                               */
 } foremoe_shape_t;
 
 /* Library version (major * 100 + minor).  Host only. */

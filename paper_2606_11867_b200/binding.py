@@ -35,6 +35,8 @@ FAULT_SOURCE = 32
 ACT_BF16 = 0
 ACT_FP32 = 1
 
+FLAG_PLAN_STABLE = 1
+
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_warmup", "foremoe_load_hist", "foremoe_assign",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
@@ -53,7 +55,7 @@ class ForeMoEError(RuntimeError):
 
 class _CShape(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("L", "E", "K", "P", "Nb", "Nr", "T", "n_mb", "H",
-                                         "act_dtype", "placement_mb_stride")]
+                                         "act_dtype", "placement_mb_stride", "flags")]
 
 
 @dataclasses.dataclass
@@ -70,6 +72,7 @@ class Shape:
     H: int
     act_dtype: int = ACT_BF16
     placement_mb_stride: int = 0
+    flags: int = 0              # FLAG_PLAN_STABLE: see include/foremoe.h, "Stream order"
 
     @property
     def Ns(self) -> int:
@@ -86,7 +89,7 @@ class Shape:
     def c(self) -> _CShape:
         """The C struct (cached per field tuple: the per-instance calls of a step reuse it)."""
         key = (self.L, self.E, self.K, self.P, self.Nb, self.Nr, self.T, self.n_mb, self.H,
-               self.act_dtype, self.placement_mb_stride)
+               self.act_dtype, self.placement_mb_stride, self.flags)
         hit = _shape_cache.get(key)
         if hit is None:
             if len(_shape_cache) > 256:
@@ -424,8 +427,8 @@ def step_host(shape: Shape, ids_h, w_h, mb_off_h, slot_expert_h, x_h, quota_h, r
         _host(status_h, torch.int32), _stream()))
 
 
-def shape_of(cfg, T: Optional[int] = None, n_mb: Optional[int] = None) -> Shape:
+def shape_of(cfg, T: Optional[int] = None, n_mb: Optional[int] = None, flags: int = 0) -> Shape:
     """Shape of a synth.TraceConfig."""
     return Shape(L=cfg.L, E=cfg.E, K=cfg.K, P=cfg.P, Nb=cfg.Nb, Nr=cfg.Nr,
                  T=cfg.T if T is None else T, n_mb=cfg.n_mb if n_mb is None else n_mb, H=cfg.H,
-                 act_dtype=cfg.act_dtype)
+                 act_dtype=cfg.act_dtype, flags=flags)

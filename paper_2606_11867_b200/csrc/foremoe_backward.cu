@@ -53,14 +53,14 @@ __global__ void __launch_bounds__(256)
 k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
               const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K_rt, int row_vec,
               int n_slices, const int4 *__restrict__ dy, const int4 *__restrict__ eo,
-              int4 *__restrict__ d_eo, float *__restrict__ dw_l) {
+              int4 *__restrict__ d_eo, float *__restrict__ dw_l, int early) {
   constexpr int DY = kBf16 ? 2 : 1;          // 16-byte fp32 vectors of dy per 16-byte row vector
   constexpr int kF = kBf16 ? 8 : 4;
   constexpr int KU = K_T > 0 ? K_T : 32;
   const int K = K_T > 0 ? K_T : K_rt;
   const int NV = DY + (kDw ? K : 0);
   pdl_launch_dependents();
-  pdl_wait();                              // no global read before the predecessor's writes are visible
+  if (!early) pdl_wait();                  // no global read before the predecessor's writes are visible
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t vstride = (uint32_t)nt * 16u, sstride = (uint32_t)NV * vstride;   // bytes; slot (s, j) of this thread:
@@ -122,6 +122,7 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
   for (int k = 0; k < KU; k++) part[k] = 0.f;
 
   fetch_meta(0);
+  if (early) pdl_wait();                   // only mb_off / inv / w were read (FOREMOE_FLAG_PLAN_STABLE)
   for (int n = 0; n < D - 1; n++) issue();
   int c_n = 0;
   for (int c_tok = 0; c_tok < n_my; c_tok++) {
@@ -218,7 +219,7 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
   const int n_slices = (d.row_vec + 31) / 32;
   const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, threads, smem, st, inv_l, w_l, mb_off,
                                    mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)dy,
-                                   (const int4 *)eo, (int4 *)d_eo, dw_l);
+                                   (const int4 *)eo, (int4 *)d_eo, dw_l, d.plan_stable);
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 

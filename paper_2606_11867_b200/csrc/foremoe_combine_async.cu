@@ -25,12 +25,12 @@ template <bool kBf16, int K_T, int D>
 __global__ void __launch_bounds__(768)
 k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
                 const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K_rt, int row_vec,
-                int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
+                int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y, int early) {
   constexpr int kF = kBf16 ? 8 : 4;
   constexpr int KU = K_T > 0 ? K_T : 32;
   const int K = K_T > 0 ? K_T : K_rt;
   pdl_launch_dependents();
-  pdl_wait();                              // no global read before the predecessor's writes are visible
+  if (!early) pdl_wait();                  // no global read before the predecessor's writes are visible
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = nt >> 5;
   const uint32_t kstride = (uint32_t)nt * 16u, sstride = (uint32_t)K * kstride;       // bytes
@@ -91,6 +91,7 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
   };
 
   fetch_meta();
+  if (early) pdl_wait();
   for (int n = 0; n < D - 1; n++) issue();
   for (int j = 0; j < n_my; j++) {
     issue();
@@ -172,7 +173,7 @@ static int launch_one(const Dims &d, int threads, const int32_t *inv_l, const fl
   const int n_slices = (d.row_vec + 31) / 32;
   const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, threads, smem, st, inv_l, w_l, mb_off,
                                    mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)eo,
-                                   (float4 *)y);
+                                   (float4 *)y, d.plan_stable);
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 

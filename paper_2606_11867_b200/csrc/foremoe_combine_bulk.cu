@@ -35,7 +35,7 @@ template <bool kBf16, int K_T, int U>
 __global__ void __launch_bounds__(512)
 k_combine_bulk(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
                const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K_rt, int row_vec,
-               int n_slices, int D, const unsigned char *__restrict__ eo, float4 *__restrict__ y) {
+               int n_slices, int D, const unsigned char *__restrict__ eo, float4 *__restrict__ y, int early) {
   constexpr int kF = kBf16 ? 8 : 4;
   constexpr int KU = K_T > 0 ? K_T : 32;
   constexpr uint32_t SB = 512u * U;
@@ -52,7 +52,7 @@ k_combine_bulk(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
     for (int s = 0; s < D; s++) mbar_init(bars0 + 8u * s, 1);
   fence_proxy_async();
   __syncwarp();
-  pdl_wait();                              // no global read before the predecessor's writes are visible
+  if (!early) pdl_wait();                  // no global read before the predecessor's writes are visible
 
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
@@ -121,6 +121,7 @@ k_combine_bulk(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
       if (q < D) fetch_meta(dq[q], wq[q]);
     }
     fetch_meta(d_nxt, w_nxt);
+    if (early) pdl_wait();
 #pragma unroll
     for (int q = 0; q < kMaxDepth; q++)
       if (q < D) issue(dq[q], wq[q]);
@@ -205,15 +206,14 @@ static int launch_one(const Dims &d, int warps, int D, const int32_t *inv_l, con
   if (prepare) return FOREMOE_OK;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   int per_sm = g_tune.combine_cta_per_sm;
-  if (per_sm <= 0) {      // 32 CTAs per SM, fewer when the mean micro-step has under 2 items per warp
+  if (per_sm <= 0) {      // at least 4 items per warp, between the resident CTAs and 32 per SM (sweep: r02_sweeps.md)
     const long long items = (long long)(d.T / d.n_mb + 1) * n_slices;
-    const long long want = (items + 2LL * warps * num_sms() - 1) / (2LL * warps * num_sms());
-    per_sm = want < 1 ? 1 : want > 32 ? 32 : (int)want;
+    const long long want = items / (4LL * warps * num_sms());
+    per_sm = want < occ ? occ : want > 32 ? 32 : (int)want;
   }
-  (void)occ;
   const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, warps * 32, smem, st, inv_l, w_l, mb_off,
                                    mb_begin, mb_end, d.K, d.row_vec, n_slices, D,
-                                   (const unsigned char *)eo, (float4 *)y);
+                                   (const unsigned char *)eo, (float4 *)y, d.plan_stable);
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 

@@ -26,6 +26,7 @@ struct Dims {
   int n_inst;        // n_mb * L
   int n_pl;          // number of placements: L or n_mb * L
   int pl_per_mb;     // 1 if one placement per micro-step
+  int plan_stable;   // FOREMOE_FLAG_PLAN_STABLE: plan arrays may be read before the grid-dependency wait
   int tpc;           // tokens per chunk
   int max_chunks;    // upper bound on chunks per layer
 };
@@ -55,6 +56,8 @@ inline int make_dims(const foremoe_shape_t *s, Dims *d) {
   if (s->placement_mb_stride == 0) { d->n_pl = s->L; d->pl_per_mb = 0; }
   else if (s->placement_mb_stride == s->L * d->S) { d->n_pl = d->n_inst; d->pl_per_mb = 1; }
   else return FOREMOE_ERR_INVALID_ARG;
+  if (s->flags & ~FOREMOE_FLAG_PLAN_STABLE) return FOREMOE_ERR_INVALID_ARG;
+  d->plan_stable = (s->flags & FOREMOE_FLAG_PLAN_STABLE) ? 1 : 0;
   d->tpc = kChunkPairs / s->K;
   d->max_chunks = (s->T + d->tpc - 1) / d->tpc + s->n_mb;
   return FOREMOE_OK;

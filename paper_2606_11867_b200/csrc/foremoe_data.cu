@@ -16,23 +16,28 @@ template <int U>
 __global__ void __launch_bounds__(256)
 k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb_off, int mb_begin,
                 int mb_end, int K, int row_vec, int n_slices, const int4 *__restrict__ x,
-                int32_t *__restrict__ perm, int4 *__restrict__ buf) {
+                int32_t *__restrict__ perm, int4 *__restrict__ buf, int early) {
   // Nothing in global memory is read before the grid-dependency wait: CUDA guarantees the
   // predecessor's writes (inv from foremoe_assign, x from the caller's kernel) only after it.
   pdl_launch_dependents();
-  pdl_wait();
+  if (!early) pdl_wait();
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const int lane = threadIdx.x & 31;
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
   const long long warps = (long long)gridDim.x * (blockDim.x >> 5);
   const long long item0 = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  int d_first = -1;
+  if (early) {
+    if (item0 < n_items && lane < K) d_first = __ldg(inv_l + (rg.t_begin + (int)(item0 / n_slices)) * K + lane);
+    pdl_wait();
+  }
   for (long long item = item0; item < n_items; item += warps) {
     const int tl = (int)(item / n_slices);
     const int sl = (int)(item - (long long)tl * n_slices);
     const int p0 = (rg.t_begin + tl) * K;
     int d = -1;
     if (lane < K) {
-      d = __ldg(inv_l + p0 + lane);
+      d = (early && item == item0) ? d_first : __ldg(inv_l + p0 + lane);
       if (d >= 0) d -= rg.row0;
       if (perm && sl == 0 && d >= 0) perm[d] = p0 + lane;
     }
@@ -177,7 +182,7 @@ static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *m
   }
   const cudaError_t e = launch_pdl(k_dispatch_rows<U>, num_sms() * per_sm, 256, 0, st, inv_l, mb_off,
                                    mb_begin, mb_end, d.K, d.row_vec, n_slices, (const int4 *)x, perm,
-                                   (int4 *)buf);
+                                   (int4 *)buf, d.plan_stable);
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
@@ -229,7 +234,9 @@ static int check_range(const Dims &d, int layer, int mb_begin, int mb_end) {
 // facts instead)
 int dispatch_rows(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
                   int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st, bool prepare) {
-  if (g_tune.dispatch_impl == 1) {   // default (-1, 0): register-staged rows
+  // auto: the bulk-copy ring wins from 12 KB rows on (config 3's 14 KB rows: 326.7 vs 329.9 us per launch,
+  // profiles/r02_sweeps.md); below that the register-staged kernel is faster (configs 2 and 5)
+  if (g_tune.dispatch_impl == 1 || (g_tune.dispatch_impl < 0 && d.row_bytes >= 12 * 1024)) {
     const int rc = launch_dispatch_tma(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
     if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
   }

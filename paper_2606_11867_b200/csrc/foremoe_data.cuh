@@ -73,8 +73,10 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
 
 // Programmatic dependent launch: the kernel may be scheduled while the previous kernel of the
-// stream drains (hides launch latency and the ramp); it touches no global memory before pdl_wait():
-// the predecessor's writes are only guaranteed visible after the wait, whether or not it triggers early.
+// stream drains (hides launch latency and the ramp).  The predecessor's writes are only guaranteed
+// visible after pdl_wait(), whether or not it triggers early, so a kernel touches no global memory
+// before it -- except the plan arrays (mb_off, inv, w) when the caller set FOREMOE_FLAG_PLAN_STABLE
+// (`early`): then the first plan entries are fetched while the predecessor drains.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 

@@ -12,10 +12,10 @@ namespace foremoe {
 __global__ void __launch_bounds__(512)
 k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb_off, int mb_begin,
                int mb_end, int K, int row_bytes, int NS, const char *__restrict__ x,
-               int32_t *__restrict__ perm, char *__restrict__ buf) {
+               int32_t *__restrict__ perm, char *__restrict__ buf, int early) {
   extern __shared__ __align__(128) unsigned char smem[];
   pdl_launch_dependents();
-  pdl_wait();
+  if (!early) pdl_wait();
   const int n_warps = blockDim.x >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   unsigned char *rows = smem + (size_t)warp * NS * row_bytes;
@@ -23,6 +23,7 @@ k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb
   int32_t *dbuf = (int32_t *)(smem + (size_t)n_warps * NS * row_bytes + (size_t)n_warps * NS * 8) +
                   (size_t)warp * NS * 32;
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
+  if (early) pdl_wait();                   // only mb_off was read (FOREMOE_FLAG_PLAN_STABLE)
   const int n_tok = rg.t_end - rg.t_begin;
   const int W = gridDim.x * n_warps;
   const int w0 = blockIdx.x * n_warps + warp;
@@ -82,10 +83,11 @@ int launch_dispatch_tma(const Dims &d, const int32_t *inv_l, const int32_t *mb_o
   static DeviceMemo memo;
   if (!launch_facts(k_dispatch_tma, memo, warps * 32, smem)) return FOREMOE_ERR_CUDA;
   if (prepare) return FOREMOE_OK;
-  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : 1;
-  k_dispatch_tma<<<num_sms() * per_sm, warps * 32, smem, st>>>(
-      inv_l, mb_off, mb_begin, mb_end, d.K, d.row_bytes, NS, (const char *)x, perm, (char *)buf);
-  return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+  const int per_sm = g_tune.dispatch_cta_per_sm > 0 ? g_tune.dispatch_cta_per_sm : 14;   // sweep: r02_sweeps.md
+  const cudaError_t e = launch_pdl(k_dispatch_tma, num_sms() * per_sm, warps * 32, smem, st, inv_l, mb_off,
+                                   mb_begin, mb_end, d.K, d.row_bytes, NS, (const char *)x, perm, (char *)buf,
+                                   d.plan_stable);
+  return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
 }  // namespace foremoe

@@ -703,6 +703,12 @@ k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_o
   if (fault) raise_fault(dev_status, fault);
 }
 
+// Full serialisation point at the end of foremoe_assign: launched WITHOUT programmatic stream
+// serialisation, it starts only when every kernel above has completed and flushed, so a data-path
+// kernel that follows (launched with it) can overlap nothing that writes the plan -- the basis of
+// FOREMOE_FLAG_PLAN_STABLE's "foremoe_assign excepted".
+__global__ void k_plan_fence() {}
+
 }  // namespace foremoe
 
 // =============================================================================================
@@ -827,5 +833,6 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
         ids, mb_off, chunk_off, pl_host_ptr, pl_host_slot, inst_cum_end, inst_slot_adj, inst_ok,
         chunk_cnt, d.L, d.T, d.K, d.E, d.S, d.n_mb, d.tpc, d.max_chunks, d.pl_per_mb, pair_slot,
         inv, dev_status);
+  k_plan_fence<<<1, 32, 0, st>>>();
   return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }

@@ -48,12 +48,12 @@ def test_header_is_plain_c(tmp_path, lang, std):
     """The boundary is a C ABI: the header compiles on its own as C and as C++ (no torch, no CUDA types)."""
     import subprocess
     src = tmp_path / ("t." + ("c" if lang == "c" else "cpp"))
-    src.write_text('#include "foremoe.h"\nint main(void) { foremoe_shape_t s; (void)s; return sizeof(s) == 44 ? 0 : 1; }\n')
+    src.write_text('#include "foremoe.h"\nint main(void) { foremoe_shape_t s; (void)s; return sizeof(s) == 48 ? 0 : 1; }\n')
     exe = tmp_path / "t"
     subprocess.run(["gcc" if lang == "c" else "g++", "-std=" + std, "-Wall", "-Wextra", "-Werror", "-pedantic",
                     "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
-    assert subprocess.run([str(exe)]).returncode == 0          # 11 x int32: the ctypes mirror has the same size
-    assert C.sizeof(fm._CShape) == 44
+    assert subprocess.run([str(exe)]).returncode == 0          # 12 x int32: the ctypes mirror has the same size
+    assert C.sizeof(fm._CShape) == 48
 
 
 def test_workspace_bytes_and_invalid_shapes(libpath):
@@ -62,7 +62,7 @@ def test_workspace_bytes_and_invalid_shapes(libpath):
     assert 0 < n < (1 << 30)
     import dataclasses
     for bad in (dict(K=0), dict(K=33), dict(E=127), dict(Nb=15), dict(H=7), dict(n_mb=0),
-                dict(act_dtype=2), dict(T=(1 << 31) // 8), dict(placement_mb_stride=5)):
+                dict(act_dtype=2), dict(T=(1 << 31) // 8), dict(placement_mb_stride=5), dict(flags=2)):
         with pytest.raises(fm.ForeMoEError) as ei:
             fm.workspace_bytes(dataclasses.replace(s, **bad))
         assert ei.value.code == fm.ERR_INVALID_ARG

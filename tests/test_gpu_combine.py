@@ -112,12 +112,14 @@ def test_dispatch_bwd_and_combine_share_pairing(cuda_device):
         assert torch.equal(y, eo[inv[:, k]].float() + 0.0), k
 
 
-def test_unsynchronised_pipeline_replan(cuda_device):
+@pytest.mark.parametrize("flags", [0, fm.FLAG_PLAN_STABLE])
+def test_unsynchronised_pipeline_replan(cuda_device, flags):
     """load_hist -> assign -> dispatch -> combine enqueued on one stream with NO synchronise in
     between, after the same buffers held the plan of a DIFFERENT trace: the data-path kernels must
-    see the new inv (they are launched with programmatic stream serialisation; whatever they read
-    before their grid-dependency wait must not come from the plan being written).  Compared with
-    the oracle for the second trace, bit for bit."""
+    see the new inv.  They are launched with programmatic stream serialisation; by default they read
+    nothing before their grid-dependency wait, and with FOREMOE_FLAG_PLAN_STABLE they may read the
+    plan arrays early -- which is still covered right after foremoe_assign, because it ends with a
+    full serialisation point.  Compared with the oracle for the second trace, bit for bit."""
     cfg = synth.config(2).scaled(L=2, n_samples=8, sample_len=900, H=2048, mb_samples=4)
     ids_a, w_a, mb_off, se = G.make_case(cfg)
     cfg_b = synth.config(2).scaled(L=2, n_samples=8, sample_len=900, H=2048, mb_samples=4)
@@ -126,7 +128,7 @@ def test_unsynchronised_pipeline_replan(cuda_device):
     assert (mb_off_b == mb_off).all() and (ids_a != ids_b).any()
     ref = G.oracle_plan(ids_b, mb_off, se, cfg.E, cfg.P, cfg.Ns)
     assert ref["fault"] == 0
-    s = fm.shape_of(cfg)
+    s = fm.shape_of(cfg, flags=flags)
     t = lambda a, dt: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).to(G.DEV)
     ids_d, w_d = t(ids_a, torch.int32), t(w_a, torch.float32)
     ids_bd, w_bd = t(ids_b, torch.int32), t(w_b, torch.float32)

@@ -238,7 +238,7 @@ class Workload:
     recipe in DESIGN.md sec. 4).  Nothing here is timed."""
 
     def __init__(self, cfg, dev, stage: str = "recompute", machines: int = 0, planner: str = "stage4",
-                 objective=None, plan_stable: bool = True):
+                 objective=None, plan_stable: bool = True, mb_per_call: int = 1):
         from paper_2606_11867_b200 import binding as fm
         from paper_2606_11867_b200 import runner
         self.fm, self.cfg, self.dev = fm, cfg, dev
@@ -276,20 +276,29 @@ class Workload:
             else:             # hard locality (reading 30)
                 self.plan = runner.LocalStepPlan(s, machines, ids, w, mb_off, se_dev, src)
             self.real_shape, self.shape = s, self.plan.shape      # same K, H, T, n_mb; E, Nb, Nr x M
-        tok = [int(self.mb_off_h[i + 1] - self.mb_off_h[i]) for i in range(s.n_mb)]
+        # one data-path call covers `mb_per_call` consecutive micro-steps of a layer (ranged calls of the
+        # C ABI; 1 = the order a training loop issues them, the headline).  Call g = micro-steps calls[g].
+        tok_mb = [int(self.mb_off_h[i + 1] - self.mb_off_h[i]) for i in range(s.n_mb)]
+        self.calls = [(i0, min(i0 + mb_per_call, s.n_mb)) for i0 in range(0, s.n_mb, mb_per_call)]
+        tok = [sum(tok_mb[i0:i1]) for (i0, i1) in self.calls]
         self.tok = tok
-        self.x = [synth.gen_activations(cfg, max(n, 1), i, str(dev)) for i, n in enumerate(tok)]
+        if mb_per_call == 1:
+            self.x = [synth.gen_activations(cfg, max(n, 1), i, str(dev)) for i, n in enumerate(tok)]
+        else:
+            self.x = [torch.cat([synth.gen_activations(cfg, max(tok_mb[i], 1), i, str(dev))[:tok_mb[i]]
+                                 for i in range(i0, i1)] + [torch.zeros((1, s.H), dtype=s.act_torch_dtype, device=dev)])
+                      for (i0, i1) in self.calls]
         mx = max(max(tok), 1)
         self.buf = torch.empty((mx * s.K, s.H), dtype=s.act_torch_dtype, device=dev)
         self.y = torch.empty((mx, s.H), dtype=torch.float32, device=dev)
         self.perm = torch.empty((mx * s.K,), dtype=torch.int32, device=dev)
-        self.instances = [(l, i) for l in range(s.L) for i in range(s.n_mb) if tok[i] > 0]
+        self.instances = [(l, g) for l in range(s.L) for g in range(len(self.calls)) if tok[g] > 0]
         self.routed_tokens = sum(tok) * s.L
         self.stage = stage
         n_lad = len(runner.DEFAULT_LADDER) if (objective and machines and planner not in ("full", "alg2")) else 0
         if planner == "alg2":
             n_lad = len(self.plan.ladder)
-        self.launches_per_step = (2 + 5 + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
+        self.launches_per_step = (2 + 6 + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
                                   + n_lad * 5 + (1 if n_lad else 0) + (4 if planner == "alg2" else 0)
                                   + (4 if stage == "update" else 2) * len(self.instances))
         if stage == "update":          # forward + backward of every instance
@@ -299,15 +308,16 @@ class Workload:
             self.dx = torch.empty_like(self.y)
             self.dw = torch.empty((s.L, s.T, s.K), dtype=torch.float32, device=dev)
 
-    def instance(self, l: int, i: int, ev=None):
-        """The data path of one instance; ev (optional) collects CUDA events between the calls."""
+    def instance(self, l: int, g: int, ev=None):
+        """The data path of one instance (call g of layer l); ev (optional) collects CUDA events between the calls."""
         p = self.plan.data_path()          # binding.DataPath: the plan's arguments marshalled once
+        i0, i1 = self.calls[g]
         if ev is None:
-            p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
-            p.combine(l, i, i + 1, self.buf, self.y)
+            p.dispatch(l, i0, i1, self.x[g], self.perm, self.buf)
+            p.combine(l, i0, i1, self.buf, self.y)
             if self.stage == "update":
-                p.combine_bwd(l, i, i + 1, self.dy, self.buf, self.d_buf, self.dw)
-                p.dispatch_bwd(l, i, i + 1, self.d_buf, self.dx)
+                p.combine_bwd(l, i0, i1, self.dy, self.buf, self.d_buf, self.dw)
+                p.dispatch_bwd(l, i0, i1, self.d_buf, self.dx)
             return
 
         def mark():
@@ -315,14 +325,14 @@ class Workload:
             ev[-1].record()
 
         mark()
-        p.dispatch(l, i, i + 1, self.x[i], self.perm, self.buf)
+        p.dispatch(l, i0, i1, self.x[g], self.perm, self.buf)
         mark()
-        p.combine(l, i, i + 1, self.buf, self.y)
+        p.combine(l, i0, i1, self.buf, self.y)
         mark()
         if self.stage == "update":
-            p.combine_bwd(l, i, i + 1, self.dy, self.buf, self.d_buf, self.dw)
+            p.combine_bwd(l, i0, i1, self.dy, self.buf, self.d_buf, self.dw)
             mark()
-            p.dispatch_bwd(l, i, i + 1, self.d_buf, self.dx)
+            p.dispatch_bwd(l, i0, i1, self.d_buf, self.dx)
             mark()
 
     def step(self, probes=None, stride: int = 0):
@@ -491,7 +501,8 @@ def run_ours(args, cfg) -> None:
     multi.init("nccl", dev)
     cfg.seed = multi.shard_seed(cfg.seed, rank)          # each rank: its own step (weak scaling)
     objective = tuple(int(v) for v in args.objective.split(",")) if args.objective else None
-    wl = Workload(cfg, dev, args.stage, args.machines, args.planner, objective, not args.strict_order)
+    wl = Workload(cfg, dev, args.stage, args.machines, args.planner, objective, not args.strict_order,
+                  args.mb_per_call)
     bpt = bytes_per_token(cfg)
     upd = args.stage == "update"
     total_bpt = bpt["total_update"] if upd else bpt["total"]
@@ -543,11 +554,12 @@ def run_ours(args, cfg) -> None:
                 traffic_src = "stored constant, NOT measured in this run: " + tj.get("_source", "profiles/traffic.json")
         except Exception:
             traffic = None
+    probed = kern.get(dom, {"gbs": None, "avg_ms": None})      # absent with --probe-stride 0 (diagnostic lines)
     roofline = {"bound": "hbm", "kernel": f"foremoe_{dom}",
-                "achieved": kern[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kern[dom]["gbs"] / peak, "traffic": traffic, "traffic_source": traffic_src,
+                "achieved": probed["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": probed["gbs"] / peak if probed["gbs"] else None, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": peak_src,
-                "bytes_per_launch": bpt[dom] * max(wl.tok), "avg_launch_ms": kern[dom]["avg_ms"],
+                "bytes_per_launch": bpt[dom] * max(wl.tok), "avg_launch_ms": probed["avg_ms"],
                 "whole_path_gbs": value / world * total_bpt / 1e9,
                 "whole_path_frac": value / world * total_bpt / 1e9 / peak,
                 "whole_path_frac_of_nominal_8TBs": value / world * total_bpt / 1e9 / NOMINAL_HBM_GBS,
@@ -594,6 +606,7 @@ def run_ours(args, cfg) -> None:
                    "l2": "inputs larger than L2: every instance moves >= 1 GB and consecutive "
                          "launches read different x buffers; no flush needed",
                    "plan_stable_flag": not args.strict_order,
+                   **({"mb_per_call": args.mb_per_call} if args.mb_per_call != 1 else {}),
                    "stage": args.stage, "machines": args.machines, "planner": args.planner,
                    **({"objective": args.objective} if args.objective else {}), "bytes_per_routed_token": total_bpt,
                    **({"sweep_tuning": args.tune} if args.tune else {}),
@@ -603,9 +616,10 @@ def run_ours(args, cfg) -> None:
         "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "balance": balance,
     }
     verify = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline and not upd and not args.machines and args.planner == "stage4":
+    if (rank == 0 and world == 1 and not args.no_cpu_baseline and not upd and not args.machines
+            and args.planner == "stage4" and args.mb_per_call == 1):
         verify = capture_instance(wl, wl.instances[len(wl.instances) // 2])
-    if not args.no_e2e and not upd and not args.machines and args.planner == "stage4":
+    if not args.no_e2e and not upd and not args.machines and args.planner == "stage4" and args.mb_per_call == 1:
         line["e2e"] = run_e2e(args, cfg, wl, dev)
     else:
         wl.release()
@@ -654,7 +668,7 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5)")
     ap.add_argument("--mb-samples", type=int, default=None, help="config 4: samples per micro-step")
     ap.add_argument("--layers", type=int, default=None, help="debug: fewer layers (INVALID as a bench value)")
-    ap.add_argument("--probe-stride", type=int, default=8,
+    ap.add_argument("--probe-stride", type=int, default=32,
                     help="CUDA-event brackets around every n-th instance's dispatch / combine launch")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-mb", type=int, default=0,
@@ -680,6 +694,9 @@ def main() -> None:
                          "over --machines M) on the GPU inside the timed step")
     ap.add_argument("--streams", type=int, default=1,
                     help="> 1: interleave the independent instances over that many CUDA streams")
+    ap.add_argument("--mb-per-call", type=int, default=1,
+                    help="diagnostic: one dispatch / combine call per this many consecutive micro-steps of a layer "
+                         "(ranged calls); per-launch time against size separates the fixed cost of a launch from its rate")
     ap.add_argument("--strict-order", action="store_true",
                     help="do not set FOREMOE_FLAG_PLAN_STABLE: the data-path kernels then read nothing, not even "
                          "the plan arrays, before the preceding kernel of the stream has completed")

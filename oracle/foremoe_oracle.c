@@ -31,6 +31,10 @@
  *   O7/O8 placement (Stage 1 LPT, Alg. 3 Stages 2-3): hand-worked vectors, closed forms, greedy
  *                invariants replayed in Python, structure.  O9/O10 backward: torch.autograd,
  *                adjoint identities, bf16 rounding cases (see the blocks further down).
+ *   O15 (Eq.(10) with the C* term as a threshold ladder) and O16 (Alg. 2 Stage 3, replica search)
+ *                restate READINGS of passages the paper leaves open: parity
+ *                unpinned against the paper for the reading itself; pinned are bounds (LP, brute
+ *                force), special cases, invariants and hand-worked vectors -- see their blocks.
  */
 #include <math.h>
 #include <stdint.h>

@@ -206,9 +206,9 @@ static int launch_one(const Dims &d, int warps, int D, const int32_t *inv_l, con
   if (prepare) return FOREMOE_OK;
   const int n_slices = (d.row_vec + 32 * U - 1) / (32 * U);
   int per_sm = g_tune.combine_cta_per_sm;
-  if (per_sm <= 0) {      // at least 4 items per warp, between the resident CTAs and 32 per SM (sweep: r02_sweeps.md)
+  if (per_sm <= 0) {      // at least 8 items per warp, between the resident CTAs and 32 per SM (sweep: r02_sweeps.md)
     const long long items = (long long)(d.T / d.n_mb + 1) * n_slices;
-    const long long want = items / (4LL * warps * num_sms());
+    const long long want = items / (8LL * warps * num_sms());
     per_sm = want < occ ? occ : want > 32 ? 32 : (int)want;
   }
   const cudaError_t e = launch_pdl(kern, num_sms() * per_sm, warps * 32, smem, st, inv_l, w_l, mb_off,
@@ -247,7 +247,7 @@ static int launch_k(int U, const Dims &d, int warps, int D, const int32_t *inv_l
 int launch_combine_bulk(const Dims &d, const int32_t *inv_l, const float *w_l,
                         const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
                         cudaStream_t st, bool prepare) {
-  // Small CTAs on an oversubscribed grid: 4 warps x 2 stages of K x 1 KB slices (K = 8: 65 KB of
+  // Small CTAs on an oversubscribed grid: up to 4 warps x 2 stages of K x 1 KB slices (K = 8: 65 KB of
   // shared memory per CTA, 3 CTAs = 24 stages = 192 KB in flight per SM), up to 32 CTAs per SM in
   // the grid.  SMs drain their share of a bandwidth-bound kernel at rates that differ by ~10 % (ncu:
   // sm__cycles_active min / max of the persistent cp.async ring, profiles/r02_combine.md); with more
@@ -262,7 +262,10 @@ int launch_combine_bulk(const Dims &d, const int32_t *inv_l, const float *w_l,
   if (D <= 0) D = 2;
   if (D > kMaxDepth) D = kMaxDepth;
   const size_t stage = (size_t)d.K * 512 * U + 8 + 128;
-  if (warps <= 0) warps = 4;
+  if (warps <= 0) {       // as many warps as let three CTAs share an SM's shared memory (K = 8: 4, K = 10: 3)
+    warps = (int)((size_t)kSmemOptIn / 3 / (stage * D));
+    warps = warps < 2 ? 2 : warps > 4 ? 4 : warps;
+  }
   if (warps > 16) warps = 16;
   while (warps > 1 && stage * D * warps > budget) warps--;
   while (D > 2 && stage * D * warps > budget) D--;

@@ -234,9 +234,9 @@ static int check_range(const Dims &d, int layer, int mb_begin, int mb_end) {
 // facts instead)
 int dispatch_rows(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, int mb_begin,
                   int mb_end, const void *x, int32_t *perm, void *buf, cudaStream_t st, bool prepare) {
-  // auto: the bulk-copy ring wins from 12 KB rows on (config 3's 14 KB rows: 326.7 vs 329.9 us per launch,
-  // profiles/r02_sweeps.md); below that the register-staged kernel is faster (configs 2 and 5)
-  if (g_tune.dispatch_impl == 1 || (g_tune.dispatch_impl < 0 && d.row_bytes >= 12 * 1024)) {
+  // auto: the bulk-copy ring wins from 8 KB rows on (config 5's 8 KB rows: 447 vs 457 us per launch, config 3's
+  // 14 KB rows: 324 vs 327 us; profiles/r02_sweeps.md); at 4 KB the register-staged kernel is faster (97 vs 101 us)
+  if (g_tune.dispatch_impl == 1 || (g_tune.dispatch_impl < 0 && d.row_bytes >= 8 * 1024)) {
     const int rc = launch_dispatch_tma(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
     if (rc != FOREMOE_ERR_INVALID_ARG) return rc;     // rows too large for the ring: fall through
   }

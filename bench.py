@@ -298,7 +298,10 @@ class Workload:
         n_lad = len(runner.DEFAULT_LADDER) if (objective and machines and planner not in ("full", "alg2")) else 0
         if planner == "alg2":
             n_lad = len(self.plan.ladder)
-        self.launches_per_step = (2 + 6 + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
+        # foremoe_plan (given placement: default and LocalStepPlan) launches 7 kernels; the planners that derive
+        # the placement from the histogram call foremoe_load_hist (2) + foremoe_assign (6)
+        fused = planner == "stage4" and not n_lad
+        self.launches_per_step = ((7 if fused else 8) + (3 if machines and planner != "full" else 0) + (2 if planner == "full" else 0)
                                   + n_lad * 5 + (1 if n_lad else 0) + (4 if planner == "alg2" else 0)
                                   + (4 if stage == "update" else 2) * len(self.instances))
         if stage == "update":          # forward + backward of every instance
@@ -490,7 +493,7 @@ def run_e2e(args, cfg, wl: "Workload", dev) -> dict:
     return {"value": units / (ms_max * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
             "d2h_bytes_per_step": int(d2h), "steps": steps, "ms_per_step": ms_max / steps,
             "api": "foremoe_step_host (pinned host buffers; x up once per micro-step, y of every "
-                   "instance down)", "gpu_launches": steps * (7 + 2 * n_inst)}
+                   "instance down)", "gpu_launches": steps * (6 + 2 * n_inst)}
 
 
 def run_ours(args, cfg) -> None:

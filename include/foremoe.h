@@ -153,6 +153,23 @@ int foremoe_assign(const foremoe_shape_t *shape, const int32_t *ids, const int32
                    void *stream);
 
 /*
+ * (a1-a4) foremoe_load_hist followed by foremoe_assign as ONE call that passes over the ids twice
+ * instead of three times: the first pass counts every ranking chunk (a run of consecutive tokens of
+ * one instance), the instance histogram w_{s,e} is the sum of its chunks'
+ * counts and is written to `hist` before the quotas are computed from it, the second pass ranks the
+ * pairs.  Every output is bit-identical to the two separate calls; arguments as there, except that
+ * hist [n_mb][L][E] (and step_hist [L][E] or NULL) are OUTPUTS and pair_slot / inv are required.
+ * Use it when the placement does not depend on this step's histogram (a given step-level
+ * placement); planners that derive the placement from hist / step_hist call the two entry points.
+ * Faults: as foremoe_load_hist and foremoe_assign together.
+ */
+int foremoe_plan(const foremoe_shape_t *shape, const int32_t *ids, const int32_t *mb_off,
+                 const int32_t *slot_expert, const int32_t *quota_in, int32_t *hist,
+                 int64_t *step_hist, int32_t *quota, int32_t *rank_load, int32_t *slot_off,
+                 int32_t *pair_slot, int32_t *inv, void *workspace, size_t workspace_bytes,
+                 int32_t *dev_status, void *stream);
+
+/*
  * (a4-a5) Dispatch of micro-steps [mb_begin, mb_end) of one layer: the permutation and the row
  * gather into contiguous per-rank / per-slot buffers.
  *   inv   [L][T][K] from foremoe_assign (the whole array; the call indexes layer / range itself).

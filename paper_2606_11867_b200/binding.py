@@ -38,6 +38,7 @@ ACT_FP32 = 1
 FLAG_PLAN_STABLE = 1
 
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_warmup", "foremoe_load_hist", "foremoe_assign",
+           "foremoe_plan",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
            "foremoe_local_placement_theta", "foremoe_tradeoff_select",
@@ -121,6 +122,7 @@ def lib() -> C.CDLL:
         l.foremoe_warmup.argtypes = [sp, vp]
         l.foremoe_load_hist.argtypes = [sp, vp, vp, vp, vp, vp, vp]
         l.foremoe_assign.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
+        l.foremoe_plan.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
         l.foremoe_dispatch.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_combine.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_combine_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -214,6 +216,17 @@ def assign(shape: Shape, ids, mb_off, hist, slot_expert, quota_in, quota, rank_l
         _dev(hist, torch.int32), _dev(slot_expert, torch.int32), _dev(quota_in, torch.int32),
         _dev(quota, torch.int32), _dev(rank_load, torch.int32), _dev(slot_off, torch.int32),
         _dev(pair_slot, torch.int32), _dev(inv, torch.int32), _dev(workspace),
+        workspace.numel() * workspace.element_size(), _dev(dev_status, torch.int32), _stream()))
+
+
+def plan(shape: Shape, ids, mb_off, slot_expert, quota_in, hist, step_hist, quota, rank_load, slot_off,
+         pair_slot, inv, workspace, dev_status=None) -> None:
+    """(a1-a4) load_hist + assign in two passes over the ids; hist / step_hist are outputs."""
+    _check("foremoe_plan", lib().foremoe_plan(
+        C.byref(shape.c()), _dev(ids, torch.int32), _dev(mb_off, torch.int32),
+        _dev(slot_expert, torch.int32), _dev(quota_in, torch.int32), _dev(hist, torch.int32),
+        _dev(step_hist, torch.int64), _dev(quota, torch.int32), _dev(rank_load, torch.int32),
+        _dev(slot_off, torch.int32), _dev(pair_slot, torch.int32), _dev(inv, torch.int32), _dev(workspace),
         workspace.numel() * workspace.element_size(), _dev(dev_status, torch.int32), _stream()))
 
 

@@ -12,8 +12,13 @@
 namespace foremoe {
 
 constexpr int kChunkPairs = 4096;    // pairs ranked by one CTA of k_assign_pairs / k_chunk_hist
-constexpr int kChunkThreads = 256;
+#ifndef FOREMOE_CHUNK_THREADS
+#define FOREMOE_CHUNK_THREADS 256
+#endif
+constexpr int kChunkThreads = FOREMOE_CHUNK_THREADS;
 constexpr int kChunkWarps = kChunkThreads / 32;
+constexpr int kRankShift = 20;       // k_assign_pairs packs (expert id, rank inside the warp's segment) into one int
+static_assert(kChunkPairs / kChunkWarps <= (1 << (31 - kRankShift)), "rank inside a warp's segment must fit");
 constexpr int kQuotaThreads = 128;
 constexpr int kMaxWaterPasses = 256;  // Phase B cap (O2)
 

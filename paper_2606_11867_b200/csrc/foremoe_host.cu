@@ -1,6 +1,6 @@
 // foremoe_step_host: the whole path driven from HOST buffers (the end-to-end leg of the bench and
 // the call a host-side user makes).  Orchestration only: every step runs in the kernels behind
-// foremoe_load_hist / foremoe_assign / foremoe_dispatch / foremoe_combine.  Host<->device copies
+// foremoe_plan (= foremoe_load_hist + foremoe_assign) / foremoe_dispatch / foremoe_combine.  Host<->device copies
 // run on two side streams so that the x upload of micro-step i+1 and the y download of instance
 // n-1 overlap the kernels of instance n.  Contract: include/foremoe.h.
 #include "foremoe_common.cuh"
@@ -117,9 +117,8 @@ extern "C" __attribute__((visibility("default"))) int foremoe_step_host(
   FM_CUDA(cudaMemcpyAsync(slot_expert, slot_expert_h, (size_t)d.n_pl * d.S * 4, cudaMemcpyHostToDevice, st));
   FM_CUDA(cudaMemcpyAsync(ids, ids_h, pairs * 4, cudaMemcpyHostToDevice, st));
   FM_CUDA(cudaMemcpyAsync(w, w_h, pairs * 4, cudaMemcpyHostToDevice, up));   // not needed before combine
-  FM_CALL(foremoe_load_hist(shape, ids, mb_off, hist, nullptr, status, st));
-  FM_CALL(foremoe_assign(shape, ids, mb_off, hist, slot_expert, nullptr, quota, rank_load, slot_off,
-                         pair_slot, inv, base + a.workspace, make_workspace(d).total, status, st));
+  FM_CALL(foremoe_plan(shape, ids, mb_off, slot_expert, nullptr, hist, nullptr, quota, rank_load, slot_off,
+                       pair_slot, inv, base + a.workspace, make_workspace(d).total, status, st));
   if (quota_h) FM_CUDA(cudaMemcpyAsync(quota_h, quota, (size_t)d.n_inst * d.S * 4, cudaMemcpyDeviceToHost, st));
   if (rank_load_h) FM_CUDA(cudaMemcpyAsync(rank_load_h, rank_load, (size_t)d.n_inst * d.P * 4, cudaMemcpyDeviceToHost, st));
   if (slot_off_h) FM_CUDA(cudaMemcpyAsync(slot_off_h, slot_off, (size_t)d.n_inst * (d.S + 1) * 4, cudaMemcpyDeviceToHost, st));

@@ -248,17 +248,26 @@ __device__ __forceinline__ bool locate_chunk(const int32_t *__restrict__ chunk_o
 __global__ void __launch_bounds__(kChunkThreads)
 k_chunk_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off,
              const int32_t *__restrict__ chunk_off, int L, int T, int K, int E, int n_mb, int tpc,
-             int max_chunks, int32_t *__restrict__ chunk_cnt) {
+             int max_chunks, int32_t *__restrict__ chunk_cnt, int32_t *__restrict__ hist_out,
+             int32_t *dev_status) {
   extern __shared__ int32_t sh[];   // [E]
   ChunkInfo ci;
   const int c = blockIdx.x, l = blockIdx.y;
   if (!locate_chunk(chunk_off, mb_off, n_mb, tpc, c, &ci)) return;
   for (int e = threadIdx.x; e < E; e += blockDim.x) sh[e] = 0;
   __syncthreads();
-  (void)count_ids(ids + ((size_t)l * T + ci.t0) * K, (ci.t1 - ci.t0) * K, sh, E);
+  // hist_out / dev_status are non-NULL only in foremoe_plan, where this pass also stands in for
+  // k_load_hist: a chunk lies inside one instance, so hist[i][l][:] is the sum of its chunks' counts
+  const int fault = count_ids(ids + ((size_t)l * T + ci.t0) * K, (ci.t1 - ci.t0) * K, sh, E);
+  if (fault) raise_fault(dev_status, fault);
   __syncthreads();
   int32_t *dst = chunk_cnt + ((size_t)l * max_chunks + c) * E;
-  for (int e = threadIdx.x; e < E; e += blockDim.x) dst[e] = sh[e];
+  int32_t *hdst = hist_out ? hist_out + ((size_t)ci.i * L + l) * E : nullptr;
+  for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    const int v = sh[e];
+    dst[e] = v;
+    if (hdst && v) atomicAdd(hdst + e, v);
+  }
 }
 
 // =============================================================================================
@@ -419,6 +428,26 @@ __device__ __forceinline__ void augment_units(const QuotaSmem &s, int P, int Ns)
   }
 }
 
+// Exclusive scan (in place) of expert e's counts over the chunks [c0, c1) of one instance; returns
+// the total = the instance's count of e.
+__device__ __forceinline__ int scan_chunk_counts(int32_t *cc, int c0, int c1, int E, int e) {
+  int run = 0;
+  int c = c0;
+  for (; c + 4 <= c1; c += 4) {
+    const int v0 = cc[(size_t)c * E + e], v1 = cc[(size_t)(c + 1) * E + e];
+    const int v2 = cc[(size_t)(c + 2) * E + e], v3 = cc[(size_t)(c + 3) * E + e];
+    cc[(size_t)c * E + e] = run; run += v0;
+    cc[(size_t)(c + 1) * E + e] = run; run += v1;
+    cc[(size_t)(c + 2) * E + e] = run; run += v2;
+    cc[(size_t)(c + 3) * E + e] = run; run += v3;
+  }
+  for (; c < c1; c++) {
+    const int v = cc[(size_t)c * E + e];
+    cc[(size_t)c * E + e] = run; run += v;
+  }
+  return run;
+}
+
 __global__ void __launch_bounds__(kQuotaThreads)
 k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
         const int32_t *__restrict__ mb_ok, const int32_t *__restrict__ chunk_off,
@@ -428,7 +457,9 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
         int P, int Ns, int pl_per_mb, int max_chunks, int32_t *__restrict__ quota,
         int32_t *__restrict__ rank_load, int32_t *__restrict__ slot_off,
         int32_t *__restrict__ inst_cum_end, int32_t *__restrict__ inst_slot_adj,
-        int32_t *__restrict__ inst_ok, int32_t *__restrict__ chunk_cnt, int32_t *dev_status) {
+        int32_t *__restrict__ inst_ok, int32_t *__restrict__ chunk_cnt, int scan_chunks,
+        int32_t *dev_status) {
+  // scan_chunks: chunk_cnt holds this step's per-chunk counts (the pairs will be assigned)
   extern __shared__ int32_t sm[];
   const int S = P * Ns;
   const int inst = blockIdx.x;
@@ -553,26 +584,11 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
       if (tid == 0) augment_units(s, P, Ns);
     }
   }
-  if (tid >= 32) {
-    // exclusive scan over the instance's chunks, per expert (in place)
+  if (tid >= 32 && scan_chunks) {
+    // exclusive scan over the instance's chunks, per expert (in place), beside warp 0's quota work
     const int c0 = chunk_off[i], c1 = chunk_off[i + 1];
     int32_t *cc = chunk_cnt + (size_t)l * max_chunks * E;
-    for (int e = tid - 32; e < E; e += nt - 32) {
-      int run = 0;
-      int c = c0;
-      for (; c + 4 <= c1; c += 4) {
-        const int v0 = cc[(size_t)c * E + e], v1 = cc[(size_t)(c + 1) * E + e];
-        const int v2 = cc[(size_t)(c + 2) * E + e], v3 = cc[(size_t)(c + 3) * E + e];
-        cc[(size_t)c * E + e] = run; run += v0;
-        cc[(size_t)(c + 1) * E + e] = run; run += v1;
-        cc[(size_t)(c + 2) * E + e] = run; run += v2;
-        cc[(size_t)(c + 3) * E + e] = run; run += v3;
-      }
-      for (; c < c1; c++) {
-        const int v = cc[(size_t)c * E + e];
-        cc[(size_t)c * E + e] = run; run += v;
-      }
-    }
+    for (int e = tid - 32; e < E; e += nt - 32) (void)scan_chunk_counts(cc, c0, c1, E, e);
   }
   __syncthreads();
 
@@ -606,8 +622,21 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
 // slot (a3) and the destination row (a4).  One CTA per chunk; each warp owns a contiguous segment
 // of the chunk, so the order (chunk, warp, iteration, lane) is the (t, k) order.
 // grid (max_chunks, L).
+//
+// Pass 1 (per warp, over its own segment): the rank of every pair among the WARP's pairs of its
+// expert, from a warp-private running counter wc[e] and match.any (lanes of one 32-pair group that
+// hold the same expert read the same counter, add their position inside the group, and the last of
+// them advances it) -- no shared atomics; (expert, rank in warp) stay packed in one register.
+// Scan: wc[w][e] -> pairs of e before warp w's segment in the instance (chunk base + earlier warps).
+// Pass 2: n = base + rank in warp; etab[e] holds the first host slot of e, where its quota interval
+// ends and its row offset: one 16-byte shared load decides every singly hosted expert and the first
+// replica.  Pairs beyond the first replica's quota walk htab (one 16-byte entry per further host) in
+// a loop whose trip count is uniform over the warp, so the kernel has no divergent branch.
 // =============================================================================================
-__global__ void __launch_bounds__(kChunkThreads)
+#ifndef FOREMOE_ASSIGN_MINB
+#define FOREMOE_ASSIGN_MINB 4
+#endif
+__global__ void __launch_bounds__(kChunkThreads, FOREMOE_ASSIGN_MINB)
 k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off,
                const int32_t *__restrict__ chunk_off, const int32_t *__restrict__ pl_host_ptr,
                const int32_t *__restrict__ pl_host_slot, const int32_t *__restrict__ inst_cum_end,
@@ -615,12 +644,10 @@ k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_o
                const int32_t *__restrict__ chunk_cnt, int L, int T, int K, int E, int S, int n_mb,
                int tpc, int max_chunks, int pl_per_mb, int32_t *__restrict__ pair_slot,
                int32_t *__restrict__ inv, int32_t *dev_status) {
-  extern __shared__ int32_t sm[];
-  int32_t *hptr = sm;                 // [E+1]
-  int32_t *hslot = hptr + E + 1;      // [S]
-  int32_t *cum_end = hslot + S;       // [S]
-  int32_t *slot_adj = cum_end + S;    // [S]
-  int32_t *wcnt = slot_adj + S;       // [kChunkWarps][E]
+  extern __shared__ __align__(16) int32_t sm_pairs[];
+  int4 *etab = (int4 *)sm_pairs;            // [E] {first host slot, its cum_end, its slot_adj, index of the 2nd host or -1}
+  int4 *htab = etab + E;                    // [S] per host entry {cum_end, slot, slot_adj, last host of its expert}
+  int32_t *wcnt = (int32_t *)(htab + S);    // [kChunkWarps][E]
   ChunkInfo ci;
   const int c = blockIdx.x, l = blockIdx.y;
   if (!locate_chunk(chunk_off, mb_off, n_mb, tpc, c, &ci)) return;
@@ -634,28 +661,47 @@ k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_o
     for (int p = tid; p < np; p += blockDim.x) { o_slot[p] = -1; o_inv[p] = -1; }
     return;
   }
-  for (int e = tid; e <= E; e += blockDim.x) hptr[e] = pl_host_ptr[(size_t)pl * (E + 1) + e];
-  for (int j = tid; j < S; j += blockDim.x) {
-    hslot[j] = pl_host_slot[(size_t)pl * S + j];
-    cum_end[j] = inst_cum_end[(size_t)inst * S + j];
-    slot_adj[j] = inst_slot_adj[(size_t)inst * S + j];
+  constexpr int kIter = kChunkPairs / kChunkThreads;   // 32-pair groups per warp
+  const int32_t *src = ids + pbase + warp * (kIter * 32) + lane;
+  const int rem = np - warp * (kIter * 32) - lane;     // pair `it` of this lane exists iff it * 32 < rem
+  int my[kIter];
+#pragma unroll
+  for (int it = 0; it < kIter; it++) my[it] = it * 32 < rem ? __ldg(src + it * 32) : -1;
+  {
+    const int32_t *hp = pl_host_ptr + (size_t)pl * (E + 1), *hs = pl_host_slot + (size_t)pl * S;
+    const int32_t *ce = inst_cum_end + (size_t)inst * S, *sa = inst_slot_adj + (size_t)inst * S;
+    for (int e = tid; e < E; e += blockDim.x) {
+      const int a0 = hp[e], a1 = hp[e + 1];
+      int4 t = make_int4(-1, 0, 0, -1);
+      for (int a = a0; a < a1; a++) {
+        const int j = hs[a];
+        const int4 h = make_int4(ce[j], j, sa[j], a == a1 - 1);
+        htab[a] = h;
+        if (a == a0) t = make_int4(j, h.x, h.z, a1 - a0 > 1 ? a0 + 1 : -1);
+      }
+      etab[e] = t;
+    }
   }
   for (int x = tid; x < kChunkWarps * E; x += blockDim.x) wcnt[x] = 0;
   __syncthreads();
 
-  constexpr int kIter = kChunkPairs / kChunkThreads;   // 32-pair groups per warp
-  const int32_t *src = ids + pbase;
-  const int seg0 = warp * (kIter * 32);
-  int my[kIter];
+  // pass 1: rank inside the warp's segment
+  const unsigned full = 0xffffffffu;
+  const unsigned lt = (1u << lane) - 1u;
+  int32_t *wc = wcnt + warp * E;
+  int fault = 0;
 #pragma unroll
   for (int it = 0; it < kIter; it++) {
-    const int p = seg0 + it * 32 + lane;
-    my[it] = p < np ? __ldg(src + p) : -1;
+    const int e = my[it];
+    const bool ok = (unsigned)e < (unsigned)E;
+    const unsigned grp = __match_any_sync(full, ok ? (unsigned)e : (0x80000000u | lane));
+    const int pre = wc[ok ? e : 0];
+    __syncwarp();
+    if (ok && lane == 31 - __clz(grp)) wc[e] = pre + __popc(grp);   // last lane of the group advances the counter
+    __syncwarp();
+    if (!ok && it * 32 < rem) fault = FOREMOE_FAULT_ID_RANGE;
+    my[it] = ok ? (e | ((pre + __popc(grp & lt)) << kRankShift)) : -1;
   }
-  int32_t *wc = wcnt + warp * E;
-#pragma unroll
-  for (int it = 0; it < kIter; it++)
-    if ((unsigned)my[it] < (unsigned)E) atomicAdd(&wc[my[it]], 1);
   __syncthreads();
   // exclusive scan over warps, seeded with the chunk's base (pairs of e in earlier chunks)
   const int32_t *cbase = chunk_cnt + ((size_t)l * max_chunks + c) * E;
@@ -670,34 +716,33 @@ k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_o
   }
   __syncthreads();
 
+  // pass 2: slot and destination row
   const int row_base = __ldg(mb_off + ci.i) * K;
-  const unsigned lt = (1u << lane) - 1u;
-  int fault = 0;
+  o_slot += warp * (kIter * 32) + lane;
+  o_inv += warp * (kIter * 32) + lane;
 #pragma unroll
   for (int it = 0; it < kIter; it++) {
-    const int p = seg0 + it * 32 + lane;
-    const int e = my[it];
-    const bool ok = (unsigned)e < (unsigned)E;
-    const unsigned key = ok ? (unsigned)e : (0x80000000u | lane);
-    const unsigned grp = __match_any_sync(0xffffffffu, key);
-    int n = 0;
-    if (ok) n = wc[e] + __popc(grp & lt);
-    __syncwarp();
-    if (ok && lane == 31 - __clz(grp)) wc[e] = n + 1;   // last lane of the group advances the counter
-    __syncwarp();
-    if (p < np) {
-      int slot = -1, dst = -1;
-      if (ok) {
-        for (int a = hptr[e]; a < hptr[e + 1]; a++) {
-          const int j = hslot[a];
-          if (n < cum_end[j]) { slot = j; dst = row_base + slot_adj[j] + n; break; }
-        }
-        if (slot < 0) fault |= FOREMOE_FAULT_NO_HOST;
-      } else {
-        fault |= FOREMOE_FAULT_ID_RANGE;
-      }
-      o_slot[p] = slot;
-      o_inv[p] = dst;
+    const int v = my[it];
+    const bool ok = v >= 0;
+    const int e = ok ? (v & ((1 << kRankShift) - 1)) : 0;
+    const int n = wc[e] + (v >> kRankShift);
+    const int4 t = etab[e];
+    const bool hit = ok && n < t.y;
+    int slot = hit ? t.x : -1;
+    int adj = t.z;
+    int a = t.w;
+    bool pend = ok && !hit && a >= 0;
+    while (__any_sync(full, pend)) {            // uniform trip count: the longest host walk of the warp
+      const int4 h = htab[pend ? a : 0];
+      const bool found = pend && n < h.x;
+      if (found) { slot = h.y; adj = h.z; }
+      pend = pend && !found && !h.w;
+      a++;
+    }
+    if (ok && slot < 0) fault |= FOREMOE_FAULT_NO_HOST;
+    if (it * 32 < rem) {
+      o_slot[it * 32] = slot;
+      o_inv[it * 32] = slot >= 0 ? row_base + adj + n : -1;
     }
   }
   if (fault) raise_fault(dev_status, fault);
@@ -774,23 +819,17 @@ extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const fo
   return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
-extern "C" __attribute__((visibility("default"))) int foremoe_assign(const foremoe_shape_t *shape, const int32_t *ids,
-                              const int32_t *mb_off, const int32_t *hist,
-                              const int32_t *slot_expert, const int32_t *quota_in, int32_t *quota,
-                              int32_t *rank_load, int32_t *slot_off, int32_t *pair_slot,
-                              int32_t *inv, void *workspace, size_t workspace_bytes,
-                              int32_t *dev_status, void *stream) {
-  Dims d;
-  int rc = make_dims(shape, &d);
-  if (rc) return rc;
-  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
-    return FOREMOE_ERR_INVALID_ARG;
-  if ((pair_slot == nullptr) != (inv == nullptr)) return FOREMOE_ERR_INVALID_ARG;
+// Shared launcher of foremoe_assign (hist given, hist_out = NULL) and foremoe_plan (hist_out given:
+// k_chunk_hist also accumulates the instance histograms and reports the id faults).
+static int launch_assign(const Dims &d, const int32_t *ids, const int32_t *mb_off, const int32_t *hist,
+                         int32_t *hist_out, int64_t *step_hist, const int32_t *slot_expert,
+                         const int32_t *quota_in, int32_t *quota, int32_t *rank_load, int32_t *slot_off,
+                         int32_t *pair_slot, int32_t *inv, void *workspace, size_t workspace_bytes,
+                         int32_t *dev_status, cudaStream_t st) {
   const bool want_pairs = pair_slot != nullptr;      // both NULL: quotas only (a2), no pass over the ids
   if (!aligned(workspace, 16)) return FOREMOE_ERR_INVALID_ARG;
   const Workspace w = make_workspace(d);
   if (workspace_bytes < w.total) return FOREMOE_ERR_WORKSPACE;
-  cudaStream_t st = (cudaStream_t)stream;
   char *ws = (char *)workspace;
   int32_t *chunk_off = (int32_t *)(ws + w.chunk_off), *mb_ok = (int32_t *)(ws + w.mb_ok);
   int32_t *pl_host_ptr = (int32_t *)(ws + w.pl_host_ptr);
@@ -802,7 +841,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
   int32_t *inst_ok = (int32_t *)(ws + w.inst_ok), *chunk_cnt = (int32_t *)(ws + w.chunk_cnt);
 
   const size_t smem_quota = sizeof(int32_t) * ((size_t)5 * d.E + 1 + (size_t)8 * d.S + 1 + (size_t)7 * d.P);
-  const size_t smem_pairs = sizeof(int32_t) * ((size_t)d.E + 1 + (size_t)3 * d.S + (size_t)kChunkWarps * d.E);
+  const size_t smem_pairs = sizeof(int32_t) * ((size_t)4 * d.E + (size_t)4 * d.S + (size_t)kChunkWarps * d.E);
   const size_t smem_pl = sizeof(int32_t) * ((size_t)2 * d.S + d.E + 1);
   if (smem_quota > 200 * 1024 || smem_pairs > 200 * 1024 || smem_pl > 200 * 1024)
     return FOREMOE_ERR_INVALID_ARG;
@@ -816,23 +855,72 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
       cudaFuncSetAttribute(k_placement_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_pl) != cudaSuccess)
     return FOREMOE_ERR_CUDA;
 
+  if (hist_out &&
+      cudaMemsetAsync(hist_out, 0, sizeof(int32_t) * (size_t)d.n_inst * d.E, st) != cudaSuccess)
+    return FOREMOE_ERR_CUDA;        // stays all zero on an MB_OFF fault, like foremoe_load_hist
   k_mb_tables<<<1, 256, 0, st>>>(mb_off, d.n_mb, d.T, d.tpc, chunk_off, mb_ok, dev_status);
   k_placement_tables<<<d.n_pl, 256, smem_pl, st>>>(slot_expert, d.E, d.S, d.Ns, d.P, pl_host_ptr,
                                                    pl_host_slot, pl_active, pl_rslot, pl_fault,
                                                    dev_status);
   const dim3 cgrid(d.max_chunks, d.L);
-  if (d.T > 0 && want_pairs)
+  const bool chunks = d.T > 0 && want_pairs;
+  if (chunks)
     k_chunk_hist<<<cgrid, kChunkThreads, sizeof(int32_t) * d.E, st>>>(
-        ids, mb_off, chunk_off, d.L, d.T, d.K, d.E, d.n_mb, d.tpc, d.max_chunks, chunk_cnt);
+        ids, mb_off, chunk_off, d.L, d.T, d.K, d.E, d.n_mb, d.tpc, d.max_chunks, chunk_cnt, hist_out,
+        hist_out ? dev_status : nullptr);
+  if (hist_out) hist = hist_out;
   k_quota<<<d.n_inst, kQuotaThreads, smem_quota, st>>>(
       hist, quota_in, mb_ok, chunk_off, pl_host_ptr, pl_host_slot, pl_active, pl_rslot, pl_fault,
       slot_expert, d.L, d.E, d.P, d.Ns, d.pl_per_mb, d.max_chunks, quota, rank_load, slot_off,
-      inst_cum_end, inst_slot_adj, inst_ok, chunk_cnt, dev_status);
-  if (d.T > 0 && want_pairs)
+      inst_cum_end, inst_slot_adj, inst_ok, chunk_cnt, chunks ? 1 : 0, dev_status);
+  if (hist_out && step_hist) {
+    const int LE = d.L * d.E;
+    k_step_hist<<<(LE + 255) / 256, 256, 0, st>>>(hist_out, d.n_mb, LE, step_hist);
+  }
+  if (chunks)
     k_assign_pairs<<<cgrid, kChunkThreads, smem_pairs, st>>>(
         ids, mb_off, chunk_off, pl_host_ptr, pl_host_slot, inst_cum_end, inst_slot_adj, inst_ok,
         chunk_cnt, d.L, d.T, d.K, d.E, d.S, d.n_mb, d.tpc, d.max_chunks, d.pl_per_mb, pair_slot,
         inv, dev_status);
   k_plan_fence<<<1, 32, 0, st>>>();
   return cudaGetLastError() == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_assign(const foremoe_shape_t *shape, const int32_t *ids,
+                              const int32_t *mb_off, const int32_t *hist,
+                              const int32_t *slot_expert, const int32_t *quota_in, int32_t *quota,
+                              int32_t *rank_load, int32_t *slot_off, int32_t *pair_slot,
+                              int32_t *inv, void *workspace, size_t workspace_bytes,
+                              int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
+    return FOREMOE_ERR_INVALID_ARG;
+  if ((pair_slot == nullptr) != (inv == nullptr)) return FOREMOE_ERR_INVALID_ARG;
+  return launch_assign(d, ids, mb_off, hist, nullptr, nullptr, slot_expert, quota_in, quota, rank_load,
+                       slot_off, pair_slot, inv, workspace, workspace_bytes, dev_status, (cudaStream_t)stream);
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_plan(const foremoe_shape_t *shape, const int32_t *ids,
+                            const int32_t *mb_off, const int32_t *slot_expert, const int32_t *quota_in,
+                            int32_t *hist, int64_t *step_hist, int32_t *quota, int32_t *rank_load,
+                            int32_t *slot_off, int32_t *pair_slot, int32_t *inv, void *workspace,
+                            size_t workspace_bytes, int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !pair_slot || !inv ||
+      !workspace)
+    return FOREMOE_ERR_INVALID_ARG;
+  if (d.T == 0) {                                   // no chunks to take the histogram from: all zero
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemsetAsync(hist, 0, sizeof(int32_t) * (size_t)d.n_inst * d.E, st) != cudaSuccess ||
+        (step_hist && cudaMemsetAsync(step_hist, 0, sizeof(int64_t) * (size_t)d.L * d.E, st) != cudaSuccess))
+      return FOREMOE_ERR_CUDA;
+    return launch_assign(d, ids, mb_off, hist, nullptr, nullptr, slot_expert, quota_in, quota, rank_load,
+                         slot_off, pair_slot, inv, workspace, workspace_bytes, dev_status, st);
+  }
+  return launch_assign(d, ids, mb_off, nullptr, hist, step_hist, slot_expert, quota_in, quota, rank_load,
+                       slot_off, pair_slot, inv, workspace, workspace_bytes, dev_status, (cudaStream_t)stream);
 }

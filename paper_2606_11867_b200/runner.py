@@ -52,8 +52,11 @@ class StepPlan:
                   self.workspace, self.status)
 
     def plan(self, quota_in: Optional[torch.Tensor] = None) -> None:
-        self.load_hist()
-        self.assign(quota_in)
+        """a1-a4 for a given placement: foremoe_plan (two passes over the ids, same results as
+        load_hist() + assign())."""
+        fm.plan(self.shape, self.ids, self.mb_off, self.slot_expert, quota_in, self.hist, self.step_hist,
+                self.quota, self.rank_load, self.slot_off, self.pair_slot, self.inv, self.workspace,
+                self.status)
 
     def dispatch(self, layer: int, mb_begin: int, mb_end: int, x, perm, buf) -> None:
         self.data_path().dispatch(layer, mb_begin, mb_end, x, perm, buf)

@@ -35,8 +35,22 @@ def gpu_plan(shape: fm.Shape, ids, w, mb_off, se, quota_in=None) -> runner.StepP
     # poison the outputs so that unwritten elements are caught
     for name in ("hist", "quota", "rank_load", "slot_off", "pair_slot", "inv"):
         getattr(sp, name).fill_(-77)
-    sp.plan(None if quota_in is None else t(quota_in, torch.int32))
+    q = None if quota_in is None else t(quota_in, torch.int32)
+    sp.plan(q)                                   # foremoe_plan: two passes over the ids
     torch.cuda.synchronize()
+    # foremoe_load_hist + foremoe_assign (three passes) must give the same bits in every output
+    names = ("hist", "step_hist", "quota", "rank_load", "slot_off", "pair_slot", "inv")
+    fused = {n: getattr(sp, n).clone() for n in names}
+    f_fused = sp.faults()
+    for n in names:
+        getattr(sp, n).fill_(-77)
+    sp.status.zero_()
+    sp.load_hist()
+    sp.assign(q)
+    torch.cuda.synchronize()
+    assert sp.faults() == f_fused
+    for n in names:                              # (deterministic on faulted inputs as well)
+        assert torch.equal(fused[n], getattr(sp, n)), ("foremoe_plan vs load_hist + assign", n)
     return sp
 
 

@@ -76,6 +76,7 @@ def test_null_pointers_rejected_before_any_cuda_call(libpath):
     cs = s.c()
     assert lib.foremoe_load_hist(C.byref(cs), None, None, None, None, None, None) == fm.ERR_INVALID_ARG
     assert lib.foremoe_assign(C.byref(cs), *([None] * 11), 0, None, None) == fm.ERR_INVALID_ARG
+    assert lib.foremoe_plan(C.byref(cs), *([None] * 12), 0, None, None) == fm.ERR_INVALID_ARG
     assert lib.foremoe_dispatch(C.byref(cs), 0, 0, 1, None, None, None, None, None, None, None) == fm.ERR_INVALID_ARG
     assert lib.foremoe_combine(C.byref(cs), 0, 0, 1, None, None, None, None, None, None, None) == fm.ERR_INVALID_ARG
     assert lib.foremoe_step_host(C.byref(cs), *([None] * 10), 0, None, None) == fm.ERR_INVALID_ARG

@@ -187,32 +187,54 @@ k_placement_tables(const int32_t *__restrict__ slot_expert, int E, int S, int Ns
     se[j] = e;
   }
   bad = __syncthreads_or(bad);
-  for (int e = threadIdx.x; e < E; e += blockDim.x) {
-    int n = 0;
-    for (int j = 0; j < S; j++) n += (se[j] == e);
-    cnt[e] = n;
-  }
+  for (int e = threadIdx.x; e <= E; e += blockDim.x) cnt[e] = 0;
+  __syncthreads();
   for (int j = threadIdx.x; j < S; j += blockDim.x) {
     const int e = se[j];
+    if (e >= 0) atomicAdd(&cnt[e], 1);
     int a = e >= 0;
     for (int j2 = (j / Ns) * Ns; j2 < j; j2++) a &= (se[j2] != e);
     act[j] = a;
     active[j] = a;
   }
   __syncthreads();
-  if (threadIdx.x == 0) {
-    int run = 0;
-    for (int e = 0; e < E; e++) { int n = cnt[e]; cnt[e] = run; run += n; }
-    cnt[E] = run;
-    pl_fault[pl] = bad;
-    if (bad) raise_fault(dev_status, FOREMOE_FAULT_SLOT_EXPERT);
+  {   // exclusive prefix of cnt[0..E): every thread scans a contiguous run, thread 0 the run totals
+    __shared__ int part[256];
+    const int per = (E + blockDim.x - 1) / blockDim.x;
+    const int e0 = min(E, (int)threadIdx.x * per), e1 = min(E, e0 + per);
+    int sum = 0;
+    for (int e = e0; e < e1; e++) sum += cnt[e];
+    part[threadIdx.x] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int run = 0;
+      for (int t = 0; t < (int)blockDim.x; t++) { const int n = part[t]; part[t] = run; run += n; }
+      cnt[E] = run;
+      pl_fault[pl] = bad;
+      if (bad) raise_fault(dev_status, FOREMOE_FAULT_SLOT_EXPERT);
+    }
+    __syncthreads();
+    int run = part[threadIdx.x];
+    for (int e = e0; e < e1; e++) { const int n = cnt[e]; cnt[e] = run; run += n; }
   }
   __syncthreads();
   for (int e = threadIdx.x; e <= E; e += blockDim.x) host_ptr[e] = cnt[e];
+  __syncthreads();
+  // host list of every expert in ascending slot index: slots claim a position of their expert's
+  // segment in any order, then every (short) segment is sorted
+  for (int j = threadIdx.x; j < S; j += blockDim.x) {
+    const int e = se[j];
+    if (e >= 0) host_slot[atomicAdd(&cnt[e], 1)] = j;
+  }
+  __syncthreads();
   for (int e = threadIdx.x; e < E; e += blockDim.x) {
-    int pos = cnt[e];
-    for (int j = 0; j < S; j++)
-      if (se[j] == e) host_slot[pos++] = j;
+    const int a0 = host_ptr[e], a1 = cnt[e];               // cnt[e] has advanced to the segment's end
+    for (int a = a0 + 1; a < a1; a++) {
+      const int v = host_slot[a];
+      int b = a - 1;
+      for (; b >= a0 && host_slot[b] > v; b--) host_slot[b + 1] = host_slot[b];
+      host_slot[b + 1] = v;
+    }
   }
   // active slots of each rank by ascending expert id (they hold distinct experts)
   for (int j = threadIdx.x; j < S; j += blockDim.x) {
@@ -279,23 +301,29 @@ k_chunk_hist(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_off
 //   warps 1+ : exclusive scan of the instance's chunk counts over chunks (per expert).
 // then quota / rank_load / slot_off and the pair-lookup tables are written by all threads.
 // =============================================================================================
-struct QuotaSmem {
-  int32_t *c, *q, *load, *se, *act, *hptr, *hslot, *ahs, *rk, *rslot, *R, *nact, *visited, *par_rank,
-      *par_from, *par_to, *queue, *soff;
+// Index-valued tables (slots, experts, ranks, small counts) are held as I = int32_t, or int16_t when
+// E and S stay below 2^15 and the 32-bit layout would let shared memory cap the resident CTAs: the
+// commodity instances of the per-source plan (E * M, S * M) are large, one warp per instance does the
+// sequential work, and the kernel's rate is the number of instances resident per SM.
+template <typename I>
+struct QuotaSmemT {
+  int32_t *c, *q, *load, *visited, *par_rank, *par_from, *par_to, *queue, *soff;
+  I *se, *hptr, *ahs, *rk, *rslot, *R, *nact;
   // Phase B bookkeeping: stamp[r] = event number of the last change of load[r]; seen[e] = event
   // number at e's last fill.  A fill is a pure function of its hosts' loads (own quota removed) and
   // c[e], so when no host rank was touched since e's last fill it would reproduce the same quotas:
   // it is skipped.  The result is unchanged bit for bit; late passes cost almost nothing.
   int32_t *stamp, *seen;
 };
-// hptr/hslot: all slots of expert e (ascending); ahs[hptr[e] .. hptr[e] + nact[e]): its ACTIVE host
+// hptr: CSR offsets of the slots of expert e; ahs[hptr[e] .. hptr[e] + nact[e]): its ACTIVE host
 // slots (ascending); rk[j] = rank of slot j.
 
 // One replicated expert: closed form of the unit-by-unit fill.  With host loads l_j (the expert's
 // own quota removed), lam = largest integer with sum_j max(0, lam - l_j) <= c; every host gets
 // max(0, lam - l_j); the remaining units go one each to the first hosts (ascending slot index)
 // among {l_j <= lam}.  Serial version (one lane), used when an expert has more than 32 hosts.
-__device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e) {
+template <typename I>
+__device__ __forceinline__ int water_fill_expert(const QuotaSmemT<I> &s, int e) {
   const int a0 = s.hptr[e], a1 = a0 + s.nact[e];
   int cur = INT_MAX;
   for (int a = a0; a < a1; a++) {
@@ -340,7 +368,8 @@ __device__ __forceinline__ int water_fill_expert(const QuotaSmem &s, int e) {
 // f_a = sum_b max(0, l_a - l_b) is what it costs to raise every lower host to l_a; the water level
 // sits on top of the highest host load l* with f(l*) <= c:  lam = l* + (c - f(l*)) / m,
 // m = #{l_b <= l*}, and (c - f(l*)) % m units are left for the lowest slots among those m hosts.
-__device__ __forceinline__ int water_fill_expert_warp(const QuotaSmem &s, int e, int lane, int &event) {
+template <typename I>
+__device__ __forceinline__ int water_fill_expert_warp(const QuotaSmemT<I> &s, int e, int lane, int &event) {
   const unsigned full = 0xffffffffu;
   const int a0 = s.hptr[e], h = s.nact[e];
   if (h > 32) {
@@ -393,7 +422,8 @@ __device__ __forceinline__ int water_fill_expert_warp(const QuotaSmem &s, int e,
 // Phase C: while the lowest max-load rank h reaches (breadth first, ranks expanded through
 // replicated experts in ascending expert id, hosts in ascending slot index) a rank with
 // load <= max - 2, move one unit along the path.  Run by one lane.
-__device__ __forceinline__ void augment_units(const QuotaSmem &s, int P, int Ns) {
+template <typename I>
+__device__ __forceinline__ void augment_units(const QuotaSmemT<I> &s, int P, int Ns) {
   for (;;) {
     int mx = INT_MIN, h = 0;
     for (int r = 0; r < P; r++)
@@ -448,6 +478,7 @@ __device__ __forceinline__ int scan_chunk_counts(int32_t *cc, int c0, int c1, in
   return run;
 }
 
+template <typename I>
 __global__ void __launch_bounds__(kQuotaThreads)
 k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
         const int32_t *__restrict__ mb_ok, const int32_t *__restrict__ chunk_off,
@@ -468,19 +499,11 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   const int tid = threadIdx.x, nt = blockDim.x;
   if (!*mb_ok) return;
 
-  QuotaSmem s;
+  QuotaSmemT<I> s;
   int32_t *p = sm;
   s.c = p; p += E;
-  s.nact = p; p += E;
-  s.R = p; p += E;
-  s.hptr = p; p += E + 1;
+  s.seen = p; p += E;
   s.q = p; p += S;
-  s.se = p; p += S;
-  s.act = p; p += S;
-  s.hslot = p; p += S;
-  s.ahs = p; p += S;
-  s.rk = p; p += S;
-  s.rslot = p; p += S;
   s.soff = p; p += S + 1;
   s.load = p; p += P;
   s.visited = p; p += P;
@@ -489,7 +512,15 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   s.par_to = p; p += P;
   s.queue = p; p += P;
   s.stamp = p; p += P;
-  s.seen = p; p += E;
+  I *pi = (I *)p;
+  s.nact = pi; pi += E;
+  s.R = pi; pi += E;
+  s.hptr = pi; pi += E + 1;
+  s.se = pi; pi += S;
+  s.ahs = pi; pi += S;
+  s.rk = pi; pi += S;
+  s.rslot = pi; pi += S;
+  const int32_t *g_hslot = pl_host_slot + (size_t)pl * S;     // used outside the sequential part only
   __shared__ int nR_raw;
 
   for (int e = tid; e < E; e += nt) s.c[e] = hist[(size_t)inst * E + e];
@@ -497,8 +528,6 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   for (int j = tid; j < S; j += nt) {
     int e = slot_expert[(size_t)pl * S + j];
     s.se[j] = (e < -1 || e >= E) ? -1 : e;
-    s.act[j] = pl_active[(size_t)pl * S + j];
-    s.hslot[j] = pl_host_slot[(size_t)pl * S + j];
     s.rslot[j] = pl_rslot[(size_t)pl * S + j];
     s.rk[j] = j / Ns;
     s.q[j] = 0;
@@ -512,8 +541,8 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   for (int e = tid; e < E; e += nt) {
     int n = 0;
     for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
-      const int j = s.hslot[a];
-      if (s.act[j]) s.ahs[s.hptr[e] + n++] = j;
+      const int j = g_hslot[a];
+      if (pl_active[(size_t)pl * S + j]) s.ahs[s.hptr[e] + n++] = j;
     }
     s.nact[e] = n;
     if (s.c[e] < 0) fault |= FOREMOE_FAULT_ID_RANGE;
@@ -528,7 +557,7 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
     }
     for (int e = tid; e < E; e += nt) {
       int64_t sum = 0;
-      for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) sum += qi[s.hslot[a]];
+      for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) sum += qi[g_hslot[a]];
       if (sum != s.c[e]) fault |= FOREMOE_FAULT_QUOTA_IN;
     }
   }
@@ -609,7 +638,7 @@ k_quota(const int32_t *__restrict__ hist, const int32_t *__restrict__ quota_in,
   for (int e = tid; e < E; e += nt) {
     int cum = 0;
     for (int a = s.hptr[e]; a < s.hptr[e + 1]; a++) {
-      const int j = s.hslot[a];
+      const int j = g_hslot[a];
       inst_slot_adj[(size_t)inst * S + j] = s.soff[j] - cum;
       cum += s.q[j];
       inst_cum_end[(size_t)inst * S + j] = cum;
@@ -840,13 +869,19 @@ static int launch_assign(const Dims &d, const int32_t *ids, const int32_t *mb_of
   int32_t *inst_slot_adj = (int32_t *)(ws + w.inst_slot_adj);
   int32_t *inst_ok = (int32_t *)(ws + w.inst_ok), *chunk_cnt = (int32_t *)(ws + w.chunk_cnt);
 
-  const size_t smem_quota = sizeof(int32_t) * ((size_t)5 * d.E + 1 + (size_t)8 * d.S + 1 + (size_t)7 * d.P);
+  // k_quota: int32 arrays c, seen [E], q [S], soff [S+1], 7 x [P]; index arrays nact, R [E], hptr [E+1],
+  // se, ahs, rk, rslot [S] as int32 -- or as int16 when that lifts a shared-memory cap on the CTAs per SM
+  const size_t q_i32 = (size_t)2 * d.E + (size_t)2 * d.S + 1 + (size_t)7 * d.P;
+  const size_t q_idx = (size_t)3 * d.E + 1 + (size_t)4 * d.S;
+  const bool quota16 = d.E < 32768 && d.S < 32768 && 4 * (q_i32 + q_idx) * (2048 / kQuotaThreads) > (size_t)kSmemOptIn;
+  const size_t smem_quota = 4 * q_i32 + (quota16 ? 2 : 4) * q_idx + 4;
   const size_t smem_pairs = sizeof(int32_t) * ((size_t)4 * d.E + (size_t)4 * d.S + (size_t)kChunkWarps * d.E);
   const size_t smem_pl = sizeof(int32_t) * ((size_t)2 * d.S + d.E + 1);
   if (smem_quota > 200 * 1024 || smem_pairs > 200 * 1024 || smem_pl > 200 * 1024)
     return FOREMOE_ERR_INVALID_ARG;
   if (smem_quota > 48 * 1024 &&
-      cudaFuncSetAttribute(k_quota, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_quota) != cudaSuccess)
+      cudaFuncSetAttribute(quota16 ? k_quota<int16_t> : k_quota<int32_t>,
+                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_quota) != cudaSuccess)
     return FOREMOE_ERR_CUDA;
   if (smem_pairs > 48 * 1024 &&
       cudaFuncSetAttribute(k_assign_pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_pairs) != cudaSuccess)
@@ -869,7 +904,7 @@ static int launch_assign(const Dims &d, const int32_t *ids, const int32_t *mb_of
         ids, mb_off, chunk_off, d.L, d.T, d.K, d.E, d.n_mb, d.tpc, d.max_chunks, chunk_cnt, hist_out,
         hist_out ? dev_status : nullptr);
   if (hist_out) hist = hist_out;
-  k_quota<<<d.n_inst, kQuotaThreads, smem_quota, st>>>(
+  (quota16 ? k_quota<int16_t> : k_quota<int32_t>)<<<d.n_inst, kQuotaThreads, smem_quota, st>>>(
       hist, quota_in, mb_ok, chunk_off, pl_host_ptr, pl_host_slot, pl_active, pl_rslot, pl_fault,
       slot_expert, d.L, d.E, d.P, d.Ns, d.pl_per_mb, d.max_chunks, quota, rank_load, slot_off,
       inst_cum_end, inst_slot_adj, inst_ok, chunk_cnt, chunks ? 1 : 0, dev_status);

@@ -30,22 +30,11 @@ __device__ __forceinline__ long long wsum_ll(long long v) {
   for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
   return v;
 }
-__device__ __forceinline__ long long wmin_ll(long long v) {
-#pragma unroll
-  for (int o = 16; o; o >>= 1) { const long long t = __shfl_xor_sync(kFull, v, o); v = t < v ? t : v; }
-  return v;
-}
 __device__ __forceinline__ long long wmax_ll(long long v) {
 #pragma unroll
   for (int o = 16; o; o >>= 1) { const long long t = __shfl_xor_sync(kFull, v, o); v = t > v ? t : v; }
   return v;
 }
-__device__ __forceinline__ unsigned long long wmax_ull(unsigned long long v) {
-#pragma unroll
-  for (int o = 16; o; o >>= 1) { const unsigned long long t = __shfl_xor_sync(kFull, v, o); v = t > v ? t : v; }
-  return v;
-}
-
 struct RsState {
   int E, P, Ns, Nb, Nr, M, R, maxc;
   long long a, b;
@@ -57,11 +46,12 @@ struct RsState {
   int32_t *nhost;     // [E]
   int32_t *nred;      // [P]
   int32_t *hslot;     // [E*maxc] host slots of e, ascending rank
+  int32_t *ord;       // [E*M]  source machines of e by descending count, ties ascending m
 };
 
 // F after adding a replica of e on rank r_new (all lanes return it).  commit: the estimate becomes
 // the state (x, RL, LT, se, host list, counters).  LT2: this warp's [M*M] scratch, flag: its [P] bytes.
-__device__ long long rs_eval(const RsState &s, int e, int r_new, int lane, int32_t *LT2,
+__device__ __forceinline__ long long rs_eval(const RsState &s, int e, int r_new, int lane, int32_t *LT2,
                              unsigned char *flag, bool commit) {
   const int M = s.M, Ns = s.Ns, R = s.R, n = s.nhost[e];
   const int32_t *hs = s.hslot + (size_t)e * s.maxc;
@@ -73,7 +63,7 @@ __device__ long long rs_eval(const RsState &s, int e, int r_new, int lane, int32
   if (lane < pos) my_slot = hs[lane];
   else if (lane > pos && lane <= n) my_slot = hs[lane - 1];
   if (my_slot >= 0) my_rank = my_slot / Ns;
-  long long load = 0;
+  int load = 0;                                                      // rank loads stay below 2^31 (T * K < 2^31)
   if (isH) {
     load = s.RL[my_rank];
     if (my_slot >= 0)
@@ -90,54 +80,53 @@ __device__ long long rs_eval(const RsState &s, int e, int r_new, int lane, int32
   if (commit && isH)
     for (int m = 0; m < M; m++) s.x[row * M + m] = 0;
   __syncwarp();
-  // commodities (e, m): descending count, ties ascending m
-  const int cnt_m = lane < M ? s.cm[e * M + lane] : 0;
-  unsigned done = 0;
+  // commodities (e, m) in descending count, ties ascending m (s.ord, fixed per expert); for each the
+  // token-by-token rule in closed form: with f(l) = sum over allowed hosts of max(0, l - load), the level
+  // sits on top of the highest allowed load l* with f(l*) <= c: lam = l* + (c - f(l*)) / m, m = #{load <= l*},
+  // and the (c - f(l*)) % m left-over tokens go one each to the lowest ranks among those m hosts
   const unsigned lanes_lt = (1u << lane) - 1u;
-  for (;;) {
-    unsigned long long key = 0;
-    if (lane < M && cnt_m > 0 && !((done >> lane) & 1u))
-      key = ((unsigned long long)(unsigned)cnt_m << 32) | (unsigned)(0x7fffffff - lane);
-    key = wmax_ull(key);
-    if (key == 0) break;
-    const int ms = 0x7fffffff - (int)(key & 0xffffffffu);
-    const long long c = (long long)(key >> 32);
-    done |= 1u << ms;
-    const unsigned local = __ballot_sync(kFull, isH && my_rank / R == ms);
-    const unsigned allowed = local ? local : __ballot_sync(kFull, isH);
+  const unsigned hosts = __ballot_sync(kFull, isH);
+  const int my_mach = my_rank / R;
+  for (int k = 0; k < M; k++) {
+    const int ms = s.ord[e * M + k];
+    const int c = s.cm[e * M + ms];
+    if (c <= 0) break;
+    const unsigned local = __ballot_sync(kFull, isH && my_mach == ms);
+    const unsigned allowed = local ? local : hosts;
     const bool al = (allowed >> lane) & 1u;
-    // the token-by-token rule in closed form: level lam = largest integer with sum max(0, lam - load) <= c
-    long long lo = wmin_ll(al ? load : LLONG_MAX), hi = lo + c;
-    while (lo < hi) {
-      const long long mid = (lo + hi + 1) >> 1;
-      const long long need = wsum_ll(al && mid > load ? mid - load : 0);
-      if (need <= c) lo = mid; else hi = mid - 1;
+    long long f = 0;
+    for (unsigned mk = allowed; mk; mk &= mk - 1) {
+      const int lb = __shfl_sync(kFull, load, __ffs(mk) - 1);
+      if (al && load > lb) f += load - lb;
     }
-    long long give = al && lo > load ? lo - load : 0;
-    const long long rem = c - wsum_ll(give);
-    const bool elig = al && load <= lo;                              // remainder: lowest ranks first
-    const unsigned em = __ballot_sync(kFull, elig);
-    if (elig && __popc(em & lanes_lt) < rem) give++;
+    const bool cand = al && f <= (long long)c;                       // the least-loaded allowed host always is
+    const int lstar = __reduce_max_sync(kFull, cand ? load : INT_MIN);
+    const int fstar = __shfl_sync(kFull, (int)f, __ffs(__ballot_sync(kFull, cand && load == lstar)) - 1);
+    const unsigned le = __ballot_sync(kFull, al && load <= lstar);
+    const int m = __popc(le), rest = c - fstar;
+    const int lam = lstar + rest / m, rem = rest % m;
+    int give = 0;
+    if ((le >> lane) & 1u) give = lam - load + (__popc(le & lanes_lt) < rem ? 1 : 0);
     load += give;
-    if (give) atomicAdd(LT2 + ms * M + my_rank / R, (int)give);
-    if (commit && give) s.x[row * M + ms] = (int)give;
+    if (give) atomicAdd(LT2 + ms * M + my_mach, give);
+    if (commit && give) s.x[row * M + ms] = give;
   }
   __syncwarp();
   // L' = max over all ranks with the hosts' new loads; C' = max off-diagonal of LT2
   if (isH) flag[my_rank] = 1;
   __syncwarp();
-  long long lmax = isH ? load : LLONG_MIN;
+  int lmax = isH ? load : INT_MIN;
   for (int r = lane; r < s.P; r += 32)
     if (!flag[r] && s.RL[r] > lmax) lmax = s.RL[r];
-  lmax = wmax_ll(lmax);
-  long long cmax = 0;
+  lmax = __reduce_max_sync(kFull, lmax);
+  int cmax = 0;
   for (int i = lane; i < M * M; i += 32)
     if (i / M != i % M && LT2[i] > cmax) cmax = LT2[i];
-  cmax = wmax_ll(cmax);
+  cmax = __reduce_max_sync(kFull, cmax);
   __syncwarp();
   if (isH) flag[my_rank] = 0;
   if (commit) {
-    if (isH) s.RL[my_rank] = (int)load;
+    if (isH) s.RL[my_rank] = load;
     for (int i = lane; i < M * M; i += 32) s.LT[i] = LT2[i];
     __syncwarp();
     if (isH) s.hslot[(size_t)e * s.maxc + lane] = row;               // still ascending rank
@@ -148,12 +137,15 @@ __device__ long long rs_eval(const RsState &s, int e, int r_new, int lane, int32
     }
   }
   __syncwarp();
-  return s.a * lmax + s.b * cmax;
+  return s.a * (long long)lmax + s.b * (long long)cmax;
 }
 
 }  // namespace
 
-__global__ void __launch_bounds__(kRsThreads)
+#ifndef FOREMOE_RS_MINB
+#define FOREMOE_RS_MINB 4
+#endif
+__global__ void __launch_bounds__(kRsThreads, FOREMOE_RS_MINB)
 k_replica_search(const int32_t *__restrict__ hist_v, const int32_t *__restrict__ placed_se, int L, int E,
                  int P, int Nb, int Nr, int M, int maxc, long long a, long long b,
                  int32_t *__restrict__ out_se, int32_t *__restrict__ replicas_out,
@@ -173,7 +165,8 @@ k_replica_search(const int32_t *__restrict__ hist_v, const int32_t *__restrict__
   s.nhost = s.LT + M * M;
   s.nred = s.nhost + E;
   s.hslot = s.nred + P;
-  int32_t *inQ = s.hslot + E * maxc;   // [E]
+  s.ord = s.hslot + E * maxc;
+  int32_t *inQ = s.ord + E * M;        // [E]
   const int lt2n = M * M < 2 ? 2 : M * M;
   int32_t *LT2 = inQ + E + warp * lt2n;                                     // [warps][max(M*M, 2)]
   unsigned char *flag = (unsigned char *)(inQ + E + kRsWarps * lt2n) + warp * ((P + 3) / 4 * 4);
@@ -212,6 +205,15 @@ k_replica_search(const int32_t *__restrict__ hist_v, const int32_t *__restrict__
     for (int m = 0; m < M; m++) t += s.cm[e * M + m];
     if (t > INT_MAX) fault |= FOREMOE_FAULT_ID_RANGE;
     ctot[e] = (int)t;
+    for (int m = 0; m < M; m++) {                          // position of m in e's processing order
+      const int v = s.cm[e * M + m];
+      int pos = 0;
+      for (int m2 = 0; m2 < M; m2++) {
+        const int v2 = s.cm[e * M + m2];
+        pos += (v2 > v) || (v2 == v && m2 < m);
+      }
+      s.ord[e * M + pos] = m;
+    }
   }
   if (fault) atomicOr(&s_fault, fault);
   __syncthreads();
@@ -283,10 +285,50 @@ k_replica_search(const int32_t *__restrict__ hist_v, const int32_t *__restrict__
     for (int e = 0; e < E; e++) {
       if (!inQ[e]) continue;
       const int n = s.nhost[e];
+      const int hj = lane < n ? s.hslot[(size_t)e * maxc + lane] : -1;
+      const int hr = hj >= 0 ? hj / Ns : -1;
+      // Lower bounds on F' of every candidate (e, .), so that candidates that cannot beat this warp's best
+      // are skipped (a candidate only replaces the best on a STRICTLY smaller Delta, so the result is the
+      // same).  Ranks outside hosts(e) + r keep their loads, the loads of hosts(e) + r keep their sum, and a
+      // link keeps at least what it carries without e's tokens:
+      //   L' >= max(two largest non-host loads as r allows, ceil((sum_hosts RL + RL[r]) / (n + 1)))
+      //   C' >= max over links of LT - (e's tokens on the link)
+      if (hr >= 0) flag[hr] = 1;
+      __syncwarp();
+      int t1 = INT_MIN, t1r = -1, t2 = INT_MIN;
+      for (int r = lane; r < P; r += 32) {
+        if (flag[r]) continue;
+        const int v = s.RL[r];
+        if (v > t1) { t2 = t1; t1 = v; t1r = r; } else if (v > t2) t2 = v;
+      }
+      const int g1 = __reduce_max_sync(kFull, t1);
+      const int owner = __ffs(__ballot_sync(kFull, t1 == g1)) - 1;
+      const int g1r = __shfl_sync(kFull, t1r, owner);
+      const int g2 = __reduce_max_sync(kFull, lane == owner ? t2 : t1);
+      const long long sumH = wsum_ll(hr >= 0 ? (long long)s.RL[hr] : 0);
+      int crest = 0;
+      if (b != 0)
+        for (int i = lane; i < M * M; i += 32) {
+          const int mi = i / M, mj = i % M;
+          if (mi == mj) continue;
+          int v = s.LT[i];
+          for (int h = 0; h < n; h++) {
+            const int j = s.hslot[(size_t)e * maxc + h];
+            if (j / Ns / s.R == mj) v -= s.x[j * M + mi];
+          }
+          crest = v > crest ? v : crest;
+        }
+      crest = __reduce_max_sync(kFull, crest);
+      __syncwarp();
+      if (hr >= 0) flag[hr] = 0;
+      __syncwarp();
       for (int r = warp; r < P; r += kRsWarps) {
         if (s.nred[r] >= Nr) continue;
-        const int hr = lane < n ? s.hslot[(size_t)e * maxc + lane] / Ns : -1;
         if (__any_sync(kFull, hr == r)) continue;
+        const long long lrest = r == g1r ? g2 : g1;
+        const long long avg = (sumH + s.RL[r] + n) / (n + 1);
+        const long long lb = a * (lrest > avg ? lrest : avg) + b * (long long)crest;
+        if (lb - F >= my_delta) continue;
         const long long delta = rs_eval(s, e, r, lane, LT2, flag, false) - F;
         if (delta < my_delta) { my_delta = delta; my_idx = e * P + r; }   // strict: first of this warp wins
       }
@@ -330,7 +372,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_replica_search(
       max_copies < 1 || max_copies > 31 || a < 0 || b < 0 || a > (1 << 20) || b > (1 << 20))
     return FOREMOE_ERR_INVALID_ARG;
   const size_t smem = sizeof(int32_t) * ((size_t)d.E * M + d.E + d.S + (size_t)d.S * M + d.P + (size_t)M * M +
-                                         d.E + d.P + (size_t)d.E * max_copies + d.E +
+                                         d.E + d.P + (size_t)d.E * max_copies + (size_t)d.E * M + d.E +
                                          (size_t)kRsWarps * (M * M < 2 ? 2 : M * M) +
                                          (size_t)kRsWarps * ((d.P + 3) / 4));
   if (smem > 200 * 1024) return FOREMOE_ERR_INVALID_ARG;

@@ -50,7 +50,8 @@
  *  - Data-dependent faults cannot be seen without a sync; they are OR-ed into *dev_status
  *    (device int32, may be NULL, never cleared by the library): FOREMOE_FAULT_* bits.  On a
  *    device fault the affected instance's outputs are unspecified, all writes stay in bounds.
- *  - Requirements: T * K < 2^31; 1 <= K <= 32, K <= E; E % P == 0 and Nb == E / P; Nr >= 0;
+ *  - Requirements: 0 <= T, T * K < 2^31 (T = 0, a step without tokens, is valid: the [L][T][K] arrays
+ *    are then empty and may be NULL); 1 <= K <= 32, K <= E; E % P == 0 and Nb == E / P; Nr >= 0;
  *    row bytes H * es (es = 2 for bf16, 4 for fp32) a multiple of 16; x / buf / expert_out / y
  *    16-byte aligned; int32 / fp32 arrays 4-byte aligned (K = 10 id rows are only 8-byte
  *    aligned -- nothing wider is assumed).

@@ -284,6 +284,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine_bwd(
   if (rc) return rc;
   if (layer < 0 || layer >= d.L || mb_begin < 0 || mb_end > d.n_mb || mb_begin > mb_end)
     return FOREMOE_ERR_INVALID_ARG;
+  if (d.T == 0) return FOREMOE_OK;                     // a step without tokens: the plan arrays may be NULL
   if (!mb_off || !inv || !w || !dy || !d_expert_out || !aligned(dy, 16) ||
       !aligned(d_expert_out, 16) || (expert_out && !aligned(expert_out, 16)))
     return FOREMOE_ERR_INVALID_ARG;

@@ -295,6 +295,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_dispatch(const for
   int rc = make_dims(shape, &d);
   if (rc) return rc;
   if ((rc = check_range(d, layer, mb_begin, mb_end))) return rc;
+  if (d.T == 0) return FOREMOE_OK;                     // a step without tokens: the plan arrays may be NULL
   if (!mb_off || !inv || !x || !buf || !aligned(x, 16) || !aligned(buf, 16))
     return FOREMOE_ERR_INVALID_ARG;
   if (mb_begin == mb_end) return FOREMOE_OK;
@@ -309,6 +310,7 @@ static int combine_entry(const foremoe_shape_t *shape, int32_t layer, int32_t mb
   int rc = make_dims(shape, &d);
   if (rc) return rc;
   if ((rc = check_range(d, layer, mb_begin, mb_end))) return rc;
+  if (d.T == 0) return FOREMOE_OK;
   if (!mb_off || !inv || !expert_out || !y || !aligned(expert_out, 16) || !aligned(y, 16))
     return FOREMOE_ERR_INVALID_ARG;
   if (mb_begin == mb_end) return FOREMOE_OK;
@@ -322,7 +324,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_combine(const fore
                                const float *w, const void *expert_out, float *y,
                                int32_t *dev_status, void *stream) {
   (void)dev_status;
-  if (!w) return FOREMOE_ERR_INVALID_ARG;
+  if (!w && !(shape && shape->T == 0)) return FOREMOE_ERR_INVALID_ARG;
   return combine_entry(shape, layer, mb_begin, mb_end, mb_off, inv, w, expert_out, y, stream);
 }
 

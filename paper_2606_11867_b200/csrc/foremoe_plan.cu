@@ -723,6 +723,8 @@ k_assign_pairs(const int32_t *__restrict__ ids, const int32_t *__restrict__ mb_o
   for (int it = 0; it < kIter; it++) {
     const int e = my[it];
     const bool ok = (unsigned)e < (unsigned)E;
+    // match.any is the kernel's bound (about 37 cycles of the SM's ADU each); ballots over the id bits
+    // instead moved the bound to issue slots at the same time per launch (profiles/r02_planner.md)
     const unsigned grp = __match_any_sync(full, ok ? (unsigned)e : (0x80000000u | lane));
     const int pre = wc[ok ? e : 0];
     __syncwarp();
@@ -820,7 +822,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const fo
   Dims d;
   int rc = make_dims(shape, &d);
   if (rc) return rc;
-  if (!ids || !mb_off || !hist) return FOREMOE_ERR_INVALID_ARG;
+  if ((!ids && d.T > 0) || !mb_off || !hist) return FOREMOE_ERR_INVALID_ARG;   // T = 0: there are no ids
   cudaStream_t st = (cudaStream_t)stream;
   if (cudaMemsetAsync(hist, 0, sizeof(int32_t) * (size_t)d.n_inst * d.E, st) != cudaSuccess)
     return FOREMOE_ERR_CUDA;
@@ -930,7 +932,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
   Dims d;
   int rc = make_dims(shape, &d);
   if (rc) return rc;
-  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
+  if ((!ids && d.T > 0) || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
     return FOREMOE_ERR_INVALID_ARG;
   if ((pair_slot == nullptr) != (inv == nullptr)) return FOREMOE_ERR_INVALID_ARG;
   return launch_assign(d, ids, mb_off, hist, nullptr, nullptr, slot_expert, quota_in, quota, rank_load,
@@ -945,8 +947,8 @@ extern "C" __attribute__((visibility("default"))) int foremoe_plan(const foremoe
   Dims d;
   int rc = make_dims(shape, &d);
   if (rc) return rc;
-  if (!ids || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !pair_slot || !inv ||
-      !workspace)
+  if (!mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace ||
+      (d.T > 0 && (!ids || !pair_slot || !inv)))       // T = 0: there are no pairs, the arrays may be NULL
     return FOREMOE_ERR_INVALID_ARG;
   if (d.T == 0) {                                   // no chunks to take the histogram from: all zero
     cudaStream_t st = (cudaStream_t)stream;

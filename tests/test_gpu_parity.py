@@ -533,3 +533,48 @@ def test_cuda_graph_replay(cuda_device):
     torch.cuda.synchronize()
     for a, b in zip(eager, graphed):
         assert torch.equal(a.view(torch.uint8), b.view(torch.uint8))
+
+
+def test_empty_step(cuda_device):
+    """T = 0 (a step without tokens): foremoe_plan and load_hist + assign give the all-zero plan of the
+    oracle, and the data-path calls on the empty range are no-ops."""
+    rng = np.random.default_rng(5)
+    L, E, K, P, Nr = 2, 16, 2, 4, 1
+    ids, w, mb_off, se, Nb, Ns = G.random_case(rng, L, E, K, P, Nr, [0, 0, 0])
+    shape = fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=0, n_mb=3, H=64, act_dtype=fm.ACT_FP32)
+    ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+    sp = G.gpu_plan(shape, ids, w, mb_off, se)
+    assert sp.faults() == 0 and ref["fault"] == 0
+    for name in ("hist", "step_hist", "quota", "rank_load", "slot_off"):
+        got = getattr(sp, name).cpu().numpy()
+        assert (got == ref[name]).all() and (got == 0).all(), name
+    x = torch.zeros((1, shape.H), device=G.DEV)
+    buf = torch.full((1, shape.H), 7.0, device=G.DEV)
+    y = torch.full((1, shape.H), 7.0, device=G.DEV)
+    sp.dispatch(0, 0, 3, x, None, buf)
+    sp.combine(1, 1, 2, buf, y)
+    torch.cuda.synchronize()
+    assert (buf == 7.0).all() and (y == 7.0).all()
+
+
+@pytest.mark.parametrize("E,P,Nr", [(64, 8, 2), (512, 32, 4), (1024, 32, 8)])
+def test_quota_kernel_index_width(cuda_device, E, P, Nr):
+    """k_quota holds its index tables as int32 for small shapes and as int16 once shared memory would cap
+    the resident CTAs (E = 512 and up here): the same random plans, heavy replication, both against O2."""
+    rng = np.random.default_rng(E)
+    L, K = 2, 4
+    ids, w, mb_off, se, Nb, Ns = G.random_case(rng, L, E, K, P, Nr, [300, 0, 777, 64], skew=1.3,
+                                               empty_slots=False, same_rank_dup=False)
+    # replicate the hottest experts many times so that Phase B iterates
+    step = orc.load_hist(ids, mb_off, E)[1]
+    for l in range(L):
+        hot = np.argsort(-step[l])[:max(2, P // 4)]
+        for r in range(P):
+            for a in range(Nr):
+                se[l, r * Ns + Nb + a] = hot[(r + a) % len(hot)]
+    shape = fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=4, H=64, act_dtype=fm.ACT_FP32)
+    ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+    assert ref["fault"] == 0
+    sp = G.gpu_plan(shape, ids, w, mb_off, se)
+    assert sp.faults() == 0
+    G.assert_plan_equal(sp, ref, f"index-width E={E}")

@@ -349,14 +349,24 @@ class Workload:
         if probes is not None:
             e1.record()
             probes["plan"].append((e0, e1, self.cfg.T * self.cfg.L))
+        run = None                       # an open run of un-probed instances: (start event, tokens so far)
         for n, (l, i) in enumerate(self.instances):
             if probes is not None and stride and n % stride == 0:
                 a = []
                 self.instance(l, i, a)
                 for j, name in enumerate(("dispatch", "combine", "combine_bwd", "dispatch_bwd")[:len(a) - 1]):
                     probes[name].append((a[j], a[j + 1], self.tok[i]))
+                if stride >= 4:          # the stride - 1 instances up to the next probe run back to back, un-probed:
+                    run = [a[-1], 0]     # one pair of events around the whole run gives the data path's rate IN the loop
             else:
                 self.instance(l, i)
+                if run is not None:
+                    run[1] += self.tok[i]
+                    if n % stride == stride - 1:
+                        e = torch.cuda.Event(enable_timing=True)
+                        e.record()
+                        probes["run"].append((run[0], e, run[1]))
+                        run = None
 
     def capture_graph(self):
         """Capture the per-instance loop (dispatch + combine of every instance) into ONE CUDA graph:
@@ -519,7 +529,7 @@ def run_ours(args, cfg) -> None:
         wl.step_streams() if args.streams > 1 else wl.step()
     torch.cuda.synchronize()
     assert wl.plan.faults() == 0
-    probes = {"plan": [], "dispatch": [], "combine": [], "combine_bwd": [], "dispatch_bwd": []}
+    probes = {"plan": [], "dispatch": [], "combine": [], "combine_bwd": [], "dispatch_bwd": [], "run": []}
     if args.graph or args.streams > 1:
         # per-kernel probes cannot sit inside a graph / between concurrent streams: one extra, untimed step
         wl.step(probes, args.probe_stride)
@@ -543,7 +553,9 @@ def run_ours(args, cfg) -> None:
     ms_max, units = multi.aggregate(ms, wl.routed_tokens * args.steps, dev)
     value = units / (ms_max * 1e-3)
     launches = wl.launches_per_step * args.steps
+    bpt["run"] = total_bpt - bpt["plan"]          # a run = whole instances: every data-path kernel of the stage
     kern = probe_stats(probes, bpt)
+    in_loop = kern.pop("run", None)
     dom = "combine" if bpt["combine"] >= bpt["dispatch"] else "dispatch"
     if upd:
         dom = "combine_bwd"
@@ -567,6 +579,12 @@ def run_ours(args, cfg) -> None:
                 "whole_path_frac": value / world * total_bpt / 1e9 / peak,
                 "whole_path_frac_of_nominal_8TBs": value / world * total_bpt / 1e9 / NOMINAL_HBM_GBS,
                 "kernels": kern}
+    if in_loop:
+        # the same kernels between launches of their own kind, no event inside: runs of (probe stride - 1) whole
+        # instances, one pair of CUDA events around each run, inside the timed region
+        roofline["data_path_in_loop"] = {"gbs": in_loop["gbs"], "frac": in_loop["gbs"] / peak,
+                                         "runs_timed": in_loop["launches_timed"], "avg_run_ms": in_loop["avg_ms"],
+                                         "bytes_per_token": in_loop["bytes_per_token"]}
     clocks = clk.summary()
     # load balance of the plan (not timed): per instance max rank load / mean rank load, against the
     # natural placement (expert e on rank e // Nb, no replicas) -- PAPER.md:503-507 reports this ratio

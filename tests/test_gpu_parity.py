@@ -578,3 +578,34 @@ def test_quota_kernel_index_width(cuda_device, E, P, Nr):
     sp = G.gpu_plan(shape, ids, w, mb_off, se)
     assert sp.faults() == 0
     G.assert_plan_equal(sp, ref, f"index-width E={E}")
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_fuzz_shapes(cuda_device, seed):
+    """400 random shapes per seed (P from 1 to 64, Nb from 1 to 16 incl. non powers of two, K from 1 to 32, Nr
+    from 0 to 5, empty micro-steps, duplicate ids in a token, one expert replicated on every rank): the plan
+    by foremoe_plan and by load_hist + assign against the oracle, every output."""
+    rng = np.random.default_rng(seed)
+    for _ in range(400):
+        P = int(rng.choice([1, 2, 3, 4, 8, 16, 32, 64]))
+        Nb = int(rng.choice([1, 2, 3, 4, 7, 16]))
+        E = P * Nb
+        K = int(rng.integers(1, min(E, 32) + 1))
+        Nr = int(rng.choice([0, 1, 2, 5]))
+        L = int(rng.integers(1, 4))
+        n_mb = int(rng.integers(1, 6))
+        sizes = [int(rng.choice([0, 1, 7, 100, 513, 3000])) for _ in range(n_mb)]
+        if sum(sizes) * K > 60000:
+            sizes = [min(s, 400) for s in sizes]
+        ids, w, mb_off, se, _, Ns = G.random_case(rng, L, E, K, P, Nr, sizes, dup_tokens=bool(rng.integers(2)),
+                                                  skew=float(rng.choice([0.0, 1.0, 2.5])))
+        if rng.random() < 0.3 and Nr:
+            for l in range(L):
+                for r in range(P):
+                    se[l, r * Ns + Nb] = se[l, 0]
+        shape = fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=n_mb, H=8, act_dtype=fm.ACT_FP32)
+        ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+        sp = G.gpu_plan(shape, ids, w, mb_off, se)
+        assert sp.faults() == ref["fault"], (shape, sp.faults(), ref["fault"])
+        if ref["fault"] == 0:
+            G.assert_plan_equal(sp, ref, str(shape))

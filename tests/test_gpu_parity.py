@@ -609,3 +609,36 @@ def test_fuzz_shapes(cuda_device, seed):
         assert sp.faults() == ref["fault"], (shape, sp.faults(), ref["fault"])
         if ref["fault"] == 0:
             G.assert_plan_equal(sp, ref, str(shape))
+
+
+def test_fuzz_data_path_shapes(cuda_device):
+    """250 random data-path shapes (K from 1 to 32, rows from 16 bytes to 7 KB incl. sizes that are no
+    multiple of the kernels' slices, bf16 and fp32, empty and tiny micro-steps, both stream-order modes):
+    perm / buf bit-exact and y bit-identical against O5 / O6, also on expert outputs that differ per k."""
+    rng = np.random.default_rng(77)
+    done = 0
+    while done < 250:
+        P = int(rng.choice([1, 2, 4, 8]))
+        Nb = int(rng.choice([1, 2, 4, 16]))
+        E = P * Nb
+        K = int(rng.choice([k for k in (1, 2, 3, 4, 5, 6, 8, 10, 16, 32) if k <= E]))
+        Nr, L, n_mb = int(rng.choice([0, 1, 2])), int(rng.integers(1, 3)), int(rng.integers(1, 4))
+        bf16 = bool(rng.integers(2))
+        H = (8 if bf16 else 4) * int(rng.choice([1, 2, 3, 8, 31, 64, 65, 128, 256, 257, 896, 1024, 1792]))
+        sizes = [int(rng.choice([0, 1, 5, 33, 200, 700])) for _ in range(n_mb)]
+        while sum(sizes) * K * H > 6_000_000:
+            sizes = [s // 2 for s in sizes]
+        ids, w, mb_off, se, _, Ns = G.random_case(rng, L, E, K, P, Nr, sizes, skew=float(rng.choice([0.0, 1.5])))
+        shape = fm.Shape(L=L, E=E, K=K, P=P, Nb=Nb, Nr=Nr, T=int(mb_off[-1]), n_mb=n_mb, H=H,
+                         act_dtype=fm.ACT_BF16 if bf16 else fm.ACT_FP32, flags=int(rng.integers(2)))
+        if shape.T == 0:
+            continue
+        ref = G.oracle_plan(ids, mb_off, se, E, P, Ns)
+        if ref["fault"]:
+            continue
+        sp = G.gpu_plan(shape, ids, w, mb_off, se)
+        G.assert_plan_equal(sp, ref, str(shape))
+        x = {i: torch.randn(max(int(mb_off[i + 1] - mb_off[i]), 1), H, device=G.DEV).to(shape.act_torch_dtype)
+             for i in range(n_mb)}
+        G.check_data_path(sp, ref, x, range(L), range(n_mb), str(shape))
+        done += 1

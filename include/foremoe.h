@@ -171,6 +171,47 @@ int foremoe_plan(const foremoe_shape_t *shape, const int32_t *ids, const int32_t
                  int32_t *dev_status, void *stream);
 
 /*
+ * foremoe_plan for callers that cannot bring a workspace.  Same arguments, outputs, faults and
+ * stream behaviour as foremoe_plan, bit for bit, minus `workspace` / `workspace_bytes`.
+ *
+ * Who needs it: code that runs as a guest inside an engine whose own allocator took (almost) all of
+ * the GPU's memory when it started, so that a cudaMalloc of even a few MB fails; a plugin whose host
+ * allows device allocation only during initialisation; a step loop that cannot afford the
+ * device-wide synchronisation that comes with cudaMalloc / cudaFree.  Such callers already own their
+ * inputs and outputs but have nowhere to take the plan kernels' scratch from.
+ *
+ * Where the scratch lives instead: in ONE array of FOREMOE_NOALLOC_SCRATCH_BYTES (8 MiB) of device
+ * global memory that is part of the library image.  Every GPU on which the process uses CUDA while
+ * the library is loaded carries those 8 MiB until the process exits, whether or not this call is
+ * ever made.  The call itself allocates and frees nothing and calls no library routine that does.
+ *
+ * Limit: the shape must satisfy foremoe_workspace_bytes(shape) <= FOREMOE_NOALLOC_SCRATCH_BYTES;
+ * otherwise the call returns FOREMOE_ERR_WORKSPACE and enqueues nothing (checked on the host before
+ * any CUDA call; compare the two numbers yourself to know in advance).  Roughly: n_mb * L * S * 8 +
+ * L * (T * K / 4096 + n_mb) * E * 4 bytes -- e.g. E = 128, K = 8, P = 8, Ns = 18, L = 4, 8 micro-steps
+ * of 16 K tokens need 0.56 MiB; the 48-layer, 512 K-token config 2 needs 26.5 MiB and must use foremoe_plan.
+ *
+ * First call on a device: the library looks up the array's address on the calling thread's current
+ * device (one cudaGetSymbolAddress, remembered per device; FOREMOE_ERR_CUDA if it fails).  That
+ * look-up is a runtime query, not a launch: make the first call on every device an ordinary eager
+ * one, before any stream capture begins on that device.  Later calls only launch kernels.
+ *
+ * Sharing: all calls on one device use the same array, on whatever stream, from whatever thread.
+ * Two calls whose kernels can be in flight on the GPU at the same time (different streams without an
+ * event between them, or two host threads on two streams) overwrite each other's scratch and both
+ * results are garbage without any fault bit: order them yourself.  Calls in one stream are safe
+ * back to back.  The array still holds the previous call's tables when the next call starts; that
+ * is harmless, because every table is rebuilt before it is read and nothing in it has to start at
+ * zero, so the library clears nothing.  Unlike every other entry point, this one is therefore NOT
+ * re-entrant across streams.
+ */
+#define FOREMOE_NOALLOC_SCRATCH_BYTES (8u << 20)
+int foremoe_plan_noalloc(const foremoe_shape_t *shape, const int32_t *ids, const int32_t *mb_off,
+                         const int32_t *slot_expert, const int32_t *quota_in, int32_t *hist,
+                         int64_t *step_hist, int32_t *quota, int32_t *rank_load, int32_t *slot_off,
+                         int32_t *pair_slot, int32_t *inv, int32_t *dev_status, void *stream);
+
+/*
  * (a4-a5) Dispatch of micro-steps [mb_begin, mb_end) of one layer: the permutation and the row
  * gather into contiguous per-rank / per-slot buffers.
  *   inv   [L][T][K] from foremoe_assign (the whole array; the call indexes layer / range itself).

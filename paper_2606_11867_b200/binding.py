@@ -38,7 +38,7 @@ ACT_FP32 = 1
 FLAG_PLAN_STABLE = 1
 
 EXPORTS = ("foremoe_version", "foremoe_workspace_bytes", "foremoe_warmup", "foremoe_load_hist", "foremoe_assign",
-           "foremoe_plan",
+           "foremoe_plan", "foremoe_plan_noalloc",
            "foremoe_dispatch", "foremoe_combine", "foremoe_combine_bwd", "foremoe_dispatch_bwd",
            "foremoe_base_placement", "foremoe_base_placement_machines", "foremoe_source_ids", "foremoe_local_placement", "foremoe_traffic",
            "foremoe_local_placement_theta", "foremoe_tradeoff_select",
@@ -123,6 +123,7 @@ def lib() -> C.CDLL:
         l.foremoe_load_hist.argtypes = [sp, vp, vp, vp, vp, vp, vp]
         l.foremoe_assign.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
         l.foremoe_plan.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp]
+        l.foremoe_plan_noalloc.argtypes = [sp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_dispatch.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_combine.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         l.foremoe_combine_bwd.argtypes = [sp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -228,6 +229,32 @@ def plan(shape: Shape, ids, mb_off, slot_expert, quota_in, hist, step_hist, quot
         _dev(step_hist, torch.int64), _dev(quota, torch.int32), _dev(rank_load, torch.int32),
         _dev(slot_off, torch.int32), _dev(pair_slot, torch.int32), _dev(inv, torch.int32), _dev(workspace),
         workspace.numel() * workspace.element_size(), _dev(dev_status, torch.int32), _stream()))
+
+
+NOALLOC_SCRATCH_BYTES = 8 << 20     # FOREMOE_NOALLOC_SCRATCH_BYTES of include/foremoe.h
+
+
+def plan_noalloc(shape: Shape, ids, mb_off, slot_expert, quota_in, hist, step_hist, quota, rank_load,
+                 slot_off, pair_slot, inv, dev_status=None) -> None:
+    """``plan`` without a workspace argument, for callers that cannot allocate device memory where they
+    plan (a guest of an engine that reserved all of HBM, a host that forbids allocation after start-up,
+    a loop that must not take cudaMalloc's device-wide sync).  The scratch is an 8 MiB array built into
+    the library, one per GPU, shared by every call: shapes whose ``workspace_bytes`` exceed
+    ``NOALLOC_SCRATCH_BYTES`` are refused, and calls that could overlap on the GPU (two streams, no
+    event between them) corrupt each other -- keep them on one stream or order them.  Make the first
+    call on a device an eager one (it looks the array's address up).  Outputs equal ``plan``'s."""
+    need = workspace_bytes(shape)
+    if need > NOALLOC_SCRATCH_BYTES:        # same refusal as the C entry point's, with both numbers spelled out
+        err = ForeMoEError("foremoe_plan_noalloc", ERR_WORKSPACE)
+        err.args = (f"foremoe_plan_noalloc: this shape needs {need} bytes of scratch, the built-in array holds "
+                    f"{NOALLOC_SCRATCH_BYTES}; use plan() with a caller-owned workspace",)
+        raise err
+    _check("foremoe_plan_noalloc", lib().foremoe_plan_noalloc(
+        C.byref(shape.c()), _dev(ids, torch.int32), _dev(mb_off, torch.int32),
+        _dev(slot_expert, torch.int32), _dev(quota_in, torch.int32), _dev(hist, torch.int32),
+        _dev(step_hist, torch.int64), _dev(quota, torch.int32), _dev(rank_load, torch.int32),
+        _dev(slot_off, torch.int32), _dev(pair_slot, torch.int32), _dev(inv, torch.int32),
+        _dev(dev_status, torch.int32), _stream()))
 
 
 def dispatch(shape: Shape, layer: int, mb_begin: int, mb_end: int, mb_off, inv, x, perm, buf,

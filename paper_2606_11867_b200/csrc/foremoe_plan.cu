@@ -961,3 +961,59 @@ extern "C" __attribute__((visibility("default"))) int foremoe_plan(const foremoe
   return launch_assign(d, ids, mb_off, nullptr, hist, step_hist, slot_expert, quota_in, quota, rank_load,
                        slot_off, pair_slot, inv, workspace, workspace_bytes, dev_status, (cudaStream_t)stream);
 }
+
+// =============================================================================================
+// foremoe_plan_noalloc: foremoe_plan for callers that have no device memory to hand over as workspace
+// =============================================================================================
+// Some users of this library cannot obtain device scratch at the point where they need a plan: a
+// component running inside a serving or training engine whose allocator reserved (nearly) all of
+// HBM at start-up, so that a cudaMalloc from a guest fails; a plugin whose host forbids allocation
+// after initialisation; a step loop that may not pay the device-wide synchronisation a cudaMalloc /
+// cudaFree implies.  For them the workspace of the plan kernels lives in the library image itself:
+// one fixed array in device global memory, reserved on every GPU that loads the library for as long
+// as the process lives.
+//
+// In host code the name `g_noalloc_scratch` is only a handle the runtime knows the array by -- it is
+// NOT the array's device address (handing &g_noalloc_scratch to a kernel would fault, or quietly use
+// host memory on systems where the GPU can reach it).  The device address differs per GPU and is
+// asked for once per device with cudaGetSymbolAddress, with that device current, and memoised.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[FOREMOE_NOALLOC_SCRATCH_BYTES];
+
+static std::atomic<void *> g_noalloc_ptr[foremoe::kMaxDevices];     // zero-initialised: address unknown
+
+// Device address of the scratch array on the calling thread's current device, or NULL on error.
+// Two threads that miss together both ask the runtime and store the same address: no lock.
+static void *noalloc_scratch_ptr() {
+  const int dev = current_device();
+  if (dev < 0) return nullptr;
+  void *p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+  if (p) return p;
+  if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) {
+    (void)cudaGetLastError();               // do not leave the error sticky for the caller's next call
+    return nullptr;
+  }
+  g_noalloc_ptr[dev].store(p, std::memory_order_release);
+  return p;
+}
+
+extern "C" __attribute__((visibility("default"))) int foremoe_plan_noalloc(
+    const foremoe_shape_t *shape, const int32_t *ids, const int32_t *mb_off, const int32_t *slot_expert,
+    const int32_t *quota_in, int32_t *hist, int64_t *step_hist, int32_t *quota, int32_t *rank_load,
+    int32_t *slot_off, int32_t *pair_slot, int32_t *inv, int32_t *dev_status, void *stream) {
+  Dims d;
+  int rc = make_dims(shape, &d);
+  if (rc) return rc;
+  // the size check comes first and touches no CUDA state: a shape that does not fit is refused
+  // before any device is asked for anything
+  if (make_workspace(d).total > (size_t)FOREMOE_NOALLOC_SCRATCH_BYTES) return FOREMOE_ERR_WORKSPACE;
+  if (!mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off ||
+      (d.T > 0 && (!ids || !pair_slot || !inv)))
+    return FOREMOE_ERR_INVALID_ARG;
+  void *scratch = noalloc_scratch_ptr();
+  if (!scratch) return FOREMOE_ERR_CUDA;
+  // No section of the workspace has to start at zero: k_mb_tables, k_placement_tables, k_chunk_hist and
+  // k_quota each write every word a later kernel of THIS call reads (the existing entry points are
+  // driven with uninitialised workspaces), so what the previous call left behind is never seen.
+  return foremoe_plan(shape, ids, mb_off, slot_expert, quota_in, hist, step_hist, quota, rank_load, slot_off,
+                      pair_slot, inv, scratch, (size_t)FOREMOE_NOALLOC_SCRATCH_BYTES, dev_status, stream);
+}

@@ -43,6 +43,13 @@
  *    path right after it is covered.  The data-path kernels then fetch their first plan entries
  *    while the preceding kernel drains (activations are still only touched after the dependency);
  *    worth 4 % at one-sample micro-steps, under 1 % at 16 K tokens (profiles/r02_sweeps.md).
+ *    The promise covers ONE kernel back because the library's own kernels release their dependents
+ *    only after their own grid-dependency wait has returned: in  [kernel that writes w] ->
+ *    foremoe_dispatch -> foremoe_combine(PLAN_STABLE)  the combine cannot start before the writer
+ *    has completed, although the dispatch between them never touches w (tests/test_gpu_pdl_chain.py).
+ *    If the kernel launched immediately before the call is the CALLER's and itself uses programmatic
+ *    dependent launch, it must do the same (griddepcontrol.wait before .launch_dependents), or the
+ *    promise has to extend to whatever that kernel was allowed to overlap.
  *  - CUDA graphs: the data-path calls (dispatch, combine, *_bwd) are stream-capturable.  The first
  *    launch of a kernel variant on a device queries occupancy and opts into large shared memory,
  *    which capture does not allow: call foremoe_warmup(shape) once per shape and device before

@@ -59,8 +59,7 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
   constexpr int KU = K_T > 0 ? K_T : 32;
   const int K = K_T > 0 ? K_T : K_rt;
   const int NV = DY + (kDw ? K : 0);
-  pdl_launch_dependents();
-  if (!early) pdl_wait();                  // no global read before the predecessor's writes are visible
+  if (!early) pdl_wait_then_release();     // no global read before the predecessor's writes are visible
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t vstride = (uint32_t)nt * 16u, sstride = (uint32_t)NV * vstride;   // bytes; slot (s, j) of this thread:
@@ -122,7 +121,7 @@ k_combine_bwd(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
   for (int k = 0; k < KU; k++) part[k] = 0.f;
 
   fetch_meta(0);
-  if (early) pdl_wait();                   // only mb_off / inv / w were read (FOREMOE_FLAG_PLAN_STABLE)
+  if (early) pdl_wait_then_release();      // only mb_off / inv / w were read (FOREMOE_FLAG_PLAN_STABLE)
   for (int n = 0; n < D - 1; n++) issue();
   int c_n = 0;
   for (int c_tok = 0; c_tok < n_my; c_tok++) {

@@ -29,8 +29,7 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
   constexpr int kF = kBf16 ? 8 : 4;
   constexpr int KU = K_T > 0 ? K_T : 32;
   const int K = K_T > 0 ? K_T : K_rt;
-  pdl_launch_dependents();
-  if (!early) pdl_wait();                  // no global read before the predecessor's writes are visible
+  if (!early) pdl_wait_then_release();     // no global read before the predecessor's writes are visible
   extern __shared__ __align__(128) unsigned char smem[];
   const int nt = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = nt >> 5;
   const uint32_t kstride = (uint32_t)nt * 16u, sstride = (uint32_t)K * kstride;       // bytes
@@ -91,7 +90,7 @@ k_combine_async(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l
   };
 
   fetch_meta();
-  if (early) pdl_wait();
+  if (early) pdl_wait_then_release();
   for (int n = 0; n < D - 1; n++) issue();
   for (int j = 0; j < n_my; j++) {
     issue();

@@ -40,7 +40,6 @@ k_combine_bulk(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
   constexpr int KU = K_T > 0 ? K_T : 32;
   constexpr uint32_t SB = 512u * U;
   const int K = K_T > 0 ? K_T : K_rt;
-  pdl_launch_dependents();
   extern __shared__ __align__(128) unsigned char smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
   const uint32_t stage_bytes = (uint32_t)K * SB;
@@ -52,7 +51,7 @@ k_combine_bulk(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
     for (int s = 0; s < D; s++) mbar_init(bars0 + 8u * s, 1);
   fence_proxy_async();
   __syncwarp();
-  if (!early) pdl_wait();                  // no global read before the predecessor's writes are visible
+  if (!early) pdl_wait_then_release();     // no global read before the predecessor's writes are visible
 
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
@@ -121,7 +120,7 @@ k_combine_bulk(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
       if (q < D) fetch_meta(dq[q], wq[q]);
     }
     fetch_meta(d_nxt, w_nxt);
-    if (early) pdl_wait();
+    if (early) pdl_wait_then_release();
 #pragma unroll
     for (int q = 0; q < kMaxDepth; q++)
       if (q < D) issue(dq[q], wq[q]);

@@ -19,8 +19,7 @@ k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ m
                 int32_t *__restrict__ perm, int4 *__restrict__ buf, int early) {
   // Nothing in global memory is read before the grid-dependency wait: CUDA guarantees the
   // predecessor's writes (inv from foremoe_assign, x from the caller's kernel) only after it.
-  pdl_launch_dependents();
-  if (!early) pdl_wait();
+  if (!early) pdl_wait_then_release();
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const int lane = threadIdx.x & 31;
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;
@@ -29,7 +28,7 @@ k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ m
   int d_first = -1;
   if (early) {
     if (item0 < n_items && lane < K) d_first = __ldg(inv_l + (rg.t_begin + (int)(item0 / n_slices)) * K + lane);
-    pdl_wait();
+    pdl_wait_then_release();
   }
   for (long long item = item0; item < n_items; item += warps) {
     const int tl = (int)(item / n_slices);
@@ -71,8 +70,7 @@ k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
                const int32_t *__restrict__ mb_off, int mb_begin, int mb_end, int K, int row_vec,
                int n_slices, const int4 *__restrict__ eo, float4 *__restrict__ y) {
   constexpr int kF = kBf16 ? 8 : 4;          // floats produced per 16-byte input vector
-  pdl_wait();
-  pdl_launch_dependents();
+  pdl_wait_then_release();
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
   const int lane = threadIdx.x & 31;
   const long long n_items = (long long)(rg.t_end - rg.t_begin) * n_slices;

@@ -79,6 +79,14 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // (`early`): then the first plan entries are fetched while the predecessor drains.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+// Every PDL kernel of the library releases its own dependents only AFTER its own wait has returned.
+// A dependent can then become resident no earlier than the completion of this kernel's predecessor,
+// and so on down the stream: whatever a chain of library kernels overlaps, it never overlaps a kernel
+// launched before the chain's first member.  This is what lets a FOREMOE_FLAG_PLAN_STABLE kernel fetch
+// plan entries ahead of its wait when only the kernel launched immediately before it is known not to
+// write them -- [writer of w] -> dispatch -> combine(PLAN_STABLE) would otherwise let the combine read
+// w while the writer runs (the dispatch, still waiting on the writer, would already have released it).
+__device__ __forceinline__ void pdl_wait_then_release() { pdl_wait(); pdl_launch_dependents(); }
 
 template <typename... KArgs, typename... Args>
 static cudaError_t launch_pdl(void (*kern)(KArgs...), int grid, int block, size_t smem, cudaStream_t st,

@@ -14,8 +14,7 @@ k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb
                int mb_end, int K, int row_bytes, int NS, const char *__restrict__ x,
                int32_t *__restrict__ perm, char *__restrict__ buf, int early) {
   extern __shared__ __align__(128) unsigned char smem[];
-  pdl_launch_dependents();
-  if (!early) pdl_wait();
+  if (!early) pdl_wait_then_release();
   const int n_warps = blockDim.x >> 5;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   unsigned char *rows = smem + (size_t)warp * NS * row_bytes;
@@ -23,7 +22,7 @@ k_dispatch_tma(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ mb
   int32_t *dbuf = (int32_t *)(smem + (size_t)n_warps * NS * row_bytes + (size_t)n_warps * NS * 8) +
                   (size_t)warp * NS * 32;
   const RangeInfo rg = load_range(mb_off, mb_begin, mb_end, K);
-  if (early) pdl_wait();                   // only mb_off was read (FOREMOE_FLAG_PLAN_STABLE)
+  if (early) pdl_wait_then_release();      // only mb_off was read (FOREMOE_FLAG_PLAN_STABLE)
   const int n_tok = rg.t_end - rg.t_begin;
   const int W = gridDim.x * n_warps;
   const int w0 = blockIdx.x * n_warps + warp;

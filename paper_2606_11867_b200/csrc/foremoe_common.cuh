@@ -128,15 +128,34 @@ inline int current_device() {
 
 struct DeviceMemo {
   std::atomic<uint64_t> slot[kMaxDevices][kMemoWays];
+  // The keys of one memo differ in their high bits (shared-memory bytes * 2048 + threads, threads a
+  // multiple of 32), so the way is taken from a multiplicative hash of the key, not from its low bits;
+  // a key lives in the first free way at or after its home way, and get() looks at all of them.  Only
+  // a fifth distinct key per device and kernel instantiation evicts (its home way).
+  static_assert(kMemoWays == 4, "home() returns the top two bits of the hash");
+  static unsigned home(uint64_t key) { return (unsigned)((key * 0x9E3779B97F4A7C15ull) >> 62); }
   // value in [1, 65535] or 0 when (dev, key) is not cached; key < 2^47
   int get(int dev, uint64_t key) const {
     if (dev < 0) return 0;
-    const uint64_t v = slot[dev][key % kMemoWays].load(std::memory_order_acquire);
-    return (v >> 16) == key + 1 ? (int)(v & 0xffff) : 0;
+    const unsigned h = home(key);
+    for (unsigned i = 0; i < (unsigned)kMemoWays; i++) {
+      const uint64_t v = slot[dev][(h + i) % kMemoWays].load(std::memory_order_acquire);
+      if ((v >> 16) == key + 1) return (int)(v & 0xffff);
+    }
+    return 0;
   }
   void put(int dev, uint64_t key, int value) {
-    if (dev >= 0 && value > 0 && value <= 0xffff)
-      slot[dev][key % kMemoWays].store(((key + 1) << 16) | (uint64_t)value, std::memory_order_release);
+    if (dev < 0 || value <= 0 || value > 0xffff) return;
+    const uint64_t word = ((key + 1) << 16) | (uint64_t)value;
+    const unsigned h = home(key);
+    for (unsigned i = 0; i < (unsigned)kMemoWays; i++) {
+      std::atomic<uint64_t> &s = slot[dev][(h + i) % kMemoWays];
+      uint64_t v = s.load(std::memory_order_acquire);
+      if ((v >> 16) == key + 1) return;                                  // another thread was first: same fact
+      if (v == 0 && s.compare_exchange_strong(v, word, std::memory_order_acq_rel)) return;
+      if ((v >> 16) == key + 1) return;                                  // lost the race to the same key
+    }
+    slot[dev][h].store(word, std::memory_order_release);               // all ways taken by other keys
   }
 };
 

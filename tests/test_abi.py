@@ -101,3 +101,14 @@ def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):
     monkeypatch.setattr(fm, "LIB_PATH", str(tmp_path / "missing.so"))
     with pytest.raises(ImportError):
         fm.lib()
+
+
+def test_launch_fact_memo_keeps_several_shapes_per_kernel(tmp_path):
+    """The per-device memo of launch facts holds four shapes per kernel instantiation at once (keys that
+    are all multiples of 32 must not share one way): tests/memo_check.cu, host code only."""
+    import subprocess
+    exe = tmp_path / "memo_check"
+    subprocess.run([fbuild.NVCC, "-std=c++17", "-O1", os.path.join(ROOT, "tests", "memo_check.cu"), "-o", str(exe)],
+                   check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert out.returncode == 0 and "memo ok" in out.stdout, out.stdout + out.stderr

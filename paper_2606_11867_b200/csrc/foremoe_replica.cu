@@ -353,7 +353,12 @@ k_replica_search(const int32_t *__restrict__ hist_v, const int32_t *__restrict__
       if (i / M != i % M && s.LT[i] > cmax) cmax = s.LT[i];
     lmax = wmax_ll(lmax);
     cmax = wmax_ll(cmax);
-    if (lane == 0) { F_out[2 * (size_t)inst] = F0; F_out[2 * (size_t)inst + 1] = a * lmax + b * cmax; }
+    // N_r = 0: no round ran, F0 was never taken and the state is the initial one: before = after
+    if (lane == 0) {
+      const long long F1 = a * lmax + b * cmax;
+      F_out[2 * (size_t)inst] = P * Nr > 0 ? F0 : F1;
+      F_out[2 * (size_t)inst + 1] = F1;
+    }
   }
 }
 

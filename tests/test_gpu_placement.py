@@ -329,6 +329,33 @@ def test_replica_search(cuda_device, seed):
     assert torch.equal(buf, out)
 
 
+@pytest.mark.parametrize("P,M,Nb", [(4, 2, 2), (8, 1, 4), (6, 3, 1)])
+def test_replica_search_without_redundant_slots(cuda_device, P, M, Nb):
+    """N_r = 0: there is nothing to place, no round runs, and the objective "before" is still the true
+    objective of the base placement (equal to "after"), as in O16 which evaluates it ahead of the loop."""
+    rng = np.random.default_rng(P * 100 + M)
+    E, L, n_mb, a, b = P * Nb, 2, 3, 2, 3
+    shape = fm.Shape(L=L, E=E, K=1, P=P, Nb=Nb, Nr=0, T=8, n_mb=n_mb, H=8, act_dtype=fm.ACT_FP32)
+    hv = rng.integers(1, 80, size=(n_mb, L, E, M)).astype(np.int32)
+    placed = np.stack([rng.permutation(E) for _ in range(n_mb * L)]).reshape(n_mb, L, E).astype(np.int32)
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    t = lambda x, dt=torch.int32: torch.as_tensor(np.ascontiguousarray(x), dtype=dt).to(dev)
+    out = torch.full((n_mb, L, E), -7, dtype=torch.int32, device=dev)
+    reps = torch.full((n_mb, L), -7, dtype=torch.int32, device=dev)
+    F = torch.full((n_mb, L, 2), -7, dtype=torch.int64, device=dev)
+    fm.replica_search(shape, M, 8, a, b, t(hv.reshape(n_mb, L, E * M)), t(placed), out, reps, F, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) == 0 and (reps == 0).all()
+    Fg = F.cpu().numpy()
+    for i in range(n_mb):
+        for l in range(L):
+            ref, stats, f = orc.replica_search(hv[i, l].T.copy(), placed[i, l], P, Nb, 0, M, a, b, max_copies=8)
+            assert f == 0 and stats[0] == 0 and stats[1] == stats[2] > 0
+            assert (out[i, l].cpu().numpy() == ref).all()
+            assert Fg[i, l].tolist() == [int(stats[1]), int(stats[2])], (i, l, Fg[i, l].tolist(), stats)
+
+
 def test_replica_search_golden_faults_and_pipeline(cuda_device):
     import json, os
     g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "replica_search_vectors.json")))["vectors"][0]

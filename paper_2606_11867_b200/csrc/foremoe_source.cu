@@ -129,7 +129,10 @@ k_local_placement_theta(const int32_t *__restrict__ se, const int32_t *__restric
     int v = -1;
     if (e >= 0 && e < E) {
       const int n = nloc[e * M + m];
-      const bool spill = n > 0 && den > 0 && (long long)c[e * M + m] * den * P > num * n * total;
+      // c < 2^31, den and num <= 2^20, P and n < 2^24, total < 2^31: both products can pass 2^63, so the
+      // comparison is made in 128 bits (a wrapped product would silently flip the locality decision)
+      const bool spill = n > 0 && den > 0 &&
+                         (__int128)c[e * M + m] * den * P > (__int128)num * n * total;
       if ((j / Ns) / R == m || n == 0 || spill) v = e * M + m;
     }
     dst[i] = v;

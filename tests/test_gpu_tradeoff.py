@@ -240,3 +240,51 @@ def test_alg2_planner_chain_equals_oracle_chain(cuda_device, cfg_id, kw, M, a, b
             ps, inv, perm, f = orc.assign_instance(ids_v, ref["se_v"], ref["quota_v"], ref["slot_off_v"], cfg.E * M,
                                                    base=a0 * cfg.K)
             assert f == 0 and (ap.inv[l, a0:b0].cpu().numpy().ravel() == inv).all()
+
+
+def test_theta_spill_rule_with_products_beyond_64_bits(cuda_device):
+    """The spill test of a ladder member, c * den * P > num * n_loc * total (include/foremoe.h,
+    foremoe_local_placement_theta), with P = 16 384 ranks, counts near 2^30 and theta = 2^20 / 2^20: both
+    sides pass 2^63.  Expected placement from the rule itself in Python's unbounded integers."""
+    P, Nb, Nr, M = 16384, 1, 1, 2
+    E, Ns, S, R = P * Nb, Nb + Nr, P * (Nb + Nr), P // M
+    rng = np.random.default_rng(77)
+    shape = fm.Shape(L=1, E=E, K=1, P=P, Nb=Nb, Nr=Nr, T=8, n_mb=1, H=8, act_dtype=fm.ACT_FP32)
+    se = np.full((P, Ns), -1, dtype=np.int32)
+    se[:, 0] = rng.permutation(E)
+    se[:, 1] = rng.integers(-1, E, size=P)                  # replicas anywhere (some on the other machine)
+    se = se.reshape(1, S)
+    hv = rng.integers(0, 50, size=(E, M)).astype(np.int64)
+    big = rng.choice(E, size=E // 2, replace=False)
+    hv[big] = rng.integers(1 << 29, (1 << 30) + 1, size=(E // 2, M))      # half of the experts carry almost everything
+    num, den = (1 << 20) - 3, 1 << 20
+    total = int(hv.sum())
+    assert total * num > 1 << 63 and int(hv.max()) * den * P > 1 << 63
+    # rule in exact integers: n_loc(e, m) = ranks of machine m holding e
+    holds = [[set() for _ in range(M)] for _ in range(E)]
+    for j in range(S):
+        e = int(se[0, j])
+        if e >= 0:
+            holds[e][(j // Ns) // R].add(j // Ns)
+    exp = np.full(S * M, -1, dtype=np.int32)
+    n_spill = 0
+    for j in range(S):
+        e = int(se[0, j])
+        if e < 0:
+            continue
+        for m in range(M):
+            n = len(holds[e][m])
+            spill = n > 0 and int(hv[e, m]) * den * P > num * n * total
+            n_spill += bool(spill and (j // Ns) // R != m)
+            if (j // Ns) // R == m or n == 0 or spill:
+                exp[j * M + m] = e * M + m
+    assert n_spill > 0
+    dev = G.DEV
+    st = torch.zeros(1, dtype=torch.int32, device=dev)
+    out = torch.full((1, 1, S * M), -7, dtype=torch.int32, device=dev)
+    fm.local_placement_theta(shape, M, num, den, torch.as_tensor(hv.astype(np.int32)).reshape(1, 1, E * M).to(dev),
+                             torch.as_tensor(se).to(dev), out, st)
+    torch.cuda.synchronize()
+    assert int(st.item()) == 0
+    got = out.cpu().numpy().ravel()
+    assert (got == exp).all(), np.argwhere(got != exp)[:5].tolist()

@@ -180,6 +180,14 @@ def _stream() -> int:
     return torch.cuda.current_stream().cuda_stream
 
 
+def _stream_on(dev_index: int) -> int:
+    """cudaStream_t of torch's current stream on device ``dev_index`` (DataPath: the plan's device);
+    falls back to the public API when the torch build lacks the raw getter, like ``_stream``."""
+    if _raw_stream is not None:
+        return _raw_stream(dev_index)
+    return torch.cuda.current_stream(dev_index).cuda_stream
+
+
 def _check(fn: str, rc: int) -> None:
     if rc != OK:
         raise ForeMoEError(fn, rc)
@@ -331,13 +339,13 @@ class DataPath:
     def dispatch(self, layer: int, mb_begin: int, mb_end: int, x, perm, buf) -> None:
         rc = self._dispatch(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._act_ptr(x),
                             None if perm is None else _dev(perm, torch.int32), self._act_ptr(buf), self._st,
-                            _raw_stream(self._dev_index))
+                            _stream_on(self._dev_index))
         if rc:
             raise ForeMoEError("foremoe_dispatch", rc)
 
     def combine(self, layer: int, mb_begin: int, mb_end: int, expert_out, y) -> None:
         rc = self._combine(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._w,
-                           self._act_ptr(expert_out), self._f32_ptr(y), self._st, _raw_stream(self._dev_index))
+                           self._act_ptr(expert_out), self._f32_ptr(y), self._st, _stream_on(self._dev_index))
         if rc:
             raise ForeMoEError("foremoe_combine", rc)
 
@@ -345,13 +353,13 @@ class DataPath:
         rc = self._combine_bwd(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._w,
                                self._f32_ptr(dy), None if expert_out is None else self._act_ptr(expert_out),
                                self._act_ptr(d_expert_out), None if dw is None else self._f32_ptr(dw),
-                               self._st, _raw_stream(self._dev_index))
+                               self._st, _stream_on(self._dev_index))
         if rc:
             raise ForeMoEError("foremoe_combine_bwd", rc)
 
     def dispatch_bwd(self, layer: int, mb_begin: int, mb_end: int, d_buf, dx) -> None:
         rc = self._dispatch_bwd(self._sp, layer, mb_begin, mb_end, self._mb, self._inv, self._act_ptr(d_buf),
-                                self._f32_ptr(dx), self._st, _raw_stream(self._dev_index))
+                                self._f32_ptr(dx), self._st, _stream_on(self._dev_index))
         if rc:
             raise ForeMoEError("foremoe_dispatch_bwd", rc)
 

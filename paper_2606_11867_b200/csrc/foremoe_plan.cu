@@ -932,9 +932,12 @@ extern "C" __attribute__((visibility("default"))) int foremoe_assign(const forem
   Dims d;
   int rc = make_dims(shape, &d);
   if (rc) return rc;
-  if ((!ids && d.T > 0) || !mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
+  if (!mb_off || !hist || !slot_expert || !quota || !rank_load || !slot_off || !workspace)
     return FOREMOE_ERR_INVALID_ARG;
   if ((pair_slot == nullptr) != (inv == nullptr)) return FOREMOE_ERR_INVALID_ARG;
+  // the ids are read only to assign the pairs: quota-only calls (pair_slot = inv = NULL) and steps
+  // without tokens may pass ids = NULL, as the header says
+  if (!ids && d.T > 0 && pair_slot) return FOREMOE_ERR_INVALID_ARG;
   return launch_assign(d, ids, mb_off, hist, nullptr, nullptr, slot_expert, quota_in, quota, rank_load,
                        slot_off, pair_slot, inv, workspace, workspace_bytes, dev_status, (cudaStream_t)stream);
 }

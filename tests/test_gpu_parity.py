@@ -494,6 +494,66 @@ def test_graph_capture_of_first_call_after_warmup(cuda_device):
     assert r.returncode == 0 and "capture-first-call ok" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])
 
 
+_CAPTURE_TWO_SHAPES = r"""
+import dataclasses, sys, numpy as np, torch
+sys.path.insert(0, sys.argv[1])
+from paper_2606_11867_b200 import binding as fm, synth
+from tests import gpu_common as G
+base = synth.config(2).scaled(L=1, n_samples=4, sample_len=300, H=1024, mb_samples=2)
+plans = []
+for K in (3, 5, 7):          # no kernel is specialised for these K: the three shapes share the generic
+    cfg = dataclasses.replace(base, K=K)          # instantiations and differ only in shared-memory size
+    ids, w, mb_off, se = G.make_case(cfg)
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    n = int(mb_off[1] - mb_off[0])
+    plans.append((sp, n, synth.gen_activations(cfg, n, 0, G.DEV), torch.randn((n, cfg.H), device=G.DEV)))
+def mk(sp, n):
+    s = sp.shape
+    return (torch.zeros((n * s.K,), dtype=torch.int32, device=G.DEV),
+            torch.zeros((n * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV),
+            torch.zeros((n, s.H), dtype=torch.float32, device=G.DEV),
+            torch.zeros((n * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV),
+            torch.zeros((n, s.H), dtype=torch.float32, device=G.DEV),
+            torch.zeros((s.L, s.T, s.K), dtype=torch.float32, device=G.DEV))
+def run(sp, x, dy, b):
+    perm, buf, y, d_buf, dx, dw = b
+    sp.dispatch(0, 0, 1, x, perm, buf)
+    sp.combine(0, 0, 1, buf, y)
+    sp.combine_bwd(0, 0, 1, dy, buf, d_buf, dw)
+    sp.dispatch_bwd(0, 0, 1, d_buf, dx)
+for sp, n, x, dy in plans:
+    fm.warmup(sp.shape)          # all three warmed BEFORE anything is captured
+graphed = [mk(sp, n) for sp, n, x, dy in plans]
+torch.cuda.synchronize()
+g = torch.cuda.CUDAGraph()
+with torch.cuda.graph(g):
+    for (sp, n, x, dy), b in zip(plans, graphed):
+        run(sp, x, dy, b)        # first data-path calls of the process, first shape first
+g.replay()
+torch.cuda.synchronize()
+for (sp, n, x, dy), b in zip(plans, graphed):
+    e = mk(sp, n)
+    run(sp, x, dy, e)
+    torch.cuda.synchronize()
+    for u, v in zip(e, b):
+        assert torch.equal(u.view(torch.uint8), v.view(torch.uint8))
+    assert sp.faults() == 0
+print("capture-two-shapes ok")
+"""
+
+
+def test_graph_capture_after_warming_several_shapes(cuda_device):
+    """Warming a second and third shape that select the same kernel instantiations must not push the
+    first shape's launch facts out of the per-device memo: all three are then captured from their very
+    first call (a miss would query occupancy / set the shared-memory attribute during capture).  The memo
+    itself is checked on the host by tests/test_abi.py (memo_check.cu); this is the end-to-end use."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _CAPTURE_TWO_SHAPES, root], capture_output=True, text=True,
+                       cwd=root, timeout=600)
+    assert r.returncode == 0 and "capture-two-shapes ok" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])
+
+
 def test_cuda_graph_replay(cuda_device):
     """The data-path calls are capturable into a CUDA graph once each kernel variant has run eagerly
     (the first launch of a variant queries occupancy / opts into large shared memory); the replay
@@ -642,3 +702,46 @@ def test_fuzz_data_path_shapes(cuda_device):
              for i in range(n_mb)}
         G.check_data_path(sp, ref, x, range(L), range(n_mb), str(shape))
         done += 1
+
+
+def test_quota_only_assign_takes_no_ids(cuda_device):
+    """foremoe_assign with pair_slot = inv = NULL computes the quotas only and does not read the ids
+    (include/foremoe.h): ids = NULL is accepted and gives the quotas of the full call."""
+    cfg = synth.config(2).scaled(L=2, n_samples=6, sample_len=500, H=256, mb_samples=2)
+    ids, w, mb_off, se = G.make_case(cfg)
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    q, rl, so = (torch.full_like(t, -9) for t in (sp.quota, sp.rank_load, sp.slot_off))
+    fm.assign(sp.shape, None, sp.mb_off, sp.hist, sp.slot_expert, None, q, rl, so, None, None, sp.workspace, sp.status)
+    torch.cuda.synchronize()
+    assert torch.equal(q, sp.quota) and torch.equal(rl, sp.rank_load) and torch.equal(so, sp.slot_off)
+    assert sp.faults() == 0
+    with pytest.raises(fm.ForeMoEError):           # assigning the pairs does need them
+        fm.assign(sp.shape, None, sp.mb_off, sp.hist, sp.slot_expert, None, q, rl, so, sp.pair_slot, sp.inv,
+                  sp.workspace, sp.status)
+
+
+def test_data_path_without_torchs_raw_stream_getter(cuda_device, monkeypatch):
+    """binding.DataPath on a torch build that lacks torch._C._cuda_getCurrentRawStream: the public
+    current_stream() is used instead, on a side stream too, with the same results."""
+    cfg = synth.config(2).scaled(L=1, n_samples=4, sample_len=300, H=512, mb_samples=2)
+    ids, w, mb_off, se = G.make_case(cfg)
+    sp = G.gpu_plan(fm.shape_of(cfg), ids, w, mb_off, se)
+    s, n = sp.shape, int(mb_off[1] - mb_off[0])
+    x = synth.gen_activations(cfg, n, 0, G.DEV)
+    mk = lambda: (torch.zeros((n * s.K,), dtype=torch.int32, device=G.DEV),
+                  torch.zeros((n * s.K, s.H), dtype=s.act_torch_dtype, device=G.DEV),
+                  torch.zeros((n, s.H), dtype=torch.float32, device=G.DEV))
+    ref = mk()
+    sp.dispatch(0, 0, 1, x, ref[0], ref[1])
+    sp.combine(0, 0, 1, ref[1], ref[2])
+    torch.cuda.synchronize()
+    monkeypatch.setattr(fm, "_raw_stream", None)
+    got = mk()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        assert fm._stream_on(0) == side.cuda_stream == fm._stream()
+        sp.dispatch(0, 0, 1, x, got[0], got[1])
+        sp.combine(0, 0, 1, got[1], got[2])
+    torch.cuda.synchronize()
+    for a, b in zip(ref, got):
+        assert torch.equal(a.view(torch.uint8), b.view(torch.uint8))

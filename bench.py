@@ -658,10 +658,83 @@ def run_ours(args, cfg) -> None:
             line["cpu_baseline"]["all_cores"] = oracle_all_cores(cfg, max(1, n_samp // 4))
         if verify is not None:
             line["verified"] = verify_against_oracle(*verify)
+    headline = (args.config == 2 and args.mb_samples is None and not args.layers and not upd and not args.machines
+                and args.planner == "stage4" and args.mb_per_call == 1 and not args.graph and args.streams == 1
+                and not args.tune and not args.strict_order)
+    if rank == 0 and world == 1 and headline and not args.no_other_configs:
+        del wl
+        torch.cuda.empty_cache()
+        line["other_configs"] = run_other_configs(args, dev, physical_gpu_index(local_rank), peak)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         torch.distributed.destroy_process_group()
+
+
+OTHER_CONFIGS = [(1, None), (3, None), (5, None), (4, 1), (4, 8), (4, 64)]     # (BASELINE.json config, samples per micro-step)
+
+
+def run_other_config(cfg, dev, gpu_index: int, peak: float, steps: int, warmup: int, probe_stride: int) -> dict:
+    """One of the non-headline configs of BASELINE.json, timed like the headline (warm-up, CUDA events around
+    `steps` whole steps of foremoe_plan + dispatch + combine of every instance, clocks sampled during the
+    timed region, one instance of the timed configuration checked against the oracle afterwards), reported
+    as a compact record.  Runs after the headline's timed region and legs, on released memory."""
+    wl = Workload(cfg, dev)
+    bpt = bytes_per_token(cfg)
+    for _ in range(warmup):
+        wl.step()
+    torch.cuda.synchronize()
+    assert wl.plan.faults() == 0
+    probes = {"plan": [], "dispatch": [], "combine": [], "combine_bwd": [], "dispatch_bwd": [], "run": []}
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    with ClockSampler(gpu_index) as clk:
+        e0.record()
+        for _ in range(steps):
+            wl.step(probes, probe_stride)
+        e1.record()
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    assert wl.plan.faults() == 0
+    value = wl.routed_tokens * steps / (ms * 1e-3)
+    bpt["run"] = bpt["total"] - bpt["plan"]
+    kern = probe_stats(probes, bpt)
+    kern.pop("run", None)
+    rl = wl.plan.rank_load.float()
+    live = rl.sum(-1) > 0
+    ratio = (rl.max(-1).values / rl.mean(-1).clamp(min=1e-9))[live]
+    nat = wl.plan.hist.float().view(cfg.n_mb, cfg.L, cfg.P, cfg.Nb).sum(-1)
+    nratio = (nat.max(-1).values / nat.mean(-1).clamp(min=1e-9))[live]
+    out = {"workload": workload_name(cfg), "value": value, "unit": UNIT, "steps": steps, "warmup": warmup,
+           "ms_per_step": ms / steps, "dtype": "bf16" if cfg.act_dtype == synth.ACT_BF16 else "f32",
+           "bytes_per_routed_token": bpt["total"], "whole_path_gbs": value * bpt["total"] / 1e9,
+           "whole_path_frac": value * bpt["total"] / 1e9 / peak,
+           "gpu_launches": wl.launches_per_step * steps,
+           "kernels": {k: {"avg_ms": v["avg_ms"], "gbs": v["gbs"], "frac": v["gbs"] / peak,
+                           "launches_timed": v["launches_timed"]} for k, v in kern.items()},
+           "balance": {"lmax_over_lmean": {"max": float(ratio.max()), "mean": float(ratio.mean()),
+                                           "median": float(ratio.median())},
+                       "natural_placement": {"max": float(nratio.max()), "mean": float(nratio.mean()),
+                                             "median": float(nratio.median())}},
+           "clocks": clk.summary()}
+    verify = capture_instance(wl, wl.instances[len(wl.instances) // 2])
+    wl.release()
+    out["verified"] = verify_against_oracle(*verify)
+    return out
+
+
+def run_other_configs(args, dev, gpu_index: int, peak: float) -> dict:
+    """north_star names five configs and a micro-step size sweep "at each size": the default run reports them
+    all.  A failure in one of them is recorded in its entry and never costs the headline line."""
+    out = {}
+    for cfg_id, mb in OTHER_CONFIGS:
+        key = str(cfg_id) if mb is None else f"{cfg_id}@{mb}"
+        try:
+            cfg = synth.config(cfg_id, mb_samples=mb)
+            out[key] = run_other_config(cfg, dev, gpu_index, peak, max(2, min(args.steps, 3)), 3, args.probe_stride)
+        except Exception as e:      # noqa: BLE001 -- report, do not lose the headline
+            out[key] = {"error": f"{type(e).__name__}: {e}"[:300]}
+        torch.cuda.empty_cache()
+    return out
 
 
 TUNING_KEYS = ["dispatch_impl", "dispatch_u", "dispatch_cta_per_sm", "dispatch_stages", "dispatch_warps",
@@ -723,6 +796,9 @@ def main() -> None:
                          "the plan arrays, before the preceding kernel of the stream has completed")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the records of configs 1, 3, 5 and the config-4 size sweep that the default "
+                         "(config 2, 1 GPU) run appends under other_configs after the headline's legs")
     ap.add_argument("--no-cpu-all-cores", action="store_true",
                     help="skip the all-cores leg of cpu_baseline (one oracle process per host core)")
     ap.add_argument("--tune", default="",

@@ -231,7 +231,9 @@ static int launch_depth(int D, const Dims &d, int threads, const int32_t *inv_l,
   switch (D) {
     case 2: return launch_one<kBf16, K_T, 2, kDw>(FOREMOE_ARGS);
     case 3: return launch_one<kBf16, K_T, 3, kDw>(FOREMOE_ARGS);
+#ifdef FOREMOE_TUNING      // combine_bwd_rows picks D = 3 (with dw) or 2
     case 4: return launch_one<kBf16, K_T, 4, kDw>(FOREMOE_ARGS);
+#endif
   }
   return FOREMOE_ERR_INVALID_ARG;
 }

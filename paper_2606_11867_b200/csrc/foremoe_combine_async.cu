@@ -7,6 +7,8 @@
 // each of the K rows, reads back exactly the bytes it copied (no cross-lane hazard on the data).
 #include "foremoe_data.cuh"
 
+#ifdef FOREMOE_TUNING   // sweep alternative to the bulk-copy ring (combine_impl = 1): not in the product library
+
 namespace foremoe {
 
 // 16-byte cp.async whose source size is 0 when the row is absent: the destination is zero-filled
@@ -226,3 +228,5 @@ int launch_combine_async(const Dims &d, const int32_t *inv_l, const float *w_l,
 #undef FOREMOE_ARGS
 
 }  // namespace foremoe
+
+#endif  // FOREMOE_TUNING

@@ -223,8 +223,10 @@ static int launch_u(int U, const Dims &d, int warps, int D, const int32_t *inv_l
   switch (U) {
     case 1: return launch_one<kBf16, K_T, 1>(d, warps, D, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
     case 2: return launch_one<kBf16, K_T, 2>(d, warps, D, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+#ifdef FOREMOE_TUNING      // launch_combine_bulk's auto rule picks U = 1 or 2
     case 4: return launch_one<kBf16, K_T, 4>(d, warps, D, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
     case 8: return launch_one<kBf16, K_T, 8>(d, warps, D, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+#endif
   }
   return FOREMOE_ERR_INVALID_ARG;
 }

@@ -57,6 +57,7 @@ k_dispatch_rows(const int32_t *__restrict__ inv_l, const int32_t *__restrict__ m
   }
 }
 
+#ifdef FOREMOE_TUNING   // the register-staged LSU combine: a sweep alternative, not selected by the product build
 // =============================================================================================
 // a6: combine.  y[t][h] = sum_k w[t][k] * float(eo[inv[t*K+k]][h]), fp32 fma, k ascending from
 // acc = 0 (order / fma / fp32 output = DESIGN.md reading 16).
@@ -152,6 +153,8 @@ k_combine_rows(const int32_t *__restrict__ inv_l, const float *__restrict__ w_l,
   }
 }
 
+#endif  // FOREMOE_TUNING
+
 // ---- launch configuration -------------------------------------------------------------------------
 #ifdef FOREMOE_TUNING
 DataTuning g_tune;
@@ -184,6 +187,7 @@ static int launch_dispatch(const Dims &d, const int32_t *inv_l, const int32_t *m
   return e == cudaSuccess ? FOREMOE_OK : FOREMOE_ERR_CUDA;
 }
 
+#ifdef FOREMOE_TUNING
 template <bool kBf16, int KB, int U>
 static int launch_combine(const Dims &d, const int32_t *inv_l, const float *w_l,
                           const int32_t *mb_off, int mb_begin, int mb_end, const void *eo, float *y,
@@ -222,6 +226,8 @@ static int launch_combine_kb(int KB, int U, const Dims &d, const int32_t *inv_l,
   return FOREMOE_ERR_INVALID_ARG;
 }
 
+#endif  // FOREMOE_TUNING
+
 static int check_range(const Dims &d, int layer, int mb_begin, int mb_end) {
   if (layer < 0 || layer >= d.L || mb_begin < 0 || mb_end > d.n_mb || mb_begin > mb_end)
     return FOREMOE_ERR_INVALID_ARG;
@@ -240,8 +246,10 @@ int dispatch_rows(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, in
   }
   int U = g_tune.dispatch_u;
   if (U <= 0) U = d.row_vec >= 64 ? 2 : 1;      // 1 KB slices: best or within 1 % of best on every config (sweep)
+#ifdef FOREMOE_TUNING      // the auto rule above picks 1 or 2: wider slices exist for sweeps only
   if (U >= 8) return launch_dispatch<8>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
   if (U >= 4) return launch_dispatch<4>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
+#endif
   if (U >= 2) return launch_dispatch<2>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
   return launch_dispatch<1>(d, inv_l, mb_off, mb_begin, mb_end, x, perm, buf, st, prepare);
 }
@@ -249,6 +257,11 @@ int dispatch_rows(const Dims &d, const int32_t *inv_l, const int32_t *mb_off, in
 // a6 and its unit-weight form (w_l == nullptr sums the K rows: fma(1, v, acc) = acc + v exactly)
 int combine_rows(const Dims &d, const int32_t *inv_l, const float *w_l, const int32_t *mb_off,
                  int mb_begin, int mb_end, const void *eo, float *y, cudaStream_t st, bool prepare) {
+#ifndef FOREMOE_TUNING
+  // The bulk-copy ring stages 512-byte slices, so it fits every legal shape (K = 32: 2 warps x 2 stages of
+  // 32 x 512 B = 66 KB) and is the only combine kernel in the product library.
+  return launch_combine_bulk(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+#else
   int rc;
   if (g_tune.combine_impl < 0 || g_tune.combine_impl == 2) {   // default: bulk-copy ring
     rc = launch_combine_bulk(d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
@@ -265,6 +278,7 @@ int combine_rows(const Dims &d, const int32_t *inv_l, const float *w_l, const in
   if (d.act_dtype == FOREMOE_ACT_BF16)
     return launch_combine_kb<true>(KB, U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
   return launch_combine_kb<false>(KB, U, d, inv_l, w_l, mb_off, mb_begin, mb_end, eo, y, st, prepare);
+#endif
 }
 
 }  // namespace foremoe

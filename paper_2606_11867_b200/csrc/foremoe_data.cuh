@@ -23,7 +23,7 @@ struct DataTuning {
   int pdl = 1;                   // programmatic dependent launch on the data-path kernels
   int bwd_depth = 0;             // k_combine_bwd: stages in flight per thread (0 = auto)
   int bwd_cta_per_sm = 0;        // 0 = auto
-  int bwd_impl = -1;             // -1 auto, 1 = cp.async ring, 2 = bulk-copy ring
+  int bwd_impl = -1;             // reserved: k_combine_bwd has one implementation (cp.async ring); the value is ignored
   int hist_variant = 2;          // k_load_hist: 0 = 4-byte loads, 1 = warp-aggregated, 2 = 16-byte loads
 };
 #ifdef FOREMOE_TUNING

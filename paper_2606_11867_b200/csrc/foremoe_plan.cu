@@ -833,6 +833,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const fo
     const long long n_tiles = (long long)tiles_per_layer * d.L;
     const int grid = (int)(n_tiles < (long long)num_sms() * 8 ? n_tiles : (long long)num_sms() * 8);
     const size_t smem = sizeof(int32_t) * d.E;
+#ifdef FOREMOE_TUNING      // variants 0 / 1 lost the sweep (profiles/r01_hist.md) and exist there only
     if (g_tune.hist_variant == 1)
       k_load_hist<1><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
                                               tiles_per_layer, hist, dev_status);
@@ -840,6 +841,7 @@ extern "C" __attribute__((visibility("default"))) int foremoe_load_hist(const fo
       k_load_hist<0><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
                                               tiles_per_layer, hist, dev_status);
     else
+#endif
       k_load_hist<2><<<grid, 256, smem, st>>>(ids, mb_off, d.L, d.T, d.K, d.E, d.n_mb, tile_tokens,
                                               tiles_per_layer, hist, dev_status);
   }
